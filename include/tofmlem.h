@@ -1,0 +1,170 @@
+/*
+ * tofmlem.h -- C ABI of libtofmlem: list-mode TOF-weighted MLEM hot path on one NVIDIA B200 (sm_100a).
+ *
+ * Source of every operation: arxiv 1706.07075 ("PAPER.md" = /root/reference/PAPER.md) as read in
+ * DESIGN.md (readings R1..R22).  The paper states the problem in prose only (events with a TOF time
+ * difference -> image by TOF-weighted list-mode MLEM; nine-region TOF-assisted
+ * data division); the call list follows BASELINE.json's north_star.
+ *
+ * Conventions
+ *   - Units: millimetres and picoseconds.  Scanner = cylinder of radius R and axial length A around the
+ *     z axis, centred at the origin.  Image layout: flat index = (iz*ny + iy)*nx + ix (x fastest), float32.
+ *   - An event is two detection points p1, p2 (mm) and dt = t1 - t2 (ps); dt > 0 puts the annihilation
+ *     nearer p2 (the TOF kernel centre is at arc length L/2 + c*dt/2 from p1).
+ *     Events are struct-of-arrays float32.
+ *   - Pointers named d_* and the members of tofmlem_events are DEVICE pointers, pointers named h_* are
+ *     HOST pointers.  All buffers are owned by the caller; the library never frees or reallocates them.
+ *     The only library-owned objects are the opaque context and its internal scratch.
+ *   - Every call enqueues work on the CUDA stream given at tofmlem_create and returns without
+ *     synchronising, unless stated otherwise.  A context must not be used from two host threads at once.
+ *   - Return value: TOFMLEM_OK (0) or a negative tofmlem_status.  No exceptions, no exit().
+ *     After TOFMLEM_ECUDA the text of the CUDA error is available from tofmlem_last_error().
+ *   - System matrix (north_star; R2,R4-R8): a_ej = l_ej * g_sigma(s_mid,ej - s_c,e) with l_ej the
+ *     exact (Siddon) chord of LOR e in voxel j clipped to the window [s_c - T sigma, s_c + T sigma] n grid
+ *     n [0, L], g the unit-area Gaussian evaluated at the clipped chord's midpoint, T = trunc_sigmas = 3,
+ *     sigma = c * FWHM / (2 * 2 sqrt(2 ln 2)).  Non-TOF contexts use a_ej = l_ej.
+ *   - Arithmetic: per-event ray set-up in fp64, per-voxel stepping/weights/accumulation in fp32,
+ *     accumulation into images with float32 atomics (order not deterministic).  Bin keys and region
+ *     ids follow the float32 specification F1 of DESIGN.md and are bit-exact.
+ */
+#ifndef TOFMLEM_H
+#define TOFMLEM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TOFMLEM_OK = 0,
+    TOFMLEM_EINVAL = -1,       /* NULL / out-of-range argument */
+    TOFMLEM_ENOMEM = -2,       /* device or host allocation failed */
+    TOFMLEM_ECUDA = -3,        /* a CUDA call failed; see tofmlem_last_error */
+    TOFMLEM_ESTATE = -4,       /* call not valid in the context's current state */
+    TOFMLEM_EUNSUPPORTED = -5  /* option or mode not available */
+} tofmlem_status;
+
+typedef struct tofmlem_ctx tofmlem_ctx; /* opaque, owned by the library */
+
+typedef struct { float radius_mm, axial_length_mm; } tofmlem_scanner;
+
+typedef struct {
+    int32_t nx, ny, nz;
+    float vx, vy, vz;  /* voxel size, mm */
+    float ox, oy, oz;  /* mm coordinate of the low corner of voxel (0,0,0) */
+} tofmlem_grid;
+
+/* Struct-of-arrays events (float32, n entries each).  dt may be NULL for LOR-only use
+ * (sensitivity LORs, non-TOF contexts); then dt = 0 is assumed. */
+typedef struct { const float *x1, *y1, *z1, *x2, *y2, *z2, *dt; } tofmlem_events;
+typedef struct { float *x1, *y1, *z1, *x2, *y2, *z2, *dt; } tofmlem_events_mut;
+
+typedef struct {
+    uint64_t n_valid;      /* events with forward projection > 0 in the last EM pass (R9) */
+    uint64_t n_skipped;    /* n - n_valid of that pass */
+    uint64_t visits;       /* voxel visits of the forward walk of that pass */
+    double sum_image_sens; /* sum_j image_j * sens_j after the last tofmlem_iterate (= n_valid, P7) */
+} tofmlem_stats;
+
+/* Option keys for tofmlem_set_option. */
+enum {
+    TOFMLEM_OPT_TRUNC_SIGMAS = 1,   /* half-width of the TOF window in sigmas, default 3.0 (R5) */
+    TOFMLEM_OPT_SENS_FLOOR_REL = 2, /* mask_j = sens_j >= value * max(sens), default 1e-2 (R11) */
+    TOFMLEM_OPT_TILE_LOG2 = 3,      /* locality bins are cubes of 2^value voxels, default 3 */
+    TOFMLEM_OPT_PROJECTOR = 4,      /* 0 = Siddon x Gaussian (default); 1 = paper's K-sample LUT */
+    TOFMLEM_OPT_SAMPLES_K = 5,      /* K of the sampled projector, default 32 */
+    TOFMLEM_OPT_SHELL_MM = 6        /* extra shell added to the region margin, default 6 mm */
+};
+
+/* Create a context.  tof_fwhm_ps <= 0 makes a non-TOF context (full-chord traversal).
+ * cuda_stream is a cudaStream_t (NULL = default stream) on the current device; every later call with
+ * this context enqueues there.  Errors: EINVAL (NULL, non-positive sizes), ENOMEM, ECUDA. */
+int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, float tof_fwhm_ps,
+                   void *cuda_stream, tofmlem_ctx **out);
+/* Synchronises the stream, frees internal scratch and the context.  NULL is allowed. */
+int tofmlem_destroy(tofmlem_ctx *ctx);
+int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value);
+/* sigma along the LOR in mm for this context (0 for non-TOF). */
+double tofmlem_sigma_mm(const tofmlem_ctx *ctx);
+
+/* Sensitivity image (north_star; R10): d_sens[j] = (1/m) sum_i l_ij over m detector-pair LORs
+ * (non-TOF chords over the whole grid).  d_sens (nvox floats) is overwritten.  lors->dt is ignored. */
+int tofmlem_sensitivity(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t m, float *d_sens);
+
+/* TOF-weighted forward projection: d_fwd[e] = sum_j a_ej d_image[j], n floats.
+ * Skipped events (non-finite fields, L = 0, empty window) give 0. */
+int tofmlem_forward(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_fwd);
+
+/* TOF-weighted backprojection ("direct voxel filling"; the paper's "starting
+ * backprojection", :247, is d_values = NULL): d_out[j] += a_ej * d_values[e] (NULL => 1).
+ * d_out (nvox floats) is accumulated into; the caller zeroes it. */
+int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_values, float *d_out);
+
+/* One fused forward+back EM pass (R1, R9): d_corr[j] += sum_{e: fwd_e > 0} a_ej / fwd_e with
+ * fwd_e = sum_k a_ek d_image[k].  d_corr is accumulated into (caller zeroes it), so that a data set can be
+ * passed in several calls or its partial corrections summed across GPUs before tofmlem_update.
+ * Updates the context's n_valid / visits counters (reset them with tofmlem_reset_stats). */
+int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr);
+int tofmlem_reset_stats(tofmlem_ctx *ctx);
+
+/* Multiplicative update (R1, R11): d_image[j] = mask_j ? d_image[j] * d_corr[j] / d_sens[j] : 0 with
+ * mask_j = d_sens[j] >= sens_floor_rel * max_k d_sens[k] (and d_sens[j] > 0), decided in float32.
+ * d_corr is zeroed afterwards (ready for the next pass). */
+int tofmlem_update(tofmlem_ctx *ctx, float *d_image, float *d_corr, const float *d_sens);
+
+/* `iters` MLEM iterations: for each, zero the internal correction image, one fused EM pass
+ * over all n events, multiplicative update.  d_image: in x0, out x_iters.  d_image and d_sens must not alias.
+ * n <= 2^32 - 1. */
+int tofmlem_iterate(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, float *d_image, const float *d_sens,
+                    int iters);
+
+/* Same as tofmlem_iterate with HOST buffers (pinned memory recommended): uploads the events in chunks
+ * overlapped with the first pass, the image and the sensitivity, runs `iters` iterations and downloads
+ * the image.  SYNCHRONISES before returning.  h_events members are host pointers here. */
+int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_events, uint64_t n, float *h_image,
+                         const float *h_sens, int iters);
+
+/* Locality binning (north_star bullet 1; specification F1 in DESIGN.md): key = dirclass * T + tile of the
+ * TOF kernel centre (12 direction classes x cubes of 2^tile_log2 voxels); invalid events get 0xFFFFFFFF.
+ * d_key[n] receives the keys (input order); d_perm[n] a permutation that sorts events by key (order inside
+ * a bin unspecified; invalid events last); d_bin_offsets (bins+1 entries, may be NULL) the start of each
+ * bin in d_perm, with d_bin_offsets[bins] = number of valid events. */
+int tofmlem_bin_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, uint32_t *d_key, uint32_t *d_perm,
+                       uint32_t *d_bin_offsets);
+uint32_t tofmlem_num_bins(const tofmlem_ctx *ctx);
+/* out[i] = in[d_perm[i]] for every member (dt skipped if either dt pointer is NULL).  in/out must not alias. */
+int tofmlem_gather_events(tofmlem_ctx *ctx, const tofmlem_events *in, const uint32_t *d_perm, uint64_t n,
+                          const tofmlem_events_mut *out);
+
+/* TOF-assisted data division (R12, R13): d_region[e] = #{ j in 1..R-1 : zb[j] <= cz_e } with
+ * cz_e the z of the TOF kernel centre (float32, F1); invalid events get -1.  h_zbounds: n_regions+1 ascending
+ * HOST floats, or NULL for the paper's partition (first region double width: "200 + 8 x 100").
+ * d_perm groups event indices by region (invalid last; order inside a region unspecified); h_counts
+ * (HOST, n_regions entries) is valid on return (this call SYNCHRONISES). n_regions <= 64. */
+int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                          const float *h_zbounds, int32_t *d_region, uint32_t *d_perm, uint64_t *h_counts);
+/* Default boundaries zb[j] = (float)k_j * vz + oz, k_j = nz * {0,2,3,..,R+1} / (R+1) (integer division). */
+int tofmlem_region_zbounds(const tofmlem_ctx *ctx, int n_regions, float *h_zbounds);
+/* Sub-grid of region r: its core slices plus ceil((trunc_sigmas*sigma + shell_mm)/vz) slices on each side,
+ * clamped to the volume (R12).  *z0,*z1 = slice range [z0, z1) in the parent volume. */
+int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zbounds, int r, tofmlem_grid *sub,
+                        int32_t *z0, int32_t *z1);
+/* Whole cfg-4 pipeline: split, gather each region's events, reconstruct every region independently on its
+ * own sub-grid and CUDA stream (`iters` iterations from x0 = mask), and SUM the extended region images into
+ * d_image_out (nvox floats, overwritten) as the paper does.  SYNCHRONISES. */
+int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                                const float *h_zbounds, float *d_image_out, const float *d_sens, int iters);
+
+/* Copies the counters of the last pass to *h_out.  SYNCHRONISES the context's stream. */
+int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out);
+/* Text of the last error of this context ("" if none).  Valid until the next call on the context. */
+const char *tofmlem_last_error(const tofmlem_ctx *ctx);
+/* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches). */
+uint64_t tofmlem_launch_count(const tofmlem_ctx *ctx);
+const char *tofmlem_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TOFMLEM_H */

@@ -1,0 +1,8 @@
+"""paper_1706_07075_b200 -- B200-native list-mode TOF-MLEM hot path (arxiv 1706.07075).
+
+`csrc/` holds the hand-written sm_100a CUDA kernels and the C ABI (include/tofmlem.h);
+`tofmlem.py` is the ctypes binding (argument marshalling only); `build.py` compiles libtofmlem.so in-tree.
+"""
+from .tofmlem import (Context, Events, Grid, Scanner, Stats, TofMlemError, lib, make_grid, version,  # noqa: F401
+                      OPT_PROJECTOR, OPT_SAMPLES_K, OPT_SENS_FLOOR_REL, OPT_SHELL_MM, OPT_TILE_LOG2,
+                      OPT_TRUNC_SIGMAS, SYMBOLS, EVENT_FIELDS)

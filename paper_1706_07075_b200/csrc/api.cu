@@ -1,0 +1,657 @@
+// api.cu -- the C ABI of libtofmlem (include/tofmlem.h): context, argument checks, stream orchestration.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "internal.cuh"
+
+using namespace tofmlem;
+
+struct tofmlem_ctx {
+    tofmlem_scanner scanner;
+    tofmlem_grid grid;
+    bool tof;
+    double sigma;  // mm
+    double trunc_sigmas = 3.0, sens_floor_rel = 1e-2, shell_mm = 6.0;
+    int tile_log2 = 3, projector = 0, samples_k = 32;
+    cudaStream_t stream = nullptr;
+    uint64_t nvox = 0;
+    // scratch owned by the context
+    float *d_corr = nullptr;
+    float *d_max = nullptr;          // max(sens) of the current iterate call
+    const float *d_max_ext = nullptr;  // region sub-contexts use the parent's global max
+    DeviceStats *d_stats = nullptr;
+    uint32_t *d_hist = nullptr, *d_cursor = nullptr;
+    size_t hist_cap = 0;
+    unsigned long long *d_rcounts = nullptr;  // 2*(kMaxRegions+1)
+    // host-buffer path
+    float *d_hev = nullptr;
+    size_t hev_cap = 0;
+    float *d_himg = nullptr, *d_hsens = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t chunk_done[2] = {nullptr, nullptr};
+    uint64_t last_n = 0;
+    uint64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(tofmlem_ctx *c, int code, const char *what) {
+    if (c) c->err = what ? what : "";
+    return code;
+}
+
+int cuda_fail(tofmlem_ctx *c, cudaError_t e, const char *where) {
+    if (c) {
+        char buf[512];
+        snprintf(buf, sizeof buf, "%s: %s (%s)", where, cudaGetErrorString(e), cudaGetErrorName(e));
+        c->err = buf;
+    }
+    return e == cudaErrorMemoryAllocation ? TOFMLEM_ENOMEM : TOFMLEM_ECUDA;
+}
+
+#define CU(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);  \
+    } while (0)
+
+#define CHECK_LAUNCH(k)                                                       \
+    do {                                                                      \
+        cudaError_t e_ = cudaGetLastError();                                  \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, "kernel launch");    \
+        ctx->launches += (k);                                                 \
+    } while (0)
+
+double sigma_from_fwhm(double fwhm_ps) { return kCmmPerPs * fwhm_ps / (2.0 * 2.0 * sqrt(2.0 * log(2.0))); }
+
+ProjParams make_params(const tofmlem_ctx *c, bool tof) {
+    ProjParams p;
+    const tofmlem_grid &g = c->grid;
+    p.nx = g.nx; p.ny = g.ny; p.nz = g.nz;
+    p.vx = g.vx; p.vy = g.vy; p.vz = g.vz;
+    p.ivx = 1.0 / p.vx; p.ivy = 1.0 / p.vy; p.ivz = 1.0 / p.vz;
+    p.ox = g.ox; p.oy = g.oy; p.oz = g.oz;
+    p.hx = p.ox + p.nx * p.vx; p.hy = p.oy + p.ny * p.vy; p.hz = p.oz + p.nz * p.vz;
+    if (tof) {
+        p.half_window = c->trunc_sigmas * c->sigma;
+        p.gauss_a = (float)(-1.4426950408889634 / (2.0 * c->sigma * c->sigma));
+        p.gauss_norm = (float)(1.0 / (c->sigma * sqrt(2.0 * M_PI)));
+    } else {
+        p.half_window = 0.0;
+        p.gauss_a = 0.0f;
+        p.gauss_norm = 1.0f;
+    }
+    return p;
+}
+
+EventPtrs ev_ptrs(const tofmlem_events *e, uint64_t off = 0) {
+    EventPtrs p{e->x1 + off, e->y1 + off, e->z1 + off, e->x2 + off, e->y2 + off, e->z2 + off,
+                e->dt ? e->dt + off : nullptr};
+    return p;
+}
+
+bool ev_ok(const tofmlem_events *e, bool need_dt) {
+    return e && e->x1 && e->y1 && e->z1 && e->x2 && e->y2 && e->z2 && (!need_dt || e->dt);
+}
+
+GridF32 grid_f32(const tofmlem_ctx *c) {
+    const tofmlem_grid &g = c->grid;
+    return GridF32{g.nx, g.ny, g.nz, g.vx, g.vy, g.vz, g.ox, g.oy, g.oz};
+}
+
+uint32_t num_bins(const tofmlem_ctx *c) {
+    const int t = 1 << c->tile_log2;
+    const uint64_t T = (uint64_t)((c->grid.nx + t - 1) >> c->tile_log2) * ((c->grid.ny + t - 1) >> c->tile_log2) *
+                       ((c->grid.nz + t - 1) >> c->tile_log2);
+    return (uint32_t)(12u * T);
+}
+
+int ensure_corr(tofmlem_ctx *ctx) {
+    if (!ctx->d_corr) {
+        CU(cudaMallocAsync(&ctx->d_corr, ctx->nvox * sizeof(float), ctx->stream));
+        CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
+    }
+    return TOFMLEM_OK;
+}
+
+void default_region_slices(int nz, int R, std::vector<int32_t> &k) {
+    k.resize(R + 1);
+    k[0] = 0;
+    for (int j = 1; j <= R; ++j) k[j] = (int32_t)(((int64_t)nz * (j + 1)) / (R + 1));
+}
+
+// zb[j] = (float)k_j * vz + oz : one float multiply, then one float add (F1); volatile blocks contraction.
+void default_zbounds(const tofmlem_ctx *c, int R, float *zb) {
+    std::vector<int32_t> k;
+    default_region_slices(c->grid.nz, R, k);
+    for (int j = 0; j <= R; ++j) {
+        volatile float kv = (float)k[j] * c->grid.vz;
+        volatile float z = kv + c->grid.oz;
+        zb[j] = z;
+    }
+}
+
+int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, float *d_image, const float *d_sens, int iters,
+                   bool compute_max) {
+    int rc = ensure_corr(ctx);
+    if (rc) return rc;
+    const ProjParams p = make_params(ctx, ctx->tof);
+    const float *dmax = ctx->d_max_ext ? ctx->d_max_ext : ctx->d_max;
+    if (compute_max && !ctx->d_max_ext) {
+        launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, ctx->stream);
+        CHECK_LAUNCH(1);
+    }
+    CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
+    for (int it = 0; it < iters; ++it) {
+        CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), ctx->stream));
+        launch_em_correction(p, ctx->tof, ev, n, d_image, ctx->d_corr, ctx->d_stats, ctx->stream);
+        CHECK_LAUNCH(n ? 1 : 0);
+        launch_update(d_image, ctx->d_corr, d_sens, dmax, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
+        CHECK_LAUNCH(1);
+    }
+    launch_dot_f64(d_image, d_sens, ctx->nvox, &ctx->d_stats->sum_image_sens, ctx->stream);
+    CHECK_LAUNCH(1);
+    ctx->last_n = n;
+    return TOFMLEM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *tofmlem_version(void) { return "tofmlem 0.1 (sm_100a)"; }
+
+int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, float tof_fwhm_ps, void *cuda_stream,
+                   tofmlem_ctx **out) {
+    if (!scanner || !grid || !out) return TOFMLEM_EINVAL;
+    *out = nullptr;
+    if (grid->nx <= 0 || grid->ny <= 0 || grid->nz <= 0 || !(grid->vx > 0) || !(grid->vy > 0) || !(grid->vz > 0) ||
+        !isfinite(grid->ox) || !isfinite(grid->oy) || !isfinite(grid->oz) || !(scanner->radius_mm > 0) ||
+        !(scanner->axial_length_mm > 0) || isnan(tof_fwhm_ps))
+        return TOFMLEM_EINVAL;
+    const uint64_t nvox = (uint64_t)grid->nx * grid->ny * grid->nz;
+    if (nvox >= (1ull << 31)) return TOFMLEM_EINVAL;
+    tofmlem_ctx *ctx = new (std::nothrow) tofmlem_ctx;
+    if (!ctx) return TOFMLEM_ENOMEM;
+    ctx->scanner = *scanner;
+    ctx->grid = *grid;
+    ctx->tof = tof_fwhm_ps > 0.0f;
+    ctx->sigma = ctx->tof ? sigma_from_fwhm(tof_fwhm_ps) : 0.0;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->nvox = nvox;
+    cudaError_t e = cudaMalloc(&ctx->d_max, sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, sizeof(DeviceStats));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_rcounts, 2 * (kMaxRegions + 1) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_stats, 0, sizeof(DeviceStats), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_max, 0, sizeof(float), ctx->stream);
+    if (e != cudaSuccess) {
+        int rc = e == cudaErrorMemoryAllocation ? TOFMLEM_ENOMEM : TOFMLEM_ECUDA;
+        cudaFree(ctx->d_max);
+        cudaFree(ctx->d_stats);
+        cudaFree(ctx->d_rcounts);
+        delete ctx;
+        return rc;
+    }
+    *out = ctx;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_destroy(tofmlem_ctx *ctx) {
+    if (!ctx) return TOFMLEM_OK;
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->copy_stream) {
+        cudaStreamSynchronize(ctx->copy_stream);
+        cudaStreamDestroy(ctx->copy_stream);
+    }
+    for (auto &ev : ctx->chunk_done)
+        if (ev) cudaEventDestroy(ev);
+    cudaFree(ctx->d_corr);
+    cudaFree(ctx->d_max);
+    cudaFree(ctx->d_stats);
+    cudaFree(ctx->d_hist);
+    cudaFree(ctx->d_cursor);
+    cudaFree(ctx->d_rcounts);
+    cudaFree(ctx->d_hev);
+    cudaFree(ctx->d_himg);
+    cudaFree(ctx->d_hsens);
+    delete ctx;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    switch (key) {
+        case TOFMLEM_OPT_TRUNC_SIGMAS:
+            if (!(value > 0.0) || !isfinite(value)) return fail(ctx, TOFMLEM_EINVAL, "trunc_sigmas must be > 0");
+            ctx->trunc_sigmas = value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_SENS_FLOOR_REL:
+            if (!(value >= 0.0) || !(value <= 1.0)) return fail(ctx, TOFMLEM_EINVAL, "sens_floor_rel in [0,1]");
+            ctx->sens_floor_rel = value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_TILE_LOG2:
+            if (value < 0 || value > 8 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "tile_log2 in 0..8");
+            ctx->tile_log2 = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_PROJECTOR:
+            if (value == 0.0) {
+                ctx->projector = 0;
+                return TOFMLEM_OK;
+            }
+            return fail(ctx, TOFMLEM_EUNSUPPORTED, "sampled projector not built yet");
+        case TOFMLEM_OPT_SAMPLES_K:
+            if (value < 1 || value > 1024 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "K in 1..1024");
+            ctx->samples_k = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_SHELL_MM:
+            if (!(value >= 0.0) || !isfinite(value)) return fail(ctx, TOFMLEM_EINVAL, "shell_mm must be >= 0");
+            ctx->shell_mm = value;
+            return TOFMLEM_OK;
+        default:
+            return fail(ctx, TOFMLEM_EINVAL, "unknown option key");
+    }
+}
+
+double tofmlem_sigma_mm(const tofmlem_ctx *ctx) { return ctx ? ctx->sigma : 0.0; }
+
+int tofmlem_sensitivity(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t m, float *d_sens) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (!ev_ok(lors, false) || !d_sens || m == 0 || m > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "sensitivity: bad argument");
+    const ProjParams p = make_params(ctx, false);
+    CU(cudaMemsetAsync(d_sens, 0, ctx->nvox * sizeof(float), ctx->stream));
+    EventPtrs ev = ev_ptrs(lors);
+    ev.dt = nullptr;
+    launch_backproject(p, false, ev, m, nullptr, d_sens, ctx->stream);
+    CHECK_LAUNCH(1);
+    launch_scale(d_sens, (float)(1.0 / (double)m), ctx->nvox, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_forward(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_fwd) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(ev, ctx->tof) || !d_image || !d_fwd || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "forward: bad argument");
+    launch_forward(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_fwd, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_values, float *d_out) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(ev, ctx->tof) || !d_out || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "backproject: bad argument");
+    launch_backproject(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_values, d_out, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_reset_stats(tofmlem_ctx *ctx) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    CU(cudaMemsetAsync(ctx->d_stats, 0, sizeof(DeviceStats), ctx->stream));
+    ctx->last_n = 0;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(ev, ctx->tof) || !d_image || !d_corr || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "em_correction: bad argument");
+    launch_em_correction(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_corr, ctx->d_stats,
+                         ctx->stream);
+    CHECK_LAUNCH(1);
+    ctx->last_n += n;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_update(tofmlem_ctx *ctx, float *d_image, float *d_corr, const float *d_sens) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (!d_image || !d_corr || !d_sens) return fail(ctx, TOFMLEM_EINVAL, "update: NULL argument");
+    launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, ctx->stream);
+    CHECK_LAUNCH(1);
+    launch_update(d_image, d_corr, d_sens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_iterate(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, float *d_image, const float *d_sens,
+                    int iters) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if ((n && !ev_ok(ev, ctx->tof)) || !d_image || !d_sens || iters < 0 || n > 0xFFFFFFFFull || d_image == d_sens)
+        return fail(ctx, TOFMLEM_EINVAL, "iterate: bad argument");
+    EventPtrs p = n ? ev_ptrs(ev) : EventPtrs{};
+    return iterate_device(ctx, p, n, d_image, d_sens, iters, true);
+}
+
+int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t n, float *h_image,
+                         const float *h_sens, int iters) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if ((n && !ev_ok(h_ev, ctx->tof)) || !h_image || !h_sens || iters < 0 || n > 0xFFFFFFFFull)
+        return fail(ctx, TOFMLEM_EINVAL, "iterate_host: bad argument");
+    const size_t vbytes = ctx->nvox * sizeof(float);
+    if (!ctx->copy_stream) {
+        CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        for (auto &e : ctx->chunk_done) CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    if (!ctx->d_himg) {
+        CU(cudaMalloc(&ctx->d_himg, vbytes));
+        CU(cudaMalloc(&ctx->d_hsens, vbytes));
+    }
+    const uint64_t stride = (n + 3) & ~3ull;  // keep every member array 16-byte aligned
+    if (ctx->hev_cap < 7 * stride) {
+        cudaFree(ctx->d_hev);
+        ctx->d_hev = nullptr;
+        ctx->hev_cap = 0;
+        CU(cudaMalloc(&ctx->d_hev, 7 * stride * sizeof(float) + 16));
+        ctx->hev_cap = 7 * stride;
+    }
+    int rc = ensure_corr(ctx);
+    if (rc) return rc;
+    cudaStream_t s = ctx->stream, cs = ctx->copy_stream;
+    CU(cudaMemcpyAsync(ctx->d_himg, h_image, vbytes, cudaMemcpyHostToDevice, s));
+    CU(cudaMemcpyAsync(ctx->d_hsens, h_sens, vbytes, cudaMemcpyHostToDevice, s));
+    launch_max_nonneg(ctx->d_hsens, ctx->nvox, ctx->d_max, s);
+    CHECK_LAUNCH(1);
+    CU(cudaMemsetAsync(ctx->d_corr, 0, vbytes, s));
+    CU(cudaMemsetAsync(ctx->d_stats, 0, sizeof(DeviceStats), s));
+    float *d = ctx->d_hev;
+    tofmlem_events dev{d, d + stride, d + 2 * stride, d + 3 * stride, d + 4 * stride, d + 5 * stride,
+                       h_ev && h_ev->dt ? d + 6 * stride : nullptr};
+    const float *hsrc[7] = {n ? h_ev->x1 : nullptr, n ? h_ev->y1 : nullptr, n ? h_ev->z1 : nullptr,
+                            n ? h_ev->x2 : nullptr, n ? h_ev->y2 : nullptr, n ? h_ev->z2 : nullptr,
+                            n ? h_ev->dt : nullptr};
+    const ProjParams p = make_params(ctx, ctx->tof);
+    if (iters > 0 && n > 0) {
+        // first pass: upload chunk k+1 on the copy stream while chunk k is projected on the compute stream
+        const uint64_t chunk = 8ull << 20;
+        int slot = 0;
+        for (uint64_t off = 0; off < n; off += chunk, slot ^= 1) {
+            const uint64_t m = n - off < chunk ? n - off : chunk;
+            for (int f = 0; f < 7; ++f)
+                if (hsrc[f])
+                    CU(cudaMemcpyAsync(d + f * stride + off, hsrc[f] + off, m * sizeof(float), cudaMemcpyHostToDevice, cs));
+            CU(cudaEventRecord(ctx->chunk_done[slot], cs));
+            CU(cudaStreamWaitEvent(s, ctx->chunk_done[slot], 0));
+            launch_em_correction(p, ctx->tof, ev_ptrs(&dev, off), m, ctx->d_himg, ctx->d_corr, ctx->d_stats, s);
+            CHECK_LAUNCH(1);
+        }
+        launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
+        CHECK_LAUNCH(1);
+        for (int it = 1; it < iters; ++it) {
+            CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), s));
+            launch_em_correction(p, ctx->tof, ev_ptrs(&dev), n, ctx->d_himg, ctx->d_corr, ctx->d_stats, s);
+            CHECK_LAUNCH(1);
+            launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
+            CHECK_LAUNCH(1);
+        }
+    } else if (iters > 0) {
+        for (int it = 0; it < iters; ++it) {
+            launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
+            CHECK_LAUNCH(1);
+        }
+    }
+    launch_dot_f64(ctx->d_himg, ctx->d_hsens, ctx->nvox, &ctx->d_stats->sum_image_sens, s);
+    CHECK_LAUNCH(1);
+    CU(cudaMemcpyAsync(h_image, ctx->d_himg, vbytes, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    ctx->last_n = n;
+    return TOFMLEM_OK;
+}
+
+uint32_t tofmlem_num_bins(const tofmlem_ctx *ctx) { return ctx ? num_bins(ctx) : 0u; }
+
+int tofmlem_bin_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, uint32_t *d_key, uint32_t *d_perm,
+                       uint32_t *d_bin_offsets) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(ev, false) || !d_key || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "bin_events: bad argument");
+    const uint32_t nb = num_bins(ctx);
+    if (ctx->hist_cap < (size_t)nb + 1) {
+        cudaFree(ctx->d_hist);
+        cudaFree(ctx->d_cursor);
+        ctx->d_hist = ctx->d_cursor = nullptr;
+        ctx->hist_cap = 0;
+        CU(cudaMalloc(&ctx->d_hist, ((size_t)nb + 1) * sizeof(uint32_t)));
+        CU(cudaMalloc(&ctx->d_cursor, ((size_t)nb + 1) * sizeof(uint32_t)));
+        ctx->hist_cap = (size_t)nb + 1;
+    }
+    const bool sort = d_perm != nullptr;
+    CU(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)nb + 1) * sizeof(uint32_t), ctx->stream));
+    launch_bin_keys(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, d_key, (sort || d_bin_offsets) ? ctx->d_hist : nullptr,
+                    nb, ctx->stream);
+    CHECK_LAUNCH(1);
+    if (sort || d_bin_offsets) {
+        launch_exclusive_scan_u32(ctx->d_hist, ctx->d_cursor, nullptr, nb + 1, ctx->stream);
+        CHECK_LAUNCH(1);
+        if (d_bin_offsets)
+            CU(cudaMemcpyAsync(d_bin_offsets, ctx->d_cursor, ((size_t)nb + 1) * sizeof(uint32_t),
+                               cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    if (sort) {
+        launch_scatter_perm(d_key, n, nb, ctx->d_cursor, d_perm, ctx->stream);
+        CHECK_LAUNCH(1);
+    }
+    return TOFMLEM_OK;
+}
+
+int tofmlem_gather_events(tofmlem_ctx *ctx, const tofmlem_events *in, const uint32_t *d_perm, uint64_t n,
+                          const tofmlem_events_mut *out) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(in, false) || !d_perm || !out || !out->x1 || !out->y1 || !out->z1 || !out->x2 || !out->y2 || !out->z2)
+        return fail(ctx, TOFMLEM_EINVAL, "gather_events: bad argument");
+    const float *src[7] = {in->x1, in->y1, in->z1, in->x2, in->y2, in->z2, in->dt};
+    float *dst[7] = {out->x1, out->y1, out->z1, out->x2, out->y2, out->z2, out->dt};
+    for (int f = 0; f < 7; ++f) {
+        if (!src[f] || !dst[f]) continue;
+        if (src[f] == dst[f]) return fail(ctx, TOFMLEM_EINVAL, "gather_events: in/out alias");
+        launch_gather(src[f], d_perm, n, dst[f], ctx->stream);
+        CHECK_LAUNCH(1);
+    }
+    return TOFMLEM_OK;
+}
+
+int tofmlem_region_zbounds(const tofmlem_ctx *ctx, int n_regions, float *h_zbounds) {
+    if (!ctx || !h_zbounds || n_regions < 1 || n_regions > kMaxRegions) return TOFMLEM_EINVAL;
+    default_zbounds(ctx, n_regions, h_zbounds);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                          const float *h_zbounds, int32_t *d_region, uint32_t *d_perm, uint64_t *h_counts) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if ((n && !ev_ok(ev, false)) || n_regions < 1 || n_regions > kMaxRegions || (n && !d_region) || !h_counts ||
+        n > 0xFFFFFFFFull)
+        return fail(ctx, TOFMLEM_EINVAL, "split_regions: bad argument");
+    RegionBounds rb;
+    rb.n_regions = n_regions;
+    if (h_zbounds) {
+        for (int j = 0; j <= n_regions; ++j) rb.zb[j] = h_zbounds[j];
+        for (int j = 0; j < n_regions; ++j)
+            if (!(rb.zb[j] <= rb.zb[j + 1])) return fail(ctx, TOFMLEM_EINVAL, "split_regions: bounds not ascending");
+    } else {
+        default_zbounds(ctx, n_regions, rb.zb);
+    }
+    unsigned long long *counts = ctx->d_rcounts, *cursor = ctx->d_rcounts + (kMaxRegions + 1);
+    CU(cudaMemsetAsync(counts, 0, 2 * (kMaxRegions + 1) * sizeof(unsigned long long), ctx->stream));
+    if (n) {
+        launch_region_ids(ev_ptrs(ev), n, rb, d_region, counts, ctx->stream);
+        CHECK_LAUNCH(1);
+    }
+    unsigned long long h[kMaxRegions + 1];
+    CU(cudaMemcpyAsync(h, counts, (n_regions + 1) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int r = 0; r < n_regions; ++r) h_counts[r] = h[r];
+    if (d_perm && n) {
+        unsigned long long start[kMaxRegions + 1];
+        unsigned long long run = 0;
+        for (int r = 0; r <= n_regions; ++r) {
+            start[r] = run;
+            run += h[r];
+        }
+        CU(cudaMemcpyAsync(cursor, start, (n_regions + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice,
+                           ctx->stream));
+        launch_region_scatter(d_region, n, n_regions, cursor, d_perm, ctx->stream);
+        CHECK_LAUNCH(1);
+        CU(cudaStreamSynchronize(ctx->stream));  // `start` lives on this stack frame
+    }
+    return TOFMLEM_OK;
+}
+
+int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zbounds, int r, tofmlem_grid *sub,
+                        int32_t *z0, int32_t *z1) {
+    if (!ctx || !sub || !z0 || !z1 || n_regions < 1 || n_regions > kMaxRegions || r < 0 || r >= n_regions)
+        return TOFMLEM_EINVAL;
+    const tofmlem_grid &g = ctx->grid;
+    int32_t k0, k1;
+    if (h_zbounds) {
+        k0 = (int32_t)floor(((double)h_zbounds[r] - g.oz) / g.vz + 1e-4);
+        k1 = (int32_t)ceil(((double)h_zbounds[r + 1] - g.oz) / g.vz - 1e-4);
+    } else {
+        std::vector<int32_t> k;
+        default_region_slices(g.nz, n_regions, k);
+        k0 = k[r];
+        k1 = k[r + 1];
+    }
+    const int32_t margin = (int32_t)ceil((ctx->trunc_sigmas * ctx->sigma + ctx->shell_mm) / (double)g.vz);
+    int32_t a = k0 - (r > 0 ? margin : 0), b = k1 + (r < n_regions - 1 ? margin : 0);
+    if (a < 0) a = 0;
+    if (b > g.nz) b = g.nz;
+    if (b <= a) return TOFMLEM_EINVAL;
+    *sub = g;
+    sub->nz = b - a;
+    sub->oz = (float)((double)g.oz + (double)a * (double)g.vz);
+    *z0 = a;
+    *z1 = b;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                                const float *h_zbounds, float *d_image_out, const float *d_sens, int iters) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (!ev_ok(ev, ctx->tof) || !d_image_out || !d_sens || iters < 0 || n == 0 || n > 0xFFFFFFFFull ||
+        n_regions < 1 || n_regions > kMaxRegions)
+        return fail(ctx, TOFMLEM_EINVAL, "reconstruct_regions: bad argument");
+    cudaStream_t s = ctx->stream;
+    const size_t slice = (size_t)ctx->grid.nx * ctx->grid.ny;
+    int32_t *d_region = nullptr;
+    uint32_t *d_perm = nullptr;
+    float *d_sorted = nullptr;
+    const uint64_t stride = (n + 3) & ~3ull;
+    std::vector<uint64_t> counts(n_regions);
+    std::vector<tofmlem_ctx *> subs(n_regions, nullptr);
+    std::vector<cudaStream_t> streams(n_regions, nullptr);
+    std::vector<float *> images(n_regions, nullptr);
+    std::vector<int32_t> z0(n_regions), z1(n_regions);
+    cudaEvent_t ready = nullptr;
+    std::vector<cudaEvent_t> done(n_regions, nullptr);
+    int rc = TOFMLEM_OK;
+    auto cleanup = [&]() {
+        for (int r = 0; r < n_regions; ++r) {
+            if (subs[r]) tofmlem_destroy(subs[r]);
+            if (streams[r]) cudaStreamDestroy(streams[r]);
+            if (done[r]) cudaEventDestroy(done[r]);
+            cudaFree(images[r]);
+        }
+        if (ready) cudaEventDestroy(ready);
+        cudaFree(d_region);
+        cudaFree(d_perm);
+        cudaFree(d_sorted);
+    };
+#define RCU(call)                                          \
+    do {                                                   \
+        cudaError_t e_ = (call);                           \
+        if (e_ != cudaSuccess) {                           \
+            rc = cuda_fail(ctx, e_, #call);                \
+            cudaDeviceSynchronize();                       \
+            cleanup();                                     \
+            return rc;                                     \
+        }                                                  \
+    } while (0)
+#define RRC(call)                      \
+    do {                               \
+        rc = (call);                   \
+        if (rc != TOFMLEM_OK) {        \
+            cudaDeviceSynchronize();   \
+            cleanup();                 \
+            return rc;                 \
+        }                              \
+    } while (0)
+    RCU(cudaMalloc(&d_region, n * sizeof(int32_t)));
+    RCU(cudaMalloc(&d_perm, n * sizeof(uint32_t)));
+    RCU(cudaMalloc(&d_sorted, 7 * stride * sizeof(float)));
+    RRC(tofmlem_split_regions(ctx, ev, n, n_regions, h_zbounds, d_region, d_perm, counts.data()));
+    tofmlem_events_mut sorted{d_sorted, d_sorted + stride, d_sorted + 2 * stride, d_sorted + 3 * stride,
+                              d_sorted + 4 * stride, d_sorted + 5 * stride, ev->dt ? d_sorted + 6 * stride : nullptr};
+    RRC(tofmlem_gather_events(ctx, ev, d_perm, n, &sorted));
+    launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, s);
+    ctx->launches += 1;
+    RCU(cudaMemsetAsync(d_image_out, 0, ctx->nvox * sizeof(float), s));
+    RCU(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
+    RCU(cudaEventRecord(ready, s));
+    uint64_t off = 0;
+    for (int r = 0; r < n_regions; ++r) {
+        tofmlem_grid sub;
+        RRC(tofmlem_region_grid(ctx, n_regions, h_zbounds, r, &sub, &z0[r], &z1[r]));
+        RCU(cudaStreamCreateWithFlags(&streams[r], cudaStreamNonBlocking));
+        RCU(cudaEventCreateWithFlags(&done[r], cudaEventDisableTiming));
+        RRC(tofmlem_create(&ctx->scanner, &sub, ctx->tof ? (float)(ctx->sigma / sigma_from_fwhm(1.0)) : 0.0f,
+                           streams[r], &subs[r]));
+        tofmlem_ctx *sc = subs[r];
+        sc->sigma = ctx->sigma;
+        sc->trunc_sigmas = ctx->trunc_sigmas;
+        sc->sens_floor_rel = ctx->sens_floor_rel;
+        sc->d_max_ext = ctx->d_max;
+        const uint64_t nv = sc->nvox;
+        RCU(cudaMalloc(&images[r], nv * sizeof(float)));
+        RCU(cudaStreamWaitEvent(streams[r], ready, 0));
+        const float *sens_r = d_sens + (size_t)z0[r] * slice;
+        launch_mask_init(images[r], sens_r, ctx->d_max, (float)ctx->sens_floor_rel, nv, streams[r]);
+        sc->launches += 1;
+        tofmlem_events sub_ev{sorted.x1 + off, sorted.y1 + off, sorted.z1 + off, sorted.x2 + off, sorted.y2 + off,
+                              sorted.z2 + off, sorted.dt ? sorted.dt + off : nullptr};
+        rc = iterate_device(sc, counts[r] ? ev_ptrs(&sub_ev) : EventPtrs{}, counts[r], images[r], sens_r, iters, false);
+        if (rc != TOFMLEM_OK) {
+            ctx->err = sc->err;
+            cudaDeviceSynchronize();
+            cleanup();
+            return rc;
+        }
+        RCU(cudaEventRecord(done[r], streams[r]));
+        off += counts[r];
+    }
+    // sum of the extended region images; overlapping margins add up
+    for (int r = 0; r < n_regions; ++r) {
+        RCU(cudaStreamWaitEvent(s, done[r], 0));
+        launch_add(d_image_out + (size_t)z0[r] * slice, images[r], subs[r]->nvox, s);
+        ctx->launches += 1 + subs[r]->launches;
+    }
+    RCU(cudaStreamSynchronize(s));
+    cleanup();
+#undef RCU
+#undef RRC
+    return TOFMLEM_OK;
+}
+
+int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out) {
+    if (!ctx || !h_out) return TOFMLEM_EINVAL;
+    DeviceStats h;
+    CU(cudaMemcpyAsync(&h, ctx->d_stats, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    h_out->n_valid = h.n_valid;
+    h_out->n_skipped = ctx->last_n >= h.n_valid ? ctx->last_n - h.n_valid : 0;
+    h_out->visits = h.visits;
+    h_out->sum_image_sens = h.sum_image_sens;
+    return TOFMLEM_OK;
+}
+
+const char *tofmlem_last_error(const tofmlem_ctx *ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
+
+uint64_t tofmlem_launch_count(const tofmlem_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,151 @@
+// image_ops.cu -- element-wise / reduction kernels over the voxel arrays (HBM-bound, 4-wide loads).
+//   update (R1, R11): x_j <- mask_j ? x_j * corr_j / sens_j : 0, corr_j <- 0
+#include "internal.cuh"
+
+namespace tofmlem {
+
+constexpr int kBlock = 256;
+constexpr int kMaxGrid = 148 * 8;
+
+static inline unsigned grid_for(uint64_t work) {
+    uint64_t g = (work + kBlock - 1) / kBlock;
+    if (g > kMaxGrid) g = kMaxGrid;
+    if (g == 0) g = 1;
+    return (unsigned)g;
+}
+
+__device__ __forceinline__ float warp_max(float v) {
+    for (int o = 16; o; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// max over non-negative floats (negative and NaN entries count as 0): uint ordering == float ordering
+__global__ void __launch_bounds__(kBlock) max_nonneg_kernel(const float *__restrict__ x, uint64_t n, float *d_max) {
+    float m = 0.0f;
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) m = fmaxf(m, __ldg(x + i));
+    m = warp_max(m);
+    __shared__ float sm[kBlock / 32];
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        m = threadIdx.x < kBlock / 32 ? sm[threadIdx.x] : 0.0f;
+        m = warp_max(m);
+        if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned int *>(d_max), __float_as_uint(m));
+    }
+}
+
+__device__ __forceinline__ float update_one(float x, float c, float s, float thr) {
+    const bool mask = (s >= thr) && (s > 0.0f);
+    return mask ? __fdiv_rn(__fmul_rn(x, c), s) : 0.0f;
+}
+
+__global__ void __launch_bounds__(kBlock) update_kernel(float *__restrict__ image, float *__restrict__ corr,
+                                                        const float *__restrict__ sens,
+                                                        const float *__restrict__ d_max, float floor_rel, uint64_t n,
+                                                        int vec_ok) {
+    const float thr = __fmul_rn(floor_rel, *d_max);
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    const uint64_t tid = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    uint64_t done = 0;
+    if (vec_ok) {
+        const uint64_t n4 = n >> 2;
+        float4 *img4 = reinterpret_cast<float4 *>(image);
+        float4 *cor4 = reinterpret_cast<float4 *>(corr);
+        const float4 *sen4 = reinterpret_cast<const float4 *>(sens);
+        for (uint64_t i = tid; i < n4; i += stride) {
+            float4 x = img4[i];
+            const float4 c = cor4[i];
+            const float4 s = __ldg(sen4 + i);
+            x.x = update_one(x.x, c.x, s.x, thr);
+            x.y = update_one(x.y, c.y, s.y, thr);
+            x.z = update_one(x.z, c.z, s.z, thr);
+            x.w = update_one(x.w, c.w, s.w, thr);
+            img4[i] = x;
+            cor4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        done = n4 << 2;
+    }
+    for (uint64_t i = done + tid; i < n; i += stride) {
+        image[i] = update_one(image[i], corr[i], __ldg(sens + i), thr);
+        corr[i] = 0.0f;
+    }
+}
+
+// x0 = mask (the harness' initial image, R15)
+__global__ void __launch_bounds__(kBlock) mask_init_kernel(float *__restrict__ image, const float *__restrict__ sens,
+                                                           const float *__restrict__ d_max, float floor_rel,
+                                                           uint64_t n) {
+    const float thr = __fmul_rn(floor_rel, *d_max);
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) {
+        const float s = __ldg(sens + i);
+        image[i] = ((s >= thr) && (s > 0.0f)) ? 1.0f : 0.0f;
+    }
+}
+
+__global__ void __launch_bounds__(kBlock) dot_f64_kernel(const float *__restrict__ a, const float *__restrict__ b,
+                                                         uint64_t n, double *d_out) {
+    double acc = 0.0;
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride)
+        acc += (double)__ldg(a + i) * (double)__ldg(b + i);
+    acc = warp_sum(acc);
+    __shared__ double sm[kBlock / 32];
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        acc = threadIdx.x < kBlock / 32 ? sm[threadIdx.x] : 0.0;
+        acc = warp_sum(acc);
+        if (threadIdx.x == 0) atomicAdd(d_out, acc);
+    }
+}
+
+__global__ void __launch_bounds__(kBlock) scale_kernel(float *__restrict__ x, float a, uint64_t n) {
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) x[i] = __fmul_rn(x[i], a);
+}
+
+__global__ void __launch_bounds__(kBlock) add_kernel(float *__restrict__ dst, const float *__restrict__ src,
+                                                     uint64_t n) {
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) dst[i] += __ldg(src + i);
+}
+
+void launch_max_nonneg(const float *x, uint64_t n, float *d_max, cudaStream_t s) {
+    cudaMemsetAsync(d_max, 0, sizeof(float), s);
+    if (n) max_nonneg_kernel<<<grid_for(n), kBlock, 0, s>>>(x, n, d_max);
+}
+
+void launch_update(float *image, float *corr, const float *sens, const float *d_max, float floor_rel, uint64_t n,
+                   cudaStream_t s) {
+    if (!n) return;
+    const int vec_ok = ((reinterpret_cast<uintptr_t>(image) | reinterpret_cast<uintptr_t>(corr) |
+                         reinterpret_cast<uintptr_t>(sens)) & 15) == 0;
+    update_kernel<<<grid_for(vec_ok ? (n >> 2) + 1 : n), kBlock, 0, s>>>(image, corr, sens, d_max, floor_rel, n,
+                                                                         vec_ok);
+}
+
+void launch_mask_init(float *image, const float *sens, const float *d_max, float floor_rel, uint64_t n,
+                      cudaStream_t s) {
+    if (n) mask_init_kernel<<<grid_for(n), kBlock, 0, s>>>(image, sens, d_max, floor_rel, n);
+}
+
+void launch_dot_f64(const float *a, const float *b, uint64_t n, double *d_out, cudaStream_t s) {
+    cudaMemsetAsync(d_out, 0, sizeof(double), s);
+    if (n) dot_f64_kernel<<<grid_for(n), kBlock, 0, s>>>(a, b, n, d_out);
+}
+
+void launch_scale(float *x, float a, uint64_t n, cudaStream_t s) {
+    if (n) scale_kernel<<<grid_for(n), kBlock, 0, s>>>(x, a, n);
+}
+
+void launch_add(float *dst, const float *src, uint64_t n, cudaStream_t s) {
+    if (n) add_kernel<<<grid_for(n), kBlock, 0, s>>>(dst, src, n);
+}
+
+}  // namespace tofmlem
