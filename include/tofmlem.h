@@ -156,6 +156,13 @@ int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zb
 int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
                                 const float *h_zbounds, float *d_image_out, const float *d_sens, int iters);
 
+/* Roofline probe (measurement aid; north_star asks for the MEASURED atomic / L2 roofline): issues n_ops float32
+ * operations against d_buf[0..n_elems) and returns the elapsed milliseconds in *h_ms (second of two passes, so
+ * the array is L2-resident when it fits).  kind 0: RED.ADD.F32 to unrelated random elements per lane; 1: RED to
+ * 32 consecutive elements of a random row per warp; 2 / 3: the same two patterns with 4-byte loads.
+ * d_buf is modified by kinds 0, 1.  SYNCHRONISES. */
+int tofmlem_probe(tofmlem_ctx *ctx, int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *h_ms);
+
 /* Copies the counters of the last pass to *h_out.  SYNCHRONISES the context's stream. */
 int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out);
 /* Text of the last error of this context ("" if none).  Valid until the next call on the context. */

@@ -650,6 +650,15 @@ int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out) {
     return TOFMLEM_OK;
 }
 
+int tofmlem_probe(tofmlem_ctx *ctx, int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *h_ms) {
+    if (!ctx || !d_buf || !h_ms || n_ops == 0) return TOFMLEM_EINVAL;
+    const int rc = run_probe(kind, d_buf, n_elems, n_ops, h_ms, ctx->stream);
+    if (rc == -1) return fail(ctx, TOFMLEM_EINVAL, "probe: bad kind or size");
+    if (rc != 0) return cuda_fail(ctx, cudaGetLastError(), "probe");
+    ctx->launches += 2;
+    return TOFMLEM_OK;
+}
+
 const char *tofmlem_last_error(const tofmlem_ctx *ctx) { return ctx ? ctx->err.c_str() : "NULL context"; }
 
 uint64_t tofmlem_launch_count(const tofmlem_ctx *ctx) { return ctx ? ctx->launches : 0; }

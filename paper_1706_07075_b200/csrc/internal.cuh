@@ -79,4 +79,7 @@ void launch_region_scatter(const int32_t *region, uint64_t n, int n_regions,
                            unsigned long long *cursor /* n_regions+1 start offsets, advanced */, uint32_t *perm,
                            cudaStream_t s);
 
+// ---- probe.cu
+int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *ms, cudaStream_t s);
+
 }  // namespace tofmlem

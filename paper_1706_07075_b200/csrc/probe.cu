@@ -1,0 +1,68 @@
+// probe.cu -- micro-benchmarks that MEASURE the roofline denominators of the projector on this GPU:
+// float32 reductions (RED.ADD.F32) and 4-byte gathers against an L2-resident array, with warp lanes
+// hitting (a) unrelated random voxels, (b) 32 consecutive voxels of a random row.  bench.py runs them
+// live beside the timed kernel (BASELINE.json north_star: "achieved fraction of the atomic- and
+// L2-bandwidth roofline", measured, not assumed).
+#include "internal.cuh"
+
+namespace tofmlem {
+
+__device__ __forceinline__ uint32_t mix32(uint32_t x) {
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+// kind: 0 random RED, 1 row-coalesced RED, 2 random gather, 3 row-coalesced gather
+template <int KIND>
+__global__ void __launch_bounds__(256) probe_kernel(float *buf, uint32_t n, int ops, float *sink) {
+    const uint32_t tid = blockIdx.x * 256u + threadIdx.x;
+    const uint32_t lane = threadIdx.x & 31u, warp = tid >> 5;
+    float acc = 0.0f;
+    uint32_t h = mix32(((KIND & 1) ? warp : tid) * 2654435761u + 12345u);
+#pragma unroll 4
+    for (int i = 0; i < ops; ++i) {
+        h = mix32(h + 0x9e3779b9u);
+        uint32_t a;
+        if (KIND & 1)
+            a = ((h % (n >> 5)) << 5) + lane;
+        else
+            a = h % n;
+        if (KIND < 2)
+            atomicAdd(buf + a, 1.0f);
+        else
+            acc += __ldg(buf + a);
+    }
+    if (KIND >= 2 && acc == 123.456f) *sink = acc;
+}
+
+int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *ms, cudaStream_t s) {
+    if (n_elems < 64 || n_elems > 0xFFFFFFFFull) return -1;
+    const int blocks = 148 * 16;
+    const uint64_t threads = (uint64_t)blocks * 256;
+    const int ops = (int)((n_ops + threads - 1) / threads);
+    float *sink = d_buf;  // never written in practice
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    for (int rep = 0; rep < 2; ++rep) {  // first pass warms L2
+        cudaEventRecord(a, s);
+        switch (kind) {
+            case 0: probe_kernel<0><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            case 1: probe_kernel<1><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            case 2: probe_kernel<2><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            case 3: probe_kernel<3><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            default: cudaEventDestroy(a); cudaEventDestroy(b); return -1;
+        }
+        cudaEventRecord(b, s);
+    }
+    cudaError_t e = cudaEventSynchronize(b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, a, b);
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    if (e != cudaSuccess) return -3;
+    // report per-op time basis: caller divides ops*threads by ms
+    *ms = *ms * (float)((double)n_ops / ((double)ops * (double)threads));
+    return 0;
+}
+
+}  // namespace tofmlem

@@ -25,7 +25,7 @@ SYMBOLS = (
     "tofmlem_forward", "tofmlem_backproject", "tofmlem_em_correction", "tofmlem_reset_stats", "tofmlem_update",
     "tofmlem_iterate", "tofmlem_iterate_host", "tofmlem_bin_events", "tofmlem_num_bins", "tofmlem_gather_events",
     "tofmlem_split_regions", "tofmlem_region_zbounds", "tofmlem_region_grid", "tofmlem_reconstruct_regions",
-    "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
+    "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
 )
 
 
@@ -232,6 +232,13 @@ class Context:
             self._h, C.byref(e), C.c_uint64(n), C.c_int(n_regions), C.c_void_p(zb),
             C.c_void_p(_ptr(image_out, torch.float32, "cuda", self.nvox)),
             C.c_void_p(_ptr(sens, torch.float32, "cuda", self.nvox)), C.c_int(iters)))
+
+    def probe(self, kind: int, buf: torch.Tensor, n_ops: int) -> float:
+        """elapsed ms of n_ops float32 REDs (kind 0,1) or gathers (2,3) against buf; see include/tofmlem.h"""
+        ms = C.c_float()
+        self._check(self._L.tofmlem_probe(self._h, C.c_int(kind), C.c_void_p(_ptr(buf, torch.float32, "cuda")),
+                                          C.c_uint64(buf.numel()), C.c_uint64(n_ops), C.byref(ms)))
+        return float(ms.value)
 
     def get_stats(self) -> Stats:
         st = Stats()
