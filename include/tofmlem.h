@@ -74,7 +74,10 @@ enum {
     TOFMLEM_OPT_TILE_LOG2 = 3,      /* locality bins are cubes of 2^value voxels, default 3 */
     TOFMLEM_OPT_PROJECTOR = 4,      /* 0 = Siddon x Gaussian (default); 1 = paper's K-sample LUT */
     TOFMLEM_OPT_SAMPLES_K = 5,      /* K of the sampled projector, default 32 */
-    TOFMLEM_OPT_SHELL_MM = 6        /* extra shell added to the region margin, default 6 mm */
+    TOFMLEM_OPT_SHELL_MM = 6,       /* extra shell added to the region margin, default 6 mm */
+    TOFMLEM_OPT_CTA_INTERLEAVE = 7  /* scatter kernels: number of list segments advanced in parallel (default 64;
+                                       1 = natural order).  Performance only, results are the same up to the
+                                       order of the float32 reductions. */
 };
 
 /* Create a context.  tof_fwhm_ps <= 0 makes a non-TOF context (full-chord traversal).

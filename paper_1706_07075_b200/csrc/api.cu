@@ -20,7 +20,8 @@ struct tofmlem_ctx {
     cudaStream_t stream = nullptr;
     uint64_t nvox = 0;
     // scratch owned by the context
-    float *d_corr = nullptr;
+    float *d_corr = nullptr;  // padded to whole groups of 4 voxels
+    unsigned cta_interleave = 64;
     float *d_max = nullptr;          // max(sens) of the current iterate call
     const float *d_max_ext = nullptr;  // region sub-contexts use the parent's global max
     DeviceStats *d_stats = nullptr;
@@ -72,11 +73,13 @@ double sigma_from_fwhm(double fwhm_ps) { return kCmmPerPs * fwhm_ps / (2.0 * 2.0
 ProjParams make_params(const tofmlem_ctx *c, bool tof) {
     ProjParams p;
     const tofmlem_grid &g = c->grid;
-    p.nx = g.nx; p.ny = g.ny; p.nz = g.nz;
-    p.vx = g.vx; p.vy = g.vy; p.vz = g.vz;
-    p.ivx = 1.0 / p.vx; p.ivy = 1.0 / p.vy; p.ivz = 1.0 / p.vz;
-    p.ox = g.ox; p.oy = g.oy; p.oz = g.oz;
-    p.hx = p.ox + p.nx * p.vx; p.hy = p.oy + p.ny * p.vy; p.hz = p.oz + p.nz * p.vz;
+    p.n[0] = g.nx; p.n[1] = g.ny; p.n[2] = g.nz;
+    p.v[0] = g.vx; p.v[1] = g.vy; p.v[2] = g.vz;
+    p.o[0] = g.ox; p.o[1] = g.oy; p.o[2] = g.oz;
+    for (int a = 0; a < 3; ++a) {
+        p.iv[a] = 1.0 / p.v[a];
+        p.h[a] = p.o[a] + p.n[a] * p.v[a];
+    }
     if (tof) {
         p.half_window = c->trunc_sigmas * c->sigma;
         p.gauss_a = (float)(-1.4426950408889634 / (2.0 * c->sigma * c->sigma));
@@ -86,7 +89,13 @@ ProjParams make_params(const tofmlem_ctx *c, bool tof) {
         p.gauss_a = 0.0f;
         p.gauss_norm = 1.0f;
     }
+    p.stride = c->cta_interleave;
     return p;
+}
+
+// 16-byte vector reductions need an aligned array made of whole groups of 4 voxels
+bool vec_ok(const tofmlem_ctx *c, const float *out) {
+    return (c->nvox & 3) == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
 }
 
 EventPtrs ev_ptrs(const tofmlem_events *e, uint64_t off = 0) {
@@ -113,8 +122,8 @@ uint32_t num_bins(const tofmlem_ctx *c) {
 
 int ensure_corr(tofmlem_ctx *ctx) {
     if (!ctx->d_corr) {
-        CU(cudaMallocAsync(&ctx->d_corr, ctx->nvox * sizeof(float), ctx->stream));
-        CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
+        CU(cudaMalloc(&ctx->d_corr, (ctx->nvox + 4) * sizeof(float)));
+        CU(cudaMemsetAsync(ctx->d_corr, 0, (ctx->nvox + 4) * sizeof(float), ctx->stream));
     }
     return TOFMLEM_OK;
 }
@@ -149,7 +158,7 @@ int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, float *d_i
     CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
     for (int it = 0; it < iters; ++it) {
         CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), ctx->stream));
-        launch_em_correction(p, ctx->tof, ev, n, d_image, ctx->d_corr, ctx->d_stats, ctx->stream);
+        launch_em_correction(p, ctx->tof, ev, n, d_image, ctx->d_corr, true, ctx->d_stats, ctx->stream);
         CHECK_LAUNCH(n ? 1 : 0);
         launch_update(d_image, ctx->d_corr, d_sens, dmax, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
         CHECK_LAUNCH(1);
@@ -252,6 +261,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             if (!(value >= 0.0) || !isfinite(value)) return fail(ctx, TOFMLEM_EINVAL, "shell_mm must be >= 0");
             ctx->shell_mm = value;
             return TOFMLEM_OK;
+        case TOFMLEM_OPT_CTA_INTERLEAVE:
+            if (value < 1 || value > 65536 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "cta_interleave in 1..65536");
+            ctx->cta_interleave = (unsigned)value;
+            return TOFMLEM_OK;
         default:
             return fail(ctx, TOFMLEM_EINVAL, "unknown option key");
     }
@@ -266,7 +279,7 @@ int tofmlem_sensitivity(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t m
     CU(cudaMemsetAsync(d_sens, 0, ctx->nvox * sizeof(float), ctx->stream));
     EventPtrs ev = ev_ptrs(lors);
     ev.dt = nullptr;
-    launch_backproject(p, false, ev, m, nullptr, d_sens, ctx->stream);
+    launch_backproject(p, false, ev, m, nullptr, d_sens, vec_ok(ctx, d_sens), ctx->stream);
     CHECK_LAUNCH(1);
     launch_scale(d_sens, (float)(1.0 / (double)m), ctx->nvox, ctx->stream);
     CHECK_LAUNCH(1);
@@ -286,7 +299,8 @@ int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, 
     if (!ctx) return TOFMLEM_EINVAL;
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || !d_out || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "backproject: bad argument");
-    launch_backproject(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_values, d_out, ctx->stream);
+    launch_backproject(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_values, d_out, vec_ok(ctx, d_out),
+                       ctx->stream);
     CHECK_LAUNCH(1);
     return TOFMLEM_OK;
 }
@@ -302,8 +316,8 @@ int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n
     if (!ctx) return TOFMLEM_EINVAL;
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || !d_image || !d_corr || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "em_correction: bad argument");
-    launch_em_correction(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_corr, ctx->d_stats,
-                         ctx->stream);
+    launch_em_correction(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_corr, vec_ok(ctx, d_corr),
+                         ctx->d_stats, ctx->stream);
     CHECK_LAUNCH(1);
     ctx->last_n += n;
     return TOFMLEM_OK;
@@ -377,14 +391,14 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
                     CU(cudaMemcpyAsync(d + f * stride + off, hsrc[f] + off, m * sizeof(float), cudaMemcpyHostToDevice, cs));
             CU(cudaEventRecord(ctx->chunk_done[slot], cs));
             CU(cudaStreamWaitEvent(s, ctx->chunk_done[slot], 0));
-            launch_em_correction(p, ctx->tof, ev_ptrs(&dev, off), m, ctx->d_himg, ctx->d_corr, ctx->d_stats, s);
+            launch_em_correction(p, ctx->tof, ev_ptrs(&dev, off), m, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, s);
             CHECK_LAUNCH(1);
         }
         launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
         CHECK_LAUNCH(1);
         for (int it = 1; it < iters; ++it) {
             CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), s));
-            launch_em_correction(p, ctx->tof, ev_ptrs(&dev), n, ctx->d_himg, ctx->d_corr, ctx->d_stats, s);
+            launch_em_correction(p, ctx->tof, ev_ptrs(&dev), n, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, s);
             CHECK_LAUNCH(1);
             launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
             CHECK_LAUNCH(1);

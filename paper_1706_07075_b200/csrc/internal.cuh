@@ -14,14 +14,13 @@ constexpr double kCmmPerPs = 0.299792458;  // speed of light, mm/ps
 // Geometry + TOF constants of one context, passed by value to the projector kernels.
 // Per-event ray set-up is done in fp64 from these; the voxel walk is fp32 in a window-local frame.
 struct ProjParams {
-    int nx, ny, nz;
-    double vx, vy, vz;     // voxel size
-    double ivx, ivy, ivz;  // 1 / voxel size
-    double ox, oy, oz;     // low corner
-    double hx, hy, hz;     // high corner o + n*v
+    int n[3];              // nx, ny, nz
+    double v[3], iv[3];    // voxel size and its reciprocal
+    double o[3], h[3];     // low corner, high corner o + n*v
     double half_window;    // trunc_sigmas * sigma (mm); unused for non-TOF
     float gauss_a;         // -log2(e) / (2 sigma^2): weight = l * 2^(gauss_a * t^2)
     float gauss_norm;      // 1 / (sigma sqrt(2 pi))
+    unsigned stride;       // CTA interleave of the scatter kernels (<= 1: natural order)
 };
 
 struct EventPtrs {
@@ -43,10 +42,11 @@ struct GridF32 {
 // ---- projector.cu
 void launch_forward(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *image, float *fwd,
                     cudaStream_t s);
+// vec_ok: `out`/`corr` is 16-byte aligned and its allocation covers whole groups of 4 voxels
 void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *values,
-                        float *out, cudaStream_t s);
+                        float *out, bool vec_ok, cudaStream_t s);
 void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *image,
-                          float *corr, DeviceStats *stats, cudaStream_t s);
+                          float *corr, bool vec_ok, DeviceStats *stats, cudaStream_t s);
 
 // ---- image_ops.cu
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);

@@ -12,7 +12,8 @@ __device__ __forceinline__ uint32_t mix32(uint32_t x) {
     return x;
 }
 
-// kind: 0 random RED, 1 row-coalesced RED, 2 random gather, 3 row-coalesced gather
+// kind: 0 random RED, 1 row-coalesced RED, 2 random gather, 3 row-coalesced gather,
+//       4 random 8-byte vector RED (red.global.add.v2.f32), 5 random 16-byte vector RED (v4)
 template <int KIND>
 __global__ void __launch_bounds__(256) probe_kernel(float *buf, uint32_t n, int ops, float *sink) {
     const uint32_t tid = blockIdx.x * 256u + threadIdx.x;
@@ -29,10 +30,14 @@ __global__ void __launch_bounds__(256) probe_kernel(float *buf, uint32_t n, int 
             a = h % n;
         if (KIND < 2)
             atomicAdd(buf + a, 1.0f);
+        else if (KIND == 4)
+            asm volatile("red.global.add.v2.f32 [%0], {%1, %1};" ::"l"(buf + (a & ~1u)), "f"(1.0f) : "memory");
+        else if (KIND == 5)
+            asm volatile("red.global.add.v4.f32 [%0], {%1, %1, %1, %1};" ::"l"(buf + (a & ~3u)), "f"(1.0f) : "memory");
         else
             acc += __ldg(buf + a);
     }
-    if (KIND >= 2 && acc == 123.456f) *sink = acc;
+    if ((KIND == 2 || KIND == 3) && acc == 123.456f) *sink = acc;
 }
 
 int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *ms, cudaStream_t s) {
@@ -51,6 +56,8 @@ int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *m
             case 1: probe_kernel<1><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
             case 2: probe_kernel<2><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
             case 3: probe_kernel<3><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            case 4: probe_kernel<4><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            case 5: probe_kernel<5><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
             default: cudaEventDestroy(a); cudaEventDestroy(b); return -1;
         }
         cudaEventRecord(b, s);
