@@ -149,6 +149,7 @@ def main():
 
     import paper_1706_07075_b200 as pkg
     import synth
+    from paper_1706_07075_b200 import sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -175,7 +176,8 @@ def main():
         return a.elapsed_time(b)
 
     # ---- inputs (synthetic, seeded; resident in HBM before any timed region)
-    ev = synth.make_events_chunked(cfg, n, start=rank * n, device=dev)
+    ev_start, _ = sharding.weak_shard_range(n, rank)
+    ev = synth.make_events_chunked(cfg, n, start=ev_start, device=dev)
     sens = torch.empty(nvox, dtype=torch.float32, device=dev)
     lors = synth.make_sens_lors_chunked(cfg, m, device=dev)
     sens_ms = timed(lambda: ctx.sensitivity(lors, m, sens))
@@ -210,8 +212,7 @@ def main():
         ctx.em_correction(ev, n, image, corr)
         if i is not None:
             k_stop[i].record()
-        if world > 1:
-            dist.all_reduce(corr)
+        sharding.allreduce_correction(corr)  # N > 1: the iteration's one exchange (NCCL sum of the partial corrections)
         ctx.update(image, corr, sens)
 
     for _ in range(args.warmup):
@@ -234,10 +235,7 @@ def main():
     total_ms = t0.elapsed_time(t1)
     launches = ctx.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = sharding.max_over_ranks_ms(total_ms, dev)
     ms_per_step = total_ms / args.steps
     value = world * n / (ms_per_step * 1e-3)
     st = ctx.get_stats()
@@ -286,10 +284,7 @@ def main():
         for _ in range(reps):
             ctx.iterate_host(h_ev, n, h_img, h_sens, 1)
         e2e_s = (time.perf_counter() - tt) / reps
-        if world > 1:
-            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = sharding.max_over_ranks_ms(e2e_s, dev)
         e2e = {"value": world * n / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 28 * n + 8 * nvox,
                "d2h_bytes_per_step": 4 * nvox, "ms_per_step": e2e_s * 1e3,
                "call": "tofmlem_iterate_host(iters=1), pinned host buffers, binned event order"}
