@@ -75,6 +75,8 @@ enum {
     TOFMLEM_OPT_PROJECTOR = 4,      /* 0 = Siddon x Gaussian (default); 1 = paper's K-sample LUT */
     TOFMLEM_OPT_SAMPLES_K = 5,      /* K of the sampled projector, default 32 */
     TOFMLEM_OPT_SHELL_MM = 6,       /* extra shell added to the region margin, default 6 mm */
+    TOFMLEM_OPT_EM_VARIANT = 8,     /* fused EM pass scheduling (performance only): 0 = persistent kernel with one work
+                                       queue per SM (default), 1 = one CTA per 256-event chunk in grid order */
     TOFMLEM_OPT_CTA_INTERLEAVE = 7  /* scatter kernels: number of list segments advanced in parallel (default 64;
                                        1 = natural order).  Performance only, results are the same up to the
                                        order of the float32 reductions. */

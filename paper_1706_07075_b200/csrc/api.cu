@@ -22,9 +22,11 @@ struct tofmlem_ctx {
     // scratch owned by the context
     float *d_corr = nullptr;  // padded to whole groups of 4 voxels
     unsigned cta_interleave = 64;
+    int em_variant = 0;
     float *d_max = nullptr;          // max(sens) of the current iterate call
     const float *d_max_ext = nullptr;  // region sub-contexts use the parent's global max
     DeviceStats *d_stats = nullptr;
+    unsigned *d_queues = nullptr;  // work counters of the persistent EM kernel
     uint32_t *d_hist = nullptr, *d_cursor = nullptr;
     size_t hist_cap = 0;
     unsigned long long *d_rcounts = nullptr;  // 2*(kMaxRegions+1)
@@ -90,6 +92,7 @@ ProjParams make_params(const tofmlem_ctx *c, bool tof) {
         p.gauss_norm = 1.0f;
     }
     p.stride = c->cta_interleave;
+    p.variant = c->em_variant;
     return p;
 }
 
@@ -158,7 +161,7 @@ int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, float *d_i
     CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
     for (int it = 0; it < iters; ++it) {
         CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), ctx->stream));
-        launch_em_correction(p, ctx->tof, ev, n, d_image, ctx->d_corr, true, ctx->d_stats, ctx->stream);
+        launch_em_correction(p, ctx->tof, ev, n, d_image, ctx->d_corr, true, ctx->d_stats, ctx->d_queues, ctx->stream);
         CHECK_LAUNCH(n ? 1 : 0);
         launch_update(d_image, ctx->d_corr, d_sens, dmax, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
         CHECK_LAUNCH(1);
@@ -195,6 +198,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
     ctx->nvox = nvox;
     cudaError_t e = cudaMalloc(&ctx->d_max, sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, sizeof(DeviceStats));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_queues, kMaxQueues * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_rcounts, 2 * (kMaxRegions + 1) * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_stats, 0, sizeof(DeviceStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_max, 0, sizeof(float), ctx->stream);
@@ -202,6 +206,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
         int rc = e == cudaErrorMemoryAllocation ? TOFMLEM_ENOMEM : TOFMLEM_ECUDA;
         cudaFree(ctx->d_max);
         cudaFree(ctx->d_stats);
+        cudaFree(ctx->d_queues);
         cudaFree(ctx->d_rcounts);
         delete ctx;
         return rc;
@@ -222,6 +227,7 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_corr);
     cudaFree(ctx->d_max);
     cudaFree(ctx->d_stats);
+    cudaFree(ctx->d_queues);
     cudaFree(ctx->d_hist);
     cudaFree(ctx->d_cursor);
     cudaFree(ctx->d_rcounts);
@@ -264,6 +270,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
         case TOFMLEM_OPT_CTA_INTERLEAVE:
             if (value < 1 || value > 65536 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "cta_interleave in 1..65536");
             ctx->cta_interleave = (unsigned)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_EM_VARIANT:
+            if (value < 0 || value > 1 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "em_variant in 0..1");
+            ctx->em_variant = (int)value;
             return TOFMLEM_OK;
         default:
             return fail(ctx, TOFMLEM_EINVAL, "unknown option key");
@@ -317,7 +327,7 @@ int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || !d_image || !d_corr || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "em_correction: bad argument");
     launch_em_correction(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_corr, vec_ok(ctx, d_corr),
-                         ctx->d_stats, ctx->stream);
+                         ctx->d_stats, ctx->d_queues, ctx->stream);
     CHECK_LAUNCH(1);
     ctx->last_n += n;
     return TOFMLEM_OK;
@@ -391,14 +401,14 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
                     CU(cudaMemcpyAsync(d + f * stride + off, hsrc[f] + off, m * sizeof(float), cudaMemcpyHostToDevice, cs));
             CU(cudaEventRecord(ctx->chunk_done[slot], cs));
             CU(cudaStreamWaitEvent(s, ctx->chunk_done[slot], 0));
-            launch_em_correction(p, ctx->tof, ev_ptrs(&dev, off), m, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, s);
+            launch_em_correction(p, ctx->tof, ev_ptrs(&dev, off), m, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, ctx->d_queues, s);
             CHECK_LAUNCH(1);
         }
         launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
         CHECK_LAUNCH(1);
         for (int it = 1; it < iters; ++it) {
             CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), s));
-            launch_em_correction(p, ctx->tof, ev_ptrs(&dev), n, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, s);
+            launch_em_correction(p, ctx->tof, ev_ptrs(&dev), n, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, ctx->d_queues, s);
             CHECK_LAUNCH(1);
             launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
             CHECK_LAUNCH(1);

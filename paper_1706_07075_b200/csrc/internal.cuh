@@ -21,6 +21,7 @@ struct ProjParams {
     float gauss_a;         // -log2(e) / (2 sigma^2): weight = l * 2^(gauss_a * t^2)
     float gauss_norm;      // 1 / (sigma sqrt(2 pi))
     unsigned stride;       // CTA interleave of the scatter kernels (<= 1: natural order)
+    int variant;           // fused EM pass: 0 = persistent per-SM queues (default), 1 = grid order
 };
 
 struct EventPtrs {
@@ -45,8 +46,10 @@ void launch_forward(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t
 // vec_ok: `out`/`corr` is 16-byte aligned and its allocation covers whole groups of 4 voxels
 void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *values,
                         float *out, bool vec_ok, cudaStream_t s);
+// queues: kMaxQueues work counters owned by the context (persistent variant), may be NULL
+constexpr int kMaxQueues = 2048;
 void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *image,
-                          float *corr, bool vec_ok, DeviceStats *stats, cudaStream_t s);
+                          float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues, cudaStream_t s);
 
 // ---- image_ops.cu
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);

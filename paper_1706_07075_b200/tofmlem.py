@@ -19,6 +19,7 @@ EVENT_FIELDS = ("x1", "y1", "z1", "x2", "y2", "z2", "dt")
 TOFMLEM_OK, TOFMLEM_EINVAL, TOFMLEM_ENOMEM, TOFMLEM_ECUDA, TOFMLEM_ESTATE, TOFMLEM_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 OPT_TRUNC_SIGMAS, OPT_SENS_FLOOR_REL, OPT_TILE_LOG2, OPT_PROJECTOR, OPT_SAMPLES_K, OPT_SHELL_MM = 1, 2, 3, 4, 5, 6
 OPT_CTA_INTERLEAVE = 7
+OPT_EM_VARIANT = 8
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = (
