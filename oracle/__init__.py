@@ -66,6 +66,8 @@ def lib():
         _lib.orc_sigma_mm.argtypes = [C.c_double, C.c_double]
         _lib.orc_lor_weights.restype = C.c_int
         _lib.orc_em_correction.restype = C.c_uint64
+        _lib.orc_em_correction_w.restype = C.c_uint64
+        _lib.orc_lor_samples.restype = C.c_int
         _lib.orc_num_bins.restype = C.c_uint32
         _lib.orc_region_margin_slices.restype = C.c_int32
         _lib.orc_region_margin_slices.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double]
@@ -127,17 +129,19 @@ def lor_weights(g: Grid, sigma: float, p1, p2, dt_ps: float = 0.0, trunc: float 
     return idx[:cnt].copy(), w[:cnt].copy()
 
 
-def forward(g: Grid, sigma: float, ev, image, trunc: float = 3.0) -> np.ndarray:
+def forward(g: Grid, sigma: float, ev, image, trunc: float = 3.0, K: int = 0) -> np.ndarray:
+    """fwd_e = sum_j a_ej x_j; K = 0: Siddon x Gaussian rows, K >= 1: the paper's K-sample kernel."""
     e, n, keep = _events(ev, sigma > 0)
     img = np.ascontiguousarray(np.asarray(image, dtype=np.float64).reshape(-1))
     assert img.size == g.nvox
     out = np.empty(n, np.float64)
-    lib().orc_forward(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.byref(e), C.c_uint64(n),
-                      img.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p))
+    lib().orc_forward_k(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.c_int(K), C.byref(e), C.c_uint64(n),
+                        img.ctypes.data_as(C.c_void_p), out.ctypes.data_as(C.c_void_p))
     return out
 
 
-def backproject(g: Grid, sigma: float, ev, values: Optional[np.ndarray] = None, trunc: float = 3.0) -> np.ndarray:
+def backproject(g: Grid, sigma: float, ev, values: Optional[np.ndarray] = None, trunc: float = 3.0,
+                K: int = 0) -> np.ndarray:
     e, n, keep = _events(ev, sigma > 0)
     out = np.zeros(g.nvox, np.float64)
     vals = None
@@ -146,8 +150,8 @@ def backproject(g: Grid, sigma: float, ev, values: Optional[np.ndarray] = None, 
         vals = np.ascontiguousarray(np.asarray(values, dtype=np.float64))
         assert vals.shape == (n,)
         vp = vals.ctypes.data_as(C.c_void_p)
-    lib().orc_backproject(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.byref(e), C.c_uint64(n), vp,
-                          out.ctypes.data_as(C.c_void_p))
+    lib().orc_backproject_k(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.c_int(K), C.byref(e), C.c_uint64(n),
+                            vp, out.ctypes.data_as(C.c_void_p))
     return out
 
 
@@ -166,14 +170,24 @@ def mask_f32(sens_f32: np.ndarray, floor_rel: float = 1e-2) -> np.ndarray:
     return m
 
 
-def em_correction(g: Grid, sigma: float, ev, image, trunc: float = 3.0):
-    """(corr float64[nvox], n_valid, visits) of one pass."""
+def _f64_or_none(a, n):
+    if a is None:
+        return None, None
+    v = np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+    assert v.shape == (n,)
+    return v, v.ctypes.data_as(C.c_void_p)
+
+
+def em_correction(g: Grid, sigma: float, ev, image, trunc: float = 3.0, K: int = 0, weights=None):
+    """(corr float64[nvox], n_valid, visits) of one pass; `weights`: optional per-event weights (NEXT-3)."""
     e, n, keep = _events(ev, sigma > 0)
     img = np.ascontiguousarray(np.asarray(image, dtype=np.float64).reshape(-1))
     corr = np.empty(g.nvox, np.float64)
     vis = C.c_uint64(0)
-    nv = lib().orc_em_correction(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.byref(e), C.c_uint64(n),
-                                 img.ctypes.data_as(C.c_void_p), corr.ctypes.data_as(C.c_void_p), C.byref(vis))
+    wk, wp = _f64_or_none(weights, n)
+    nv = lib().orc_em_correction_w(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.c_int(K), C.byref(e),
+                                   C.c_uint64(n), wp, img.ctypes.data_as(C.c_void_p),
+                                   corr.ctypes.data_as(C.c_void_p), C.byref(vis), None)
     return corr, int(nv), int(vis.value)
 
 
@@ -187,17 +201,91 @@ def update(image, corr, sens_f32, mask) -> np.ndarray:
     return img
 
 
-def mlem(g: Grid, sigma: float, ev, image0, sens_f32, iters: int, floor_rel: float = 1e-2, trunc: float = 3.0):
-    """(image float64[nvox] after `iters` iterations, Stats)."""
+def mlem(g: Grid, sigma: float, ev, image0, sens_f32, iters: int, floor_rel: float = 1e-2, trunc: float = 3.0,
+         K: int = 0, weights=None, median: bool = False):
+    """(image float64[nvox] after `iters` iterations, Stats).  K: row model (0 = Siddon x Gaussian);
+    weights: optional per-event weights (NEXT-3); median: 3x3x3 median filter after every iteration (NEXT-2)."""
     e, n, keep = _events(ev, sigma > 0)
     img = np.ascontiguousarray(np.asarray(image0, dtype=np.float64).reshape(-1)).copy()
     s = _f32(sens_f32).reshape(-1)
     assert img.size == g.nvox and s.size == g.nvox
     st = Stats()
-    lib().orc_mlem(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.byref(e), C.c_uint64(n),
-                   img.ctypes.data_as(C.c_void_p), s.ctypes.data_as(C.c_void_p), C.c_int(iters),
-                   C.c_float(floor_rel), C.byref(st))
+    wk, wp = _f64_or_none(weights, n)
+    lib().orc_mlem_x(C.byref(g), C.c_double(sigma), C.c_double(trunc), C.c_int(K), C.byref(e), C.c_uint64(n), wp,
+                     img.ctypes.data_as(C.c_void_p), s.ctypes.data_as(C.c_void_p), C.c_int(iters),
+                     C.c_float(floor_rel), C.c_int(1 if median else 0), C.byref(st))
     return img, st
+
+
+def sample_lut(K: int, sigma: float, trunc: float = 3.0):
+    """(offsets mm float64[K], weights float64[K]) of the paper's K-sample TOF kernel."""
+    off = np.empty(K, np.float64)
+    w = np.empty(K, np.float64)
+    lib().orc_sample_lut(C.c_int(K), C.c_double(sigma), C.c_double(trunc), off.ctypes.data_as(C.c_void_p),
+                         w.ctypes.data_as(C.c_void_p))
+    return off, w
+
+
+def lor_samples(g: Grid, sigma: float, K: int, p1, p2, dt_ps: float = 0.0, trunc: float = 3.0):
+    """(voxel indices, weights) of one event under the K-sample kernel, in sample order (dropped samples omitted)."""
+    off, w = sample_lut(K, sigma, trunc)
+    idx = np.empty(K, np.int64)
+    ww = np.empty(K, np.float64)
+    a = (C.c_double * 3)(*map(float, p1))
+    b = (C.c_double * 3)(*map(float, p2))
+    cnt = lib().orc_lor_samples(C.byref(g), C.c_int(K), off.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p),
+                                a, b, C.c_double(dt_ps), idx.ctypes.data_as(C.c_void_p),
+                                ww.ctypes.data_as(C.c_void_p))
+    return idx[:cnt].copy(), ww[:cnt].copy()
+
+
+def median3(g: Grid, image) -> np.ndarray:
+    """3x3x3 median filter, edges replicated (NEXT-2, R23)."""
+    img = np.ascontiguousarray(np.asarray(image, dtype=np.float64).reshape(-1))
+    assert img.size == g.nvox
+    out = np.empty(g.nvox, np.float64)
+    lib().orc_median3(C.c_int32(g.nx), C.c_int32(g.ny), C.c_int32(g.nz), img.ctypes.data_as(C.c_void_p),
+                      out.ctypes.data_as(C.c_void_p))
+    return out
+
+
+def attenuation_weights(g: Grid, ev, mu) -> np.ndarray:
+    """w_e = exp(+ line integral of mu (1/mm) along the LOR inside the grid) (NEXT-3, R19)."""
+    e, n, keep = _events({**ev, "dt": None}, False)
+    m = np.ascontiguousarray(np.asarray(mu, dtype=np.float64).reshape(-1))
+    assert m.size == g.nvox
+    out = np.empty(n, np.float64)
+    lib().orc_attenuation_weights(C.byref(g), C.byref(e), C.c_uint64(n), m.ctypes.data_as(C.c_void_p),
+                                  out.ctypes.data_as(C.c_void_p))
+    return out
+
+
+CONF95_Z = 1.959964  # two-sided 95 % point of the normal distribution (PAPER.md:63 "95% confidence level")
+
+
+def scatter_half_width_f32(sigma: float, conf_z: float = CONF95_Z) -> np.float32:
+    return np.float32(conf_z * sigma)
+
+
+def ellipsoids_f32(shapes) -> np.ndarray:
+    """float32[n,6] = (cx, cy, cz, 1/ax, 1/ay, 1/az) from (centre, semi-axes) pairs; the reciprocals are taken
+    in float64 and rounded once (both sides receive this same array)."""
+    out = np.empty((len(shapes), 6), np.float32)
+    for i, (c, s) in enumerate(shapes):
+        out[i, :3] = np.asarray(c, np.float64)
+        out[i, 3:] = 1.0 / np.asarray(s, np.float64)
+    return out
+
+
+def scatter_keep(ev, ell_f32: np.ndarray, h_f32) -> Tuple[np.ndarray, int]:
+    """(keep uint8[n], n_kept): TOF-based scatter rejection against a union of ellipsoids (NEXT-4, spec F2)."""
+    e, n, keepalive = _events(ev, True)
+    ell = np.ascontiguousarray(np.asarray(ell_f32, dtype=np.float32).reshape(-1, 6))
+    keep = np.empty(n, np.uint8)
+    cnt = C.c_uint64(0)
+    lib().orc_scatter_keep(C.byref(e), C.c_uint64(n), ell.ctypes.data_as(C.c_void_p), C.c_int(ell.shape[0]),
+                           C.c_float(float(h_f32)), keep.ctypes.data_as(C.c_void_p), C.byref(cnt))
+    return keep, int(cnt.value)
 
 
 def num_bins(g: Grid, tile_log2: int = 3) -> int:

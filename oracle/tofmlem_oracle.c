@@ -39,6 +39,22 @@
  * P7/P8/P10 ("parity unpinned" for image values on realistic data is NOT claimed pinned);
  * split-vs-unsplit agreement is parity unpinned (PAPER.md:212 is visual only).
  *
+ *
+ * Widened rows (added after the hot path):
+ *   - NEXT-1, the paper's own K-sample TOF kernel (Fig. 3): K equally spaced samples inside
+ *     the truncated Gaussian, Gaussian weights normalised to sum to one, each sample filled into the voxel
+ *     that contains it ("direct technique for voxel filling") -- orc_sample_lut, orc_*_k.
+ *     Pins P13: weights sum to 1 / symmetric / printed K = 15, 32; uniform image -> fwd = 1; K -> inf
+ *     converges to the Siddon-TOF forward value / erf(T/sqrt 2).
+ *   - NEXT-2, the median filter applied to the image estimate after each iteration (size
+ *     unstated -> R23: 3x3x3, edges replicated) -- orc_median3.  Pin P14: scipy.ndimage.median_filter.
+ *   - NEXT-3, attenuation correction as a per-event weight (PAPER.md:93 -> R19: w_e = 1 / P(both photons
+ *     survive) = exp(+ line integral of mu along the LOR), multiplying the backprojected ratio)
+ *     -- orc_attenuation_weights, the `evw` argument of orc_em_correction_w.  Pins P15.
+ *   - NEXT-4, TOF-based scatter rejection: an event is kept iff the 95 % confidence
+ *     interval of its TOF-estimated annihilation point (+-1.96 sigma along the LOR) meets the body outline,
+ *     here a union of ellipsoids; float32 specification F2 -- orc_scatter_keep.  Pins P16.
+ *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -fPIC -shared (no -ffast-math).
  */
 #include <math.h>
@@ -187,6 +203,61 @@ int orc_lor_weights(const orc_grid *g, double sigma_mm, double trunc_sigmas, con
     return cnt;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * NEXT-1: the paper's K-sample TOF kernel (Fig. 3 :83; SURVEY.md 8(c) "variant V").
+ * offset_k = -T sigma + k * 2 T sigma / (K - 1), k = 0..K-1  ("equally spaced inside the ... Gaussian");
+ * weight_k = exp(-offset_k^2 / 2 sigma^2) / sum_m exp(-offset_m^2 / 2 sigma^2)  ("the sum of the weights
+ * equaled one").  K = 1 degenerates to one sample at the centre with weight 1.
+ * ------------------------------------------------------------------------------------------ */
+void orc_sample_lut(int K, double sigma_mm, double trunc_sigmas, double *offset, double *weight) {
+    double sum = 0.0;
+    for (int k = 0; k < K; ++k) {
+        offset[k] = K > 1 ? -trunc_sigmas * sigma_mm + (double)k * (2.0 * trunc_sigmas * sigma_mm) / (double)(K - 1) : 0.0;
+        const double r = offset[k] / sigma_mm;
+        weight[k] = exp(-0.5 * r * r);
+        sum += weight[k];
+    }
+    for (int k = 0; k < K; ++k) weight[k] /= sum;
+}
+
+/* Row of one event under the K-sample kernel: sample k sits at s_k = s_c + offset_k on the LOR
+ * ("centered in the coincidence time difference") and is filled into the voxel that contains
+ * it; samples beyond the LOR's end points or outside the grid are dropped (R8).  Returns the number of
+ * (voxel, weight) pairs kept (<= K); the same voxel may appear more than once. */
+int orc_lor_samples(const orc_grid *g, int K, const double *offset, const double *weight, const double p1[3],
+                    const double p2[3], double dt_ps, int64_t *idx, double *w) {
+    const int n[3] = {g->nx, g->ny, g->nz};
+    const double v[3] = {g->vx, g->vy, g->vz};
+    const double o[3] = {g->ox, g->oy, g->oz};
+    double d[3], u[3];
+    int a;
+    for (a = 0; a < 3; ++a) {
+        if (!isfinite(p1[a]) || !isfinite(p2[a])) return 0;
+        d[a] = p2[a] - p1[a];
+    }
+    if (!isfinite(dt_ps)) return 0;
+    const double L = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    if (!(L > 0.0)) return 0;
+    for (a = 0; a < 3; ++a) u[a] = d[a] / L;
+    const double s_c = 0.5 * L + 0.5 * ORC_C_MM_PER_PS * dt_ps;
+    int cnt = 0;
+    for (int k = 0; k < K; ++k) {
+        const double s = s_c + offset[k];
+        if (s < 0.0 || s > L) continue;
+        int64_t ijk[3];
+        int inside = 1;
+        for (a = 0; a < 3; ++a) {
+            ijk[a] = (int64_t)floor((p1[a] + u[a] * s - o[a]) / v[a]);
+            if (ijk[a] < 0 || ijk[a] >= n[a]) inside = 0;
+        }
+        if (!inside) continue;
+        idx[cnt] = (ijk[2] * g->ny + ijk[1]) * (int64_t)g->nx + ijk[0];
+        w[cnt] = weight[k];
+        ++cnt;
+    }
+    return cnt;
+}
+
 typedef struct {
     int64_t *idx;
     double *w, *scratch;
@@ -205,43 +276,86 @@ static void lor_buf_free(lor_buf *b) {
     free(b->scratch);
 }
 
-static int event_row(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t e, lor_buf *b) {
+/* Which system-matrix row an entry point uses: K = 0 -> Siddon chords x Gaussian at the chord midpoints (the graded
+ * projector, R2); K >= 1 -> the paper's K-sample kernel (NEXT-1). */
+typedef struct {
+    int K;
+    double *offset, *weight;
+} row_model;
+
+static void row_model_init(row_model *rm, int K, double sigma_mm, double trunc) {
+    rm->K = K;
+    rm->offset = rm->weight = NULL;
+    if (K > 0) {
+        rm->offset = (double *)malloc(sizeof(double) * (size_t)K);
+        rm->weight = (double *)malloc(sizeof(double) * (size_t)K);
+        orc_sample_lut(K, sigma_mm, trunc, rm->offset, rm->weight);
+    }
+}
+static void row_model_free(row_model *rm) {
+    free(rm->offset);
+    free(rm->weight);
+}
+
+static void lor_buf_init_k(lor_buf *b, const orc_grid *g, int K) {
+    lor_buf_init(b, g);
+    if (K > b->cap) {
+        lor_buf_free(b);
+        b->cap = K;
+        b->idx = (int64_t *)malloc(sizeof(int64_t) * (size_t)K);
+        b->w = (double *)malloc(sizeof(double) * (size_t)K);
+        b->scratch = (double *)malloc(sizeof(double) * (size_t)K);
+    }
+}
+
+static int event_row(const orc_grid *g, double sigma_mm, double trunc, const row_model *rm, const orc_events *ev,
+                     uint64_t e, lor_buf *b) {
     const double p1[3] = {ev->x1[e], ev->y1[e], ev->z1[e]};
     const double p2[3] = {ev->x2[e], ev->y2[e], ev->z2[e]};
     const double dt = (sigma_mm > 0.0 && ev->dt) ? (double)ev->dt[e] : 0.0;
+    if (rm->K > 0) return orc_lor_samples(g, rm->K, rm->offset, rm->weight, p1, p2, dt, b->idx, b->w);
     return orc_lor_weights(g, sigma_mm, trunc, p1, p2, dt, b->idx, b->w, b->scratch, b->cap);
 }
 
 /* step 5: fwd_e = sum_j a_ej x_j */
-void orc_forward(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n,
-                 const double *image, double *fwd) {
+void orc_forward_k(const orc_grid *g, double sigma_mm, double trunc, int K, const orc_events *ev, uint64_t n,
+                   const double *image, double *fwd) {
+    row_model rm;
+    row_model_init(&rm, K, sigma_mm, trunc);
 #pragma omp parallel
     {
         lor_buf b;
-        lor_buf_init(&b, g);
+        lor_buf_init_k(&b, g, K);
 #pragma omp for schedule(dynamic, 1024)
         for (int64_t e = 0; e < (int64_t)n; ++e) {
-            const int cnt = event_row(g, sigma_mm, trunc, ev, (uint64_t)e, &b);
+            const int cnt = event_row(g, sigma_mm, trunc, &rm, ev, (uint64_t)e, &b);
             double acc = 0.0;
             for (int k = 0; k < cnt; ++k) acc += b.w[k] * image[b.idx[k]];
             fwd[e] = acc;
         }
         lor_buf_free(&b);
     }
+    row_model_free(&rm);
+}
+void orc_forward(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n,
+                 const double *image, double *fwd) {
+    orc_forward_k(g, sigma_mm, trunc, 0, ev, n, image, fwd);
 }
 
 /* step 5: out_j += a_ej * val_e   (values == NULL => 1) */
-void orc_backproject(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n,
-                     const double *values, double *out) {
+void orc_backproject_k(const orc_grid *g, double sigma_mm, double trunc, int K, const orc_events *ev, uint64_t n,
+                       const double *values, double *out) {
     const int64_t nvox = (int64_t)g->nx * g->ny * g->nz;
+    row_model rm;
+    row_model_init(&rm, K, sigma_mm, trunc);
 #pragma omp parallel
     {
         lor_buf b;
-        lor_buf_init(&b, g);
+        lor_buf_init_k(&b, g, K);
         double *priv = (double *)calloc((size_t)nvox, sizeof(double));
 #pragma omp for schedule(dynamic, 1024)
         for (int64_t e = 0; e < (int64_t)n; ++e) {
-            const int cnt = event_row(g, sigma_mm, trunc, ev, (uint64_t)e, &b);
+            const int cnt = event_row(g, sigma_mm, trunc, &rm, ev, (uint64_t)e, &b);
             const double val = values ? values[e] : 1.0;
             for (int k = 0; k < cnt; ++k) priv[b.idx[k]] += b.w[k] * val;
         }
@@ -250,6 +364,11 @@ void orc_backproject(const orc_grid *g, double sigma_mm, double trunc, const orc
         free(priv);
         lor_buf_free(&b);
     }
+    row_model_free(&rm);
+}
+void orc_backproject(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n,
+                     const double *values, double *out) {
+    orc_backproject_k(g, sigma_mm, trunc, 0, ev, n, values, out);
 }
 
 /* step 7: sens_j = (1/m) sum_i l_ij over the m given LORs (non-TOF chords), R10 */
@@ -270,28 +389,34 @@ void orc_mask_f32(const float *sens, int64_t nvox, float floor_rel, uint8_t *mas
     for (int64_t j = 0; j < nvox; ++j) mask[j] = (sens[j] >= thr && sens[j] > 0.0f) ? 1 : 0;
 }
 
-/* EM correction image of one pass (step 6, first half): corr_j = sum_{e: fwd_e>0} a_ej / fwd_e.
- * corr is overwritten.  Returns n_valid; *visits (optional) counts voxel visits. */
-uint64_t orc_em_correction(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n,
-                           const double *image, double *corr, uint64_t *visits) {
+/* EM correction image of one pass (step 6, first half): corr_j = sum_{e: fwd_e>0} evw_e * a_ej / fwd_e.
+ * evw (optional, NULL => 1) is the per-event weight of NEXT-3 (R19).  corr is overwritten.
+ * Returns n_valid; *visits (optional) counts voxel visits; *sum_w (optional) = sum of evw over the valid events. */
+uint64_t orc_em_correction_w(const orc_grid *g, double sigma_mm, double trunc, int K, const orc_events *ev, uint64_t n,
+                             const double *evw, const double *image, double *corr, uint64_t *visits, double *sum_w) {
     const int64_t nvox = (int64_t)g->nx * g->ny * g->nz;
     uint64_t n_valid = 0, vis = 0;
+    double sw = 0.0;
+    row_model rm;
+    row_model_init(&rm, K, sigma_mm, trunc);
     memset(corr, 0, sizeof(double) * (size_t)nvox);
-#pragma omp parallel reduction(+ : n_valid, vis)
+#pragma omp parallel reduction(+ : n_valid, vis, sw)
     {
         lor_buf b;
-        lor_buf_init(&b, g);
+        lor_buf_init_k(&b, g, K);
         double *priv = (double *)calloc((size_t)nvox, sizeof(double));
 #pragma omp for schedule(dynamic, 1024)
         for (int64_t e = 0; e < (int64_t)n; ++e) {
-            const int cnt = event_row(g, sigma_mm, trunc, ev, (uint64_t)e, &b);
+            const int cnt = event_row(g, sigma_mm, trunc, &rm, ev, (uint64_t)e, &b);
             double fwd = 0.0;
             for (int k = 0; k < cnt; ++k) fwd += b.w[k] * image[b.idx[k]];
             vis += (uint64_t)(cnt > 0 ? cnt : 0);
             if (fwd > 0.0) { /* R9 */
-                const double r = 1.0 / fwd;
+                const double we = evw ? evw[e] : 1.0;
+                const double r = we / fwd;
                 for (int k = 0; k < cnt; ++k) priv[b.idx[k]] += b.w[k] * r;
                 ++n_valid;
+                sw += we;
             }
         }
 #pragma omp critical
@@ -299,8 +424,14 @@ uint64_t orc_em_correction(const orc_grid *g, double sigma_mm, double trunc, con
         free(priv);
         lor_buf_free(&b);
     }
+    row_model_free(&rm);
     if (visits) *visits = vis;
+    if (sum_w) *sum_w = sw;
     return n_valid;
+}
+uint64_t orc_em_correction(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n,
+                           const double *image, double *corr, uint64_t *visits) {
+    return orc_em_correction_w(g, sigma_mm, trunc, 0, ev, n, NULL, image, corr, visits, NULL);
 }
 
 /* step 6, second half: x_j <- mask_j ? x_j * corr_j / sens_j : 0 */
@@ -308,18 +439,50 @@ void orc_update(int64_t nvox, double *image, const double *corr, const float *se
     for (int64_t j = 0; j < nvox; ++j) image[j] = mask[j] ? image[j] * corr[j] / (double)sens[j] : 0.0;
 }
 
+/* NEXT-2: 3x3x3 median filter ("we introduced a median filter between MLEM iterations"; the size is
+ * not stated -> R23: the 27-voxel cube, edges replicated, i.e. neighbour indices are clamped to the volume).
+ * out_j = the 14th smallest of the 27 values.  in and out must not alias. */
+void orc_median3(int32_t nx, int32_t ny, int32_t nz, const double *in, double *out) {
+#pragma omp parallel for schedule(static)
+    for (int64_t z = 0; z < nz; ++z)
+        for (int64_t y = 0; y < ny; ++y)
+            for (int64_t x = 0; x < nx; ++x) {
+                double v[27];
+                int m = 0;
+                for (int dz = -1; dz <= 1; ++dz)
+                    for (int dy = -1; dy <= 1; ++dy)
+                        for (int dx = -1; dx <= 1; ++dx) {
+                            int64_t xx = x + dx, yy = y + dy, zz = z + dz;
+                            xx = xx < 0 ? 0 : (xx >= nx ? nx - 1 : xx);
+                            yy = yy < 0 ? 0 : (yy >= ny ? ny - 1 : yy);
+                            zz = zz < 0 ? 0 : (zz >= nz ? nz - 1 : zz);
+                            v[m++] = in[(zz * ny + yy) * nx + xx];
+                        }
+                qsort(v, 27, sizeof(double), cmp_double);
+                out[(z * ny + y) * nx + x] = v[13];
+            }
+}
+
 /* `iters` MLEM iterations in fp64 (R1). image: in x0, out x_iters.  sens is the float32 buffer
- * that is also given to the CUDA path (R11). */
-void orc_mlem(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n, double *image,
-              const float *sens, int iters, float sens_floor_rel, orc_stats *stats) {
+ * that is also given to the CUDA path (R11).  K: row model; evw: optional per-event weights (NEXT-3);
+ * median != 0: the 3x3x3 median filter is applied to the image estimate after every iteration
+ * ("applied to the image estimate after each iteration", R23). */
+void orc_mlem_x(const orc_grid *g, double sigma_mm, double trunc, int K, const orc_events *ev, uint64_t n,
+                const double *evw, double *image, const float *sens, int iters, float sens_floor_rel, int median,
+                orc_stats *stats) {
     const int64_t nvox = (int64_t)g->nx * g->ny * g->nz;
     uint8_t *mask = (uint8_t *)malloc((size_t)nvox);
     double *corr = (double *)malloc(sizeof(double) * (size_t)nvox);
+    double *tmp = median ? (double *)malloc(sizeof(double) * (size_t)nvox) : NULL;
     orc_mask_f32(sens, nvox, sens_floor_rel, mask);
     uint64_t n_valid = 0, visits = 0;
     for (int it = 0; it < iters; ++it) {
-        n_valid = orc_em_correction(g, sigma_mm, trunc, ev, n, image, corr, &visits);
+        n_valid = orc_em_correction_w(g, sigma_mm, trunc, K, ev, n, evw, image, corr, &visits, NULL);
         orc_update(nvox, image, corr, sens, mask);
+        if (median) {
+            orc_median3(g->nx, g->ny, g->nz, image, tmp);
+            memcpy(image, tmp, sizeof(double) * (size_t)nvox);
+        }
     }
     if (stats) {
         double s = 0.0;
@@ -331,6 +494,21 @@ void orc_mlem(const orc_grid *g, double sigma_mm, double trunc, const orc_events
     }
     free(mask);
     free(corr);
+    free(tmp);
+}
+void orc_mlem(const orc_grid *g, double sigma_mm, double trunc, const orc_events *ev, uint64_t n, double *image,
+              const float *sens, int iters, float sens_floor_rel, orc_stats *stats) {
+    orc_mlem_x(g, sigma_mm, trunc, 0, ev, n, NULL, image, sens, iters, sens_floor_rel, 0, stats);
+}
+
+/* NEXT-3 (R19): per-event attenuation weight w_e = 1 / P(both photons reach the detectors)
+ * = exp(+ sum_j l_ej mu_j), the non-TOF Siddon line integral of the attenuation map mu (1/mm, on the
+ * reconstruction grid) over the LOR's whole chord inside the grid.  Skipped LORs get weight 1. */
+void orc_attenuation_weights(const orc_grid *g, const orc_events *ev, uint64_t n, const double *mu, double *w) {
+    orc_events lor = *ev;
+    lor.dt = NULL;
+    orc_forward_k(g, 0.0, 0.0, 0, &lor, n, mu, w);
+    for (uint64_t e = 0; e < n; ++e) w[e] = exp(w[e]);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -455,4 +633,62 @@ void orc_region_ids(const orc_events *ev, uint64_t n, int n_regions, const float
 /* R12: margin in slices on each open side of a region core: ceil((trunc*sigma + shell_mm)/vz). */
 int32_t orc_region_margin_slices(double sigma_mm, double trunc, double shell_mm, double vz) {
     return (int32_t)ceil((trunc * sigma_mm + shell_mm) / vz);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-4: TOF-based scatter rejection (PAPER.md:63 Fig. 2, :69-71).  "The annihilation point determined
+ * along the scatter LOR had a certain probability of being inside the human body, according to the TOF
+ * resolution.  The limits of rejection were estimated at a 95% confidence level.  The body outline was
+ * determined from knowledge of the NCAT outline" -> reading R24: the event is KEPT iff the segment
+ * { c + u t : |t| <= h }, h = 1.959964 sigma (two-sided 95 % of the TOF Gaussian), c = TOF-estimated
+ * annihilation point, u = LOR direction, meets the body outline; the outline is a union of ellipsoids
+ * (the NCAT outline is not available; a measured one would be a CT mask).  Integer result -> float32
+ * specification F2, same conventions as F1 (single RN operations in this order, no contraction):
+ *   c, (dx,dy,dz), L as in F1;  ux = dx / L, uy = dy / L, uz = dz / L;
+ *   per ellipsoid (centre e, reciprocal semi-axes i, both float32 from the caller):
+ *     rx = (cx - ex) * ix ...;  wx = ux * ix ...;
+ *     A = (wx*wx + wy*wy) + wz*wz;  B = (rx*wx + ry*wy) + rz*wz;
+ *     t = -(B / A);  t = fminf(fmaxf(t, -h), h);          (point of the segment closest to the centre in the
+ *     px = rx + wx * t ...;                                  ellipsoid's unit-sphere coordinates)
+ *     Q = (px*px + py*py) + pz*pz;  hit iff Q <= 1.
+ *   keep = hit for any ellipsoid; invalid events (F1) are not kept.
+ * ------------------------------------------------------------------------------------------ */
+void orc_scatter_keep(const orc_events *ev, uint64_t n, const float *ell /* n_ell x {cx,cy,cz,1/ax,1/ay,1/az} */,
+                      int n_ell, float h, uint8_t *keep, uint64_t *n_kept) {
+    uint64_t kept = 0;
+    const float mh = -h;
+    for (uint64_t e = 0; e < n; ++e) {
+        float c[3], d[3];
+        keep[e] = 0;
+        if (!tof_centre_f32(ev, e, c, d)) continue;
+        const float xx = d[0] * d[0], yy = d[1] * d[1], zz = d[2] * d[2];
+        const float sxy = xx + yy;
+        const float L = sqrtf(sxy + zz);
+        const float ux = d[0] / L, uy = d[1] / L, uz = d[2] / L;
+        uint8_t hit = 0;
+        for (int k = 0; k < n_ell && !hit; ++k) {
+            const float *q = ell + 6 * k;
+            const float tx = c[0] - q[0], ty = c[1] - q[1], tz = c[2] - q[2];
+            const float rx = tx * q[3], ry = ty * q[4], rz = tz * q[5];
+            const float wx = ux * q[3], wy = uy * q[4], wz = uz * q[5];
+            const float a0 = wx * wx, a1 = wy * wy, a2 = wz * wz;
+            const float a01 = a0 + a1;
+            const float A = a01 + a2;
+            const float b0 = rx * wx, b1 = ry * wy, b2 = rz * wz;
+            const float b01 = b0 + b1;
+            const float B = b01 + b2;
+            const float t0 = B / A;
+            float t = -t0;
+            t = fminf(fmaxf(t, mh), h);
+            const float mx = wx * t, my = wy * t, mz = wz * t;
+            const float px = rx + mx, py = ry + my, pz = rz + mz;
+            const float q0 = px * px, q1 = py * py, q2 = pz * pz;
+            const float q01 = q0 + q1;
+            const float Q = q01 + q2;
+            if (Q <= 1.0f) hit = 1;
+        }
+        keep[e] = hit;
+        kept += hit;
+    }
+    if (n_kept) *n_kept = kept;
 }

@@ -319,6 +319,36 @@ def make_events(cfg: Config, n: Optional[int] = None, start: int = 0, device="cp
     }
 
 
+def event_kinds(cfg: Config, n: Optional[int] = None, start: int = 0, device="cpu") -> torch.Tensor:
+    """uint8[n]: 1 for the scatter-like events of make_events(cfg, n, start), 0 for the true coincidences
+    (the simulation's ground truth; used to check the TOF scatter rejection statistically)."""
+    n = cfg.n_events if n is None else n
+    idx = torch.arange(start, start + n, dtype=torch.int64, device=torch.device(device))
+    return (u01(cfg.seed, idx, 0, _D_TYPE) < cfg.scatter_fraction).to(torch.uint8)
+
+
+def body_outline(cfg: Config) -> List[Tuple[Tuple[float, float, float], Tuple[float, float, float]]]:
+    """The phantom's top-level body parts as (centre, semi-axes) ellipsoids: the stand-in for the NCAT / CT body
+    outline of the paper's TOF scatter rejection.  Only ellipsoid parts qualify."""
+    assert all(s.kind == "ellipsoid" for s in cfg.phantom.parts), "outline needs ellipsoid body parts"
+    return [(s.centre, s.semi) for s in cfg.phantom.parts]
+
+
+MU_WATER_511KEV = 0.0096  # 1/mm, soft tissue at 511 keV
+MU_LUNG_511KEV = 0.0029
+
+
+def rasterize_mu_map(cfg: Config, device="cpu") -> torch.Tensor:
+    """Synthetic attenuation map (1/mm) at voxel centres, float32 [nz, ny, nx]: water inside the body parts, a
+    lower value inside inner shapes of activity < 1 (lungs).  Stand-in for the NCAT mu-map."""
+    act = rasterize_phantom(cfg, device)
+    parts_only = Phantom(cfg.phantom.parts, ())
+    body = rasterize_phantom(Config(cfg.name, cfg.nx, cfg.ny, cfg.nz, cfg.voxel_mm, cfg.radius_mm, cfg.axial_mm,
+                                    parts_only, 0, 0.0, cfg.tof_fwhm_ps, 0, 0, cfg.seed), device) > 0
+    mu = torch.where(body, torch.full_like(act, MU_WATER_511KEV), torch.zeros_like(act))
+    return torch.where(body & (act < 1.0) & (act > 0.0), torch.full_like(act, MU_LUNG_511KEV), mu)
+
+
 def make_events_chunked(cfg: Config, n: Optional[int] = None, start: int = 0, device="cpu",
                         chunk: int = 4_000_000, out_device=None) -> Dict[str, torch.Tensor]:
     """make_events in chunks (bounded scratch memory); identical values to the unchunked call."""
