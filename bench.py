@@ -140,6 +140,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-bin", action="store_true", help="skip locality binning (for comparison)")
+    ap.add_argument("--subbins", type=int, default=0, help="TOFMLEM_OPT_SUBBINS override (0 = library default)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -165,6 +166,8 @@ def main():
     m = args.sens_lors or cfg.sens_lors
     g = pkg.make_grid(cfg.nx, cfg.ny, cfg.nz, cfg.voxel_mm)
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    if args.subbins:
+        ctx.set_option(pkg.OPT_SUBBINS, args.subbins)
     nvox = g.nvox
 
     def timed(fn):

@@ -65,6 +65,8 @@ typedef struct {
     uint64_t n_skipped;    /* n - n_valid of that pass */
     uint64_t visits;       /* voxel visits of the forward walk of that pass */
     double sum_image_sens; /* sum_j image_j * sens_j after the last tofmlem_iterate (= n_valid, P7) */
+    uint64_t reductions;   /* reduction instructions (scalar or 16-byte) the scatter walk of that pass sent to the L2
+                              atomic units: the unit of the l2_atomic roofline */
 } tofmlem_stats;
 
 /* Option keys for tofmlem_set_option. */
@@ -77,9 +79,15 @@ enum {
     TOFMLEM_OPT_SHELL_MM = 6,       /* extra shell added to the region margin, default 6 mm */
     TOFMLEM_OPT_EM_VARIANT = 8,     /* fused EM pass scheduling (performance only): 0 = persistent kernel with one work
                                        queue per SM (default), 1 = one CTA per 256-event chunk in grid order */
-    TOFMLEM_OPT_CTA_INTERLEAVE = 7  /* scatter kernels: number of list segments advanced in parallel (default 64;
+    TOFMLEM_OPT_CTA_INTERLEAVE = 7, /* scatter kernels: number of list segments advanced in parallel (default 64;
                                        1 = natural order).  Performance only, results are the same up to the
                                        order of the float32 reductions. */
+    TOFMLEM_OPT_MEDIAN = 10,        /* 1: tofmlem_iterate applies the 3x3x3 median filter to the image estimate after
+                                       every update (R23); default 0 */
+    TOFMLEM_OPT_SUBBINS = 9         /* tofmlem_bin_events: order the events INSIDE each locality bin by predicted
+                                       voxel-visit count, in `value` sub-bins (1..64, default 16; 1 = off), so that
+                                       the events of a warp walk windows of nearly equal length.  Keys, bin offsets
+                                       and bin membership do not change (the order inside a bin is unspecified). */
 };
 
 /* Create a context.  tof_fwhm_ps <= 0 makes a non-TOF context (full-chord traversal).
@@ -160,6 +168,48 @@ int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zb
  * d_image_out (nvox floats, overwritten) as the paper does.  SYNCHRONISES. */
 int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
                                 const float *h_zbounds, float *d_image_out, const float *d_sens, int iters);
+
+/* ---- Widened rows: the steps the paper runs around the hot path -------------------------
+ *
+ * NEXT-1, the paper's own TOF kernel (Fig. 3): tofmlem_set_option(TOFMLEM_OPT_PROJECTOR, 1) switches
+ * forward / backproject / em_correction / iterate of a TOF context to K equally spaced samples inside the truncated
+ * Gaussian (offset_k = -T sigma + k 2 T sigma/(K-1), Gaussian weights normalised to sum to one, K =
+ * TOFMLEM_OPT_SAMPLES_K, default 32), centred on the measured time difference; each sample is filled into the voxel
+ * that contains it; samples beyond the LOR's end points or outside the grid are dropped.  The voxel of a sample is
+ * decided in fp64.  `visits` then counts the samples kept. */
+
+/* NEXT-2 ("we introduced a median filter between MLEM iterations"; size unstated -> R23): 3x3x3 median
+ * filter, edges replicated: d_out[j] = the 14th smallest of the 27 values around voxel j.  d_in, d_out: nvox floats,
+ * must not alias.  Bit-exact (the result is one of the inputs).  TOFMLEM_OPT_MEDIAN = 1 makes tofmlem_iterate
+ * apply it after every update. */
+int tofmlem_median3(tofmlem_ctx *ctx, const float *d_in, float *d_out);
+
+/* NEXT-3 ("Attenuation correction was implemented in the forward projection by a weight inversely
+ * proportional to the probability of the event being attenuated" -> R19): d_weight[e] = exp(+ sum_j l_ej d_mu[j]),
+ * the reciprocal of the probability that both photons of LOR e survive; l_ej = non-TOF Siddon chords over the whole
+ * grid, d_mu = attenuation map (1/mm, nvox floats on the context's grid).  LORs that miss the grid get 1. */
+int tofmlem_attenuation_weights(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t n, const float *d_mu,
+                                float *d_weight);
+/* EM pass / iterations with a per-event weight: d_corr[j] += d_weight[e] * a_ej / fwd_e (d_weight = NULL => 1, i.e.
+ * tofmlem_em_correction / tofmlem_iterate).  d_weight: n floats in the SAME order as the events (after
+ * tofmlem_bin_events, permute it with tofmlem_gather_f32). */
+int tofmlem_em_correction_weighted(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_weight,
+                                   const float *d_image, float *d_corr);
+int tofmlem_iterate_weighted(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_weight,
+                             float *d_image, const float *d_sens, int iters);
+/* d_out[i] = d_in[d_perm[i]], n floats; d_in and d_out must not alias. */
+int tofmlem_gather_f32(tofmlem_ctx *ctx, const float *d_in, const uint32_t *d_perm, uint64_t n, float *d_out);
+
+/* NEXT-4, TOF-based scatter rejection (PAPER.md:63 Fig. 2, :69-71 -> R24): d_keep[e] = 1 iff the segment
+ * {c + u t : |t| <= half_width_mm} meets the body outline, else 0; c = TOF-estimated annihilation point, u = LOR
+ * direction, half_width_mm <= 0 selects 1.959964 sigma ("limits of rejection ... at a 95% confidence level").
+ * The outline is a union of n_ellipsoids <= 64 ellipsoids, h_ellipsoids = HOST array of 6 floats each
+ * (centre x, y, z, then the RECIPROCAL semi-axes 1/ax, 1/ay, 1/az).  float32 specification F2: the flags
+ * are bit-exact.  Invalid events are not kept.  d_perm (may be NULL) receives the indices of the kept events in its
+ * first *h_n_kept entries (order unspecified), ready for tofmlem_gather_events.  SYNCHRONISES (h_n_kept is HOST). */
+int tofmlem_scatter_reject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *h_ellipsoids,
+                           int n_ellipsoids, float half_width_mm, uint8_t *d_keep, uint32_t *d_perm,
+                           uint64_t *h_n_kept);
 
 /* Roofline probe (measurement aid; north_star asks for the MEASURED atomic / L2 roofline): issues n_ops float32
  * operations against d_buf[0..n_elems) and returns the elapsed milliseconds in *h_ms (second of two passes, so

@@ -27,8 +27,17 @@ struct tofmlem_ctx {
     const float *d_max_ext = nullptr;  // region sub-contexts use the parent's global max
     DeviceStats *d_stats = nullptr;
     unsigned *d_queues = nullptr;  // work counters of the persistent EM kernel
-    uint32_t *d_hist = nullptr, *d_cursor = nullptr;
+    uint32_t *d_hist = nullptr, *d_cursor = nullptr, *d_scan_tmp = nullptr;
     size_t hist_cap = 0;
+    uint8_t *d_sub = nullptr;  // sub-bin of every event of the last tofmlem_bin_events
+    size_t sub_cap = 0;
+    int subbins = 16;
+    int median = 0;                    // 3x3x3 median filter after every update of tofmlem_iterate (NEXT-2)
+    float *d_tmp_image = nullptr;      // median filter output
+    SampleLutEntry *d_lut = nullptr;   // K-sample TOF kernel (NEXT-1)
+    int lut_k = 0;
+    double lut_sigma = 0.0, lut_trunc = 0.0;
+    std::vector<SampleLutEntry> h_lut;
     unsigned long long *d_rcounts = nullptr;  // 2*(kMaxRegions+1)
     // host-buffer path
     float *d_hev = nullptr;
@@ -148,8 +157,60 @@ void default_zbounds(const tofmlem_ctx *c, int R, float *zb) {
     }
 }
 
-int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, float *d_image, const float *d_sens, int iters,
-                   bool compute_max) {
+// Look-up table of the paper's K-sample TOF kernel (Fig. 3): offset_k = -T sigma + k 2 T sigma/(K-1),
+// weight_k = exp(-offset_k^2 / 2 sigma^2) / sum_m exp(-offset_m^2 / 2 sigma^2); K = 1: one sample at the centre.
+int ensure_lut(tofmlem_ctx *ctx) {
+    const int K = ctx->samples_k;
+    if (ctx->d_lut && ctx->lut_k == K && ctx->lut_sigma == ctx->sigma && ctx->lut_trunc == ctx->trunc_sigmas)
+        return TOFMLEM_OK;
+    CU(cudaStreamSynchronize(ctx->stream));  // a previous launch may still read the old table
+    cudaFree(ctx->d_lut);
+    ctx->d_lut = nullptr;
+    std::vector<double> w(K);
+    ctx->h_lut.assign(K, SampleLutEntry{});
+    const double hw = ctx->trunc_sigmas * ctx->sigma;
+    double sum = 0.0;
+    for (int k = 0; k < K; ++k) {
+        const double off = K > 1 ? -hw + (double)k * (2.0 * hw) / (double)(K - 1) : 0.0;
+        const double r = off / ctx->sigma;
+        w[k] = exp(-0.5 * r * r);
+        sum += w[k];
+        ctx->h_lut[k].offset = off;
+    }
+    for (int k = 0; k < K; ++k) ctx->h_lut[k].weight = (float)(w[k] / sum);
+    CU(cudaMalloc(&ctx->d_lut, K * sizeof(SampleLutEntry)));
+    CU(cudaMemcpyAsync(ctx->d_lut, ctx->h_lut.data(), K * sizeof(SampleLutEntry), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->lut_k = K;
+    ctx->lut_sigma = ctx->sigma;
+    ctx->lut_trunc = ctx->trunc_sigmas;
+    return TOFMLEM_OK;
+}
+
+// One fused EM pass with the context's projector (0 = Siddon x Gaussian, 1 = K-sample kernel).
+int em_pass(tofmlem_ctx *ctx, const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw,
+            const float *d_image, float *d_corr, bool vec, cudaStream_t s) {
+    if (n == 0) return TOFMLEM_OK;
+    if (ctx->projector == 1) {
+        int rc = ensure_lut(ctx);
+        if (rc) return rc;
+        launch_sampled_em(p, ctx->d_lut, ctx->samples_k, ev, n, evw, d_image, d_corr, ctx->d_stats, s);
+    } else {
+        launch_em_correction(p, ctx->tof, ev, n, evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, s);
+    }
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int median_in_place(tofmlem_ctx *ctx, float *d_image, cudaStream_t s) {
+    if (!ctx->d_tmp_image) CU(cudaMalloc(&ctx->d_tmp_image, ctx->nvox * sizeof(float)));
+    launch_median3(d_image, ctx->d_tmp_image, ctx->grid.nx, ctx->grid.ny, ctx->grid.nz, s);
+    CHECK_LAUNCH(1);
+    CU(cudaMemcpyAsync(d_image, ctx->d_tmp_image, ctx->nvox * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    return TOFMLEM_OK;
+}
+
+int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, const float *evw, float *d_image,
+                   const float *d_sens, int iters, bool compute_max) {
     int rc = ensure_corr(ctx);
     if (rc) return rc;
     const ProjParams p = make_params(ctx, ctx->tof);
@@ -160,11 +221,15 @@ int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, float *d_i
     }
     CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
     for (int it = 0; it < iters; ++it) {
-        CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), ctx->stream));
-        launch_em_correction(p, ctx->tof, ev, n, d_image, ctx->d_corr, true, ctx->d_stats, ctx->d_queues, ctx->stream);
-        CHECK_LAUNCH(n ? 1 : 0);
+        CU(cudaMemsetAsync(ctx->d_stats, 0, 3 * sizeof(unsigned long long), ctx->stream));
+        rc = em_pass(ctx, p, ev, n, evw, d_image, ctx->d_corr, true, ctx->stream);
+        if (rc) return rc;
         launch_update(d_image, ctx->d_corr, d_sens, dmax, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
         CHECK_LAUNCH(1);
+        if (ctx->median) {  // the filter is applied to the image estimate after each iteration (R23)
+            rc = median_in_place(ctx, d_image, ctx->stream);
+            if (rc) return rc;
+        }
     }
     launch_dot_f64(d_image, d_sens, ctx->nvox, &ctx->d_stats->sum_image_sens, ctx->stream);
     CHECK_LAUNCH(1);
@@ -230,6 +295,10 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_queues);
     cudaFree(ctx->d_hist);
     cudaFree(ctx->d_cursor);
+    cudaFree(ctx->d_scan_tmp);
+    cudaFree(ctx->d_sub);
+    cudaFree(ctx->d_tmp_image);
+    cudaFree(ctx->d_lut);
     cudaFree(ctx->d_rcounts);
     cudaFree(ctx->d_hev);
     cudaFree(ctx->d_himg);
@@ -254,11 +323,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             ctx->tile_log2 = (int)value;
             return TOFMLEM_OK;
         case TOFMLEM_OPT_PROJECTOR:
-            if (value == 0.0) {
-                ctx->projector = 0;
-                return TOFMLEM_OK;
-            }
-            return fail(ctx, TOFMLEM_EUNSUPPORTED, "sampled projector not built yet");
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "projector is 0 (Siddon) or 1 (K samples)");
+            if (value == 1.0 && !ctx->tof) return fail(ctx, TOFMLEM_EUNSUPPORTED, "the K-sample kernel needs a TOF context");
+            ctx->projector = (int)value;
+            return TOFMLEM_OK;
         case TOFMLEM_OPT_SAMPLES_K:
             if (value < 1 || value > 1024 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "K in 1..1024");
             ctx->samples_k = (int)value;
@@ -274,6 +342,14 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
         case TOFMLEM_OPT_EM_VARIANT:
             if (value < 0 || value > 1 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "em_variant in 0..1");
             ctx->em_variant = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_MEDIAN:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "median is 0 or 1");
+            ctx->median = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_SUBBINS:
+            if (value < 1 || value > 64 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "subbins in 1..64");
+            ctx->subbins = (int)value;
             return TOFMLEM_OK;
         default:
             return fail(ctx, TOFMLEM_EINVAL, "unknown option key");
@@ -300,7 +376,14 @@ int tofmlem_forward(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, cons
     if (!ctx) return TOFMLEM_EINVAL;
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || !d_image || !d_fwd || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "forward: bad argument");
-    launch_forward(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_fwd, ctx->stream);
+    if (ctx->projector == 1) {
+        int rc = ensure_lut(ctx);
+        if (rc) return rc;
+        launch_sampled_forward(make_params(ctx, true), ctx->d_lut, ctx->samples_k, ev_ptrs(ev), n, d_image, d_fwd,
+                               ctx->stream);
+    } else {
+        launch_forward(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_fwd, ctx->stream);
+    }
     CHECK_LAUNCH(1);
     return TOFMLEM_OK;
 }
@@ -309,8 +392,15 @@ int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, 
     if (!ctx) return TOFMLEM_EINVAL;
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || !d_out || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "backproject: bad argument");
-    launch_backproject(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_values, d_out, vec_ok(ctx, d_out),
-                       ctx->stream);
+    if (ctx->projector == 1) {
+        int rc = ensure_lut(ctx);
+        if (rc) return rc;
+        launch_sampled_backproject(make_params(ctx, true), ctx->d_lut, ctx->samples_k, ev_ptrs(ev), n, d_values, d_out,
+                                   ctx->stream);
+    } else {
+        launch_backproject(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_values, d_out, vec_ok(ctx, d_out),
+                           ctx->stream);
+    }
     CHECK_LAUNCH(1);
     return TOFMLEM_OK;
 }
@@ -322,15 +412,20 @@ int tofmlem_reset_stats(tofmlem_ctx *ctx) {
     return TOFMLEM_OK;
 }
 
-int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr) {
+int tofmlem_em_correction_weighted(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_weight,
+                                   const float *d_image, float *d_corr) {
     if (!ctx) return TOFMLEM_EINVAL;
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || !d_image || !d_corr || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "em_correction: bad argument");
-    launch_em_correction(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_corr, vec_ok(ctx, d_corr),
-                         ctx->d_stats, ctx->d_queues, ctx->stream);
-    CHECK_LAUNCH(1);
+    int rc = em_pass(ctx, make_params(ctx, ctx->tof), ev_ptrs(ev), n, d_weight, d_image, d_corr, vec_ok(ctx, d_corr),
+                     ctx->stream);
+    if (rc) return rc;
     ctx->last_n += n;
     return TOFMLEM_OK;
+}
+
+int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr) {
+    return tofmlem_em_correction_weighted(ctx, ev, n, nullptr, d_image, d_corr);
 }
 
 int tofmlem_update(tofmlem_ctx *ctx, float *d_image, float *d_corr, const float *d_sens) {
@@ -343,13 +438,75 @@ int tofmlem_update(tofmlem_ctx *ctx, float *d_image, float *d_corr, const float 
     return TOFMLEM_OK;
 }
 
-int tofmlem_iterate(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, float *d_image, const float *d_sens,
-                    int iters) {
+int tofmlem_iterate_weighted(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_weight,
+                             float *d_image, const float *d_sens, int iters) {
     if (!ctx) return TOFMLEM_EINVAL;
     if ((n && !ev_ok(ev, ctx->tof)) || !d_image || !d_sens || iters < 0 || n > 0xFFFFFFFFull || d_image == d_sens)
         return fail(ctx, TOFMLEM_EINVAL, "iterate: bad argument");
     EventPtrs p = n ? ev_ptrs(ev) : EventPtrs{};
-    return iterate_device(ctx, p, n, d_image, d_sens, iters, true);
+    return iterate_device(ctx, p, n, d_weight, d_image, d_sens, iters, true);
+}
+
+int tofmlem_iterate(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, float *d_image, const float *d_sens,
+                    int iters) {
+    return tofmlem_iterate_weighted(ctx, ev, n, nullptr, d_image, d_sens, iters);
+}
+
+int tofmlem_median3(tofmlem_ctx *ctx, const float *d_in, float *d_out) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (!d_in || !d_out || d_in == d_out) return fail(ctx, TOFMLEM_EINVAL, "median3: NULL or aliased argument");
+    launch_median3(d_in, d_out, ctx->grid.nx, ctx->grid.ny, ctx->grid.nz, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_attenuation_weights(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t n, const float *d_mu,
+                                float *d_weight) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(lors, false) || !d_mu || !d_weight || n > 0xFFFFFFFFull)
+        return fail(ctx, TOFMLEM_EINVAL, "attenuation_weights: bad argument");
+    EventPtrs ev = ev_ptrs(lors);
+    ev.dt = nullptr;
+    launch_forward(make_params(ctx, false), false, ev, n, d_mu, d_weight, ctx->stream);  // line integral of mu
+    CHECK_LAUNCH(1);
+    launch_exp(d_weight, n, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_gather_f32(tofmlem_ctx *ctx, const float *d_in, const uint32_t *d_perm, uint64_t n, float *d_out) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if (n == 0) return TOFMLEM_OK;
+    if (!d_in || !d_perm || !d_out || d_in == d_out) return fail(ctx, TOFMLEM_EINVAL, "gather_f32: bad argument");
+    launch_gather(d_in, d_perm, n, d_out, ctx->stream);
+    CHECK_LAUNCH(1);
+    return TOFMLEM_OK;
+}
+
+int tofmlem_scatter_reject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *h_ellipsoids,
+                           int n_ellipsoids, float half_width_mm, uint8_t *d_keep, uint32_t *d_perm,
+                           uint64_t *h_n_kept) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    if ((n && !ev_ok(ev, true)) || !h_ellipsoids || n_ellipsoids < 1 || n_ellipsoids > kMaxEllipsoids ||
+        (n && !d_keep) || !h_n_kept || n > 0xFFFFFFFFull || isnan(half_width_mm))
+        return fail(ctx, TOFMLEM_EINVAL, "scatter_reject: bad argument");
+    EllipsoidSet es;
+    es.n = n_ellipsoids;
+    for (int i = 0; i < 6 * n_ellipsoids; ++i) es.v[i] = h_ellipsoids[i];
+    // default half width: the two-sided 95 % point of the TOF Gaussian ("95% confidence level")
+    const float h = half_width_mm > 0.0f ? half_width_mm : (float)(1.959964 * ctx->sigma);
+    unsigned long long *counter = ctx->d_rcounts;
+    CU(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), ctx->stream));
+    if (n) {
+        launch_scatter_keep(ev_ptrs(ev), n, es, h, d_keep, d_perm, counter, ctx->stream);
+        CHECK_LAUNCH(1);
+    }
+    unsigned long long kept = 0;
+    CU(cudaMemcpyAsync(&kept, counter, sizeof kept, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    *h_n_kept = kept;
+    return TOFMLEM_OK;
 }
 
 int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t n, float *h_image,
@@ -401,17 +558,19 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
                     CU(cudaMemcpyAsync(d + f * stride + off, hsrc[f] + off, m * sizeof(float), cudaMemcpyHostToDevice, cs));
             CU(cudaEventRecord(ctx->chunk_done[slot], cs));
             CU(cudaStreamWaitEvent(s, ctx->chunk_done[slot], 0));
-            launch_em_correction(p, ctx->tof, ev_ptrs(&dev, off), m, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, ctx->d_queues, s);
-            CHECK_LAUNCH(1);
+            rc = em_pass(ctx, p, ev_ptrs(&dev, off), m, nullptr, ctx->d_himg, ctx->d_corr, true, s);
+            if (rc) return rc;
         }
         launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
         CHECK_LAUNCH(1);
+        if (ctx->median && (rc = median_in_place(ctx, ctx->d_himg, s))) return rc;
         for (int it = 1; it < iters; ++it) {
-            CU(cudaMemsetAsync(ctx->d_stats, 0, 2 * sizeof(unsigned long long), s));
-            launch_em_correction(p, ctx->tof, ev_ptrs(&dev), n, ctx->d_himg, ctx->d_corr, true, ctx->d_stats, ctx->d_queues, s);
-            CHECK_LAUNCH(1);
+            CU(cudaMemsetAsync(ctx->d_stats, 0, 3 * sizeof(unsigned long long), s));
+            rc = em_pass(ctx, p, ev_ptrs(&dev), n, nullptr, ctx->d_himg, ctx->d_corr, true, s);
+            if (rc) return rc;
             launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
             CHECK_LAUNCH(1);
+            if (ctx->median && (rc = median_in_place(ctx, ctx->d_himg, s))) return rc;
         }
     } else if (iters > 0) {
         for (int it = 0; it < iters; ++it) {
@@ -435,29 +594,56 @@ int tofmlem_bin_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, u
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, false) || !d_key || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "bin_events: bad argument");
     const uint32_t nb = num_bins(ctx);
-    if (ctx->hist_cap < (size_t)nb + 1) {
+    const bool sort = d_perm != nullptr;
+    // sub-bins only matter for the permutation; the fine histogram must still fit 32-bit indices
+    uint32_t S = sort ? (uint32_t)ctx->subbins : 1u;
+    while (S > 1 && (uint64_t)nb * S + 1 > 0x7FFFFFFFull) S >>= 1;
+    const size_t nfine = (size_t)nb * S + 1;
+    if (ctx->hist_cap < nfine) {
         cudaFree(ctx->d_hist);
         cudaFree(ctx->d_cursor);
-        ctx->d_hist = ctx->d_cursor = nullptr;
+        cudaFree(ctx->d_scan_tmp);
+        ctx->d_hist = ctx->d_cursor = ctx->d_scan_tmp = nullptr;
         ctx->hist_cap = 0;
-        CU(cudaMalloc(&ctx->d_hist, ((size_t)nb + 1) * sizeof(uint32_t)));
-        CU(cudaMalloc(&ctx->d_cursor, ((size_t)nb + 1) * sizeof(uint32_t)));
-        ctx->hist_cap = (size_t)nb + 1;
+        CU(cudaMalloc(&ctx->d_hist, nfine * sizeof(uint32_t)));
+        CU(cudaMalloc(&ctx->d_cursor, nfine * sizeof(uint32_t)));
+        CU(cudaMalloc(&ctx->d_scan_tmp, (size_t)scan_tmp_elems((uint32_t)nfine) * sizeof(uint32_t)));
+        ctx->hist_cap = nfine;
     }
-    const bool sort = d_perm != nullptr;
-    CU(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)nb + 1) * sizeof(uint32_t), ctx->stream));
-    launch_bin_keys(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, d_key, (sort || d_bin_offsets) ? ctx->d_hist : nullptr,
-                    nb, ctx->stream);
+    if (S > 1 && ctx->sub_cap < n) {
+        cudaFree(ctx->d_sub);
+        ctx->d_sub = nullptr;
+        ctx->sub_cap = 0;
+        CU(cudaMalloc(&ctx->d_sub, n));
+        ctx->sub_cap = n;
+    }
+    SubBin sb;
+    sb.S = S;
+    sb.half_window = ctx->tof ? (float)(ctx->trunc_sigmas * ctx->sigma) : 0.0f;
+    {
+        // largest visit count of a window: its length times the l1 norm of u / v, plus the first voxel
+        const tofmlem_grid &g = ctx->grid;
+        const double diag = sqrt(pow(g.nx * (double)g.vx, 2) + pow(g.ny * (double)g.vy, 2) + pow(g.nz * (double)g.vz, 2));
+        const double len = ctx->tof ? fmin(2.0 * sb.half_window, diag) : diag;
+        const double vmax = fmin(len * sqrt(1.0 / (g.vx * g.vx) + 1.0 / (g.vy * g.vy) + 1.0 / (g.vz * g.vz)) + 3.0,
+                                 (double)g.nx + g.ny + g.nz);
+        sb.quantum = S > 2 ? (uint32_t)fmax(1.0, ceil(vmax / (double)(S - 2))) : 1u << 30;
+    }
+    uint8_t *d_sub = S > 1 ? ctx->d_sub : nullptr;
+    CU(cudaMemsetAsync(ctx->d_hist, 0, nfine * sizeof(uint32_t), ctx->stream));
+    launch_bin_keys(grid_f32(ctx), ctx->tile_log2, sb, ev_ptrs(ev), n, d_key, d_sub,
+                    (sort || d_bin_offsets) ? ctx->d_hist : nullptr, nb, ctx->stream);
     CHECK_LAUNCH(1);
     if (sort || d_bin_offsets) {
-        launch_exclusive_scan_u32(ctx->d_hist, ctx->d_cursor, nullptr, nb + 1, ctx->stream);
-        CHECK_LAUNCH(1);
-        if (d_bin_offsets)
-            CU(cudaMemcpyAsync(d_bin_offsets, ctx->d_cursor, ((size_t)nb + 1) * sizeof(uint32_t),
-                               cudaMemcpyDeviceToDevice, ctx->stream));
+        const int k = launch_exclusive_scan_u32(ctx->d_hist, ctx->d_cursor, ctx->d_scan_tmp, (uint32_t)nfine, ctx->stream);
+        CHECK_LAUNCH(k);
+        if (d_bin_offsets) {
+            launch_strided_copy(ctx->d_cursor, S, nb + 1, d_bin_offsets, ctx->stream);
+            CHECK_LAUNCH(1);
+        }
     }
     if (sort) {
-        launch_scatter_perm(d_key, n, nb, ctx->d_cursor, d_perm, ctx->stream);
+        launch_scatter_perm(d_key, d_sub, S, n, nb, ctx->d_cursor, d_perm, ctx->stream);
         CHECK_LAUNCH(1);
     }
     return TOFMLEM_OK;
@@ -630,6 +816,9 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         sc->sigma = ctx->sigma;
         sc->trunc_sigmas = ctx->trunc_sigmas;
         sc->sens_floor_rel = ctx->sens_floor_rel;
+        sc->projector = ctx->projector;
+        sc->samples_k = ctx->samples_k;
+        sc->median = ctx->median;
         sc->d_max_ext = ctx->d_max;
         const uint64_t nv = sc->nvox;
         RCU(cudaMalloc(&images[r], nv * sizeof(float)));
@@ -639,7 +828,7 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         sc->launches += 1;
         tofmlem_events sub_ev{sorted.x1 + off, sorted.y1 + off, sorted.z1 + off, sorted.x2 + off, sorted.y2 + off,
                               sorted.z2 + off, sorted.dt ? sorted.dt + off : nullptr};
-        rc = iterate_device(sc, counts[r] ? ev_ptrs(&sub_ev) : EventPtrs{}, counts[r], images[r], sens_r, iters, false);
+        rc = iterate_device(sc, counts[r] ? ev_ptrs(&sub_ev) : EventPtrs{}, counts[r], nullptr, images[r], sens_r, iters, false);
         if (rc != TOFMLEM_OK) {
             ctx->err = sc->err;
             cudaDeviceSynchronize();
@@ -670,6 +859,7 @@ int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out) {
     h_out->n_valid = h.n_valid;
     h_out->n_skipped = ctx->last_n >= h.n_valid ? ctx->last_n - h.n_valid : 0;
     h_out->visits = h.visits;
+    h_out->reductions = h.reds;
     h_out->sum_image_sens = h.sum_image_sens;
     return TOFMLEM_OK;
 }

@@ -48,8 +48,51 @@ __device__ __forceinline__ int centre_voxel(float c, float o, float v, int n) {
     return (int)f;
 }
 
-__global__ void __launch_bounds__(kBlock) bin_keys_kernel(GridF32 g, int tile_log2, EventPtrs ev, uint64_t n,
-                                                          uint32_t *__restrict__ key, uint32_t *__restrict__ hist,
+// Predicted number of voxel visits of the event's clipped TOF window (float32, a sorting heuristic only: it decides
+// the ORDER of events inside a locality bin, which the specification leaves open (R14), never a reported value).
+__device__ __forceinline__ int predicted_visits(const GridF32 &g, const SubBin &sb, const EventPtrs &ev, uint64_t e,
+                                                const float d[3]) {
+    const float p1[3] = {__ldg(ev.x1 + e), __ldg(ev.y1 + e), __ldg(ev.z1 + e)};
+    const float dt = ev.dt ? __ldg(ev.dt + e) : 0.0f;
+    const float L = sqrtf(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    const float iL = 1.0f / L;
+    const float o[3] = {g.ox, g.oy, g.oz}, v[3] = {g.vx, g.vy, g.vz};
+    const int n[3] = {g.nx, g.ny, g.nz};
+    float u[3], s_lo = 0.0f, s_hi = L;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        u[a] = d[a] * iL;
+        const float lo = o[a], hi = o[a] + (float)n[a] * v[a];
+        if (u[a] == 0.0f) {
+            if (p1[a] < lo || p1[a] >= hi) return 0;
+        } else {
+            const float iu = 1.0f / u[a];
+            const float ta = (lo - p1[a]) * iu, tb = (hi - p1[a]) * iu;
+            s_lo = fmaxf(s_lo, fminf(ta, tb));
+            s_hi = fminf(s_hi, fmaxf(ta, tb));
+        }
+    }
+    if (sb.half_window > 0.0f) {
+        const float s_c = 0.5f * L + kHalfC * dt;
+        s_lo = fmaxf(s_lo, s_c - sb.half_window);
+        s_hi = fminf(s_hi, s_c + sb.half_window);
+    }
+    if (!(s_hi > s_lo)) return 0;
+    int visits = 1;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float qa = floorf((p1[a] + u[a] * s_lo - o[a]) / v[a]), qb = floorf((p1[a] + u[a] * s_hi - o[a]) / v[a]);
+        visits += (int)fabsf(qb - qa);
+    }
+    return visits;
+}
+
+// key (F1) of every event; with `sub` also the sub-bin (events of one locality bin ordered by predicted visit count,
+// so that the 32 events of a warp run loops of nearly equal length) and the histogram of the fine key
+// key * sb.S + sub (invalid events: the last fine bin).
+__global__ void __launch_bounds__(kBlock) bin_keys_kernel(GridF32 g, int tile_log2, SubBin sb, EventPtrs ev,
+                                                          uint64_t n, uint32_t *__restrict__ key,
+                                                          uint8_t *__restrict__ sub, uint32_t *__restrict__ hist,
                                                           uint32_t nbins) {
     const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
     if (e >= n) return;
@@ -58,6 +101,7 @@ __global__ void __launch_bounds__(kBlock) bin_keys_kernel(GridF32 g, int tile_lo
                    Tz = (uint32_t)((g.nz + t - 1) >> tile_log2);
     float c[3], d[3];
     uint32_t k = 0xFFFFFFFFu;
+    uint32_t sbin = 0;
     if (tof_centre(ev, e, c, d)) {
         const int ix = centre_voxel(c[0], g.ox, g.vx, g.nx);
         const int iy = centre_voxel(c[1], g.oy, g.vy, g.ny);
@@ -75,9 +119,14 @@ __global__ void __launch_bounds__(kBlock) bin_keys_kernel(GridF32 g, int tile_lo
         const float db = neg ? -db0 : db0, dc = neg ? -dc0 : dc0;
         const uint32_t dirclass = 4u * (uint32_t)a + 2u * (db < 0.0f ? 1u : 0u) + (dc < 0.0f ? 1u : 0u);
         k = dirclass * (Tx * Ty * Tz) + tile;
+        if (sub) {
+            const int vis = predicted_visits(g, sb, ev, e, d);
+            sbin = vis <= 0 ? 0u : min(sb.S - 1u, 1u + (uint32_t)vis / sb.quantum);
+        }
     }
     key[e] = k;
-    if (hist) atomicAdd(hist + (k < nbins ? k : nbins), 1u);
+    if (sub) sub[e] = (uint8_t)sbin;
+    if (hist) atomicAdd(hist + (k < nbins ? k * sb.S + sbin : nbins * sb.S), 1u);
 }
 
 // single-block exclusive scan (n <= a few 10^5 bins): per-thread segments + shared-memory scan of the sums
@@ -106,14 +155,72 @@ __global__ void __launch_bounds__(1024) exclusive_scan_kernel(const uint32_t *__
     }
 }
 
-__global__ void __launch_bounds__(kBlock) scatter_perm_kernel(const uint32_t *__restrict__ key, uint64_t n,
+// Three-kernel exclusive scan for long histograms: chunk sums -> single-block scan of the sums -> per-chunk scan.
+constexpr int kScanItems = 8, kScanChunk = kBlock * kScanItems;
+
+__global__ void __launch_bounds__(kBlock) scan_chunk_sums_kernel(const uint32_t *__restrict__ in, uint32_t n,
+                                                                 uint32_t *__restrict__ sums) {
+    __shared__ uint32_t wsum[kBlock / 32];
+    const uint32_t base = blockIdx.x * kScanChunk;
+    uint32_t s = 0;
+    for (int i = threadIdx.x; i < kScanChunk; i += kBlock)
+        if (base + i < n) s += in[base + i];
+    s = __reduce_add_sync(0xffffffffu, s);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+        for (int w = 0; w < kBlock / 32; ++w) t += wsum[w];
+        sums[blockIdx.x] = t;
+    }
+}
+
+__global__ void __launch_bounds__(kBlock) scan_chunks_kernel(const uint32_t *__restrict__ in, uint32_t n,
+                                                             const uint32_t *__restrict__ chunk_base,
+                                                             uint32_t *__restrict__ out) {
+    __shared__ uint32_t wsum[kBlock / 32];
+    const uint32_t lo = blockIdx.x * kScanChunk + threadIdx.x * kScanItems;
+    uint32_t v[kScanItems], s = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        v[i] = lo + i < n ? in[lo + i] : 0u;
+        s += v[i];
+    }
+    // exclusive prefix of the per-thread sums inside the block
+    uint32_t inc = s;
+    const unsigned lane = threadIdx.x & 31u;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= (unsigned)off) inc += t;
+    }
+    if (lane == 31) wsum[threadIdx.x >> 5] = inc;
+    __syncthreads();
+    uint32_t run = chunk_base[blockIdx.x] + inc - s;
+    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) run += wsum[w];
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (lo + i < n) out[lo + i] = run;
+        run += v[i];
+    }
+}
+
+__global__ void __launch_bounds__(kBlock) scatter_perm_kernel(const uint32_t *__restrict__ key,
+                                                              const uint8_t *__restrict__ sub, uint32_t S, uint64_t n,
                                                               uint32_t nbins, uint32_t *__restrict__ cursor,
                                                               uint32_t *__restrict__ perm) {
     const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
     if (e >= n) return;
     const uint32_t k = key[e];
-    const uint32_t pos = atomicAdd(cursor + (k < nbins ? k : nbins), 1u);
+    const uint32_t pos = atomicAdd(cursor + (k < nbins ? k * S + (sub ? sub[e] : 0u) : nbins * S), 1u);
     perm[pos] = (uint32_t)e;
+}
+
+// offsets of the (coarse) locality bins out of the fine-bin offsets: out[k] = fine[k * S], k = 0..nbins
+__global__ void __launch_bounds__(kBlock) strided_copy_kernel(const uint32_t *__restrict__ fine, uint32_t S,
+                                                              uint32_t count, uint32_t *__restrict__ out) {
+    const uint32_t k = blockIdx.x * kBlock + threadIdx.x;
+    if (k < count) out[k] = fine[(size_t)k * S];
 }
 
 __global__ void __launch_bounds__(kBlock) gather_kernel(const float *__restrict__ in, const uint32_t *__restrict__ perm,
@@ -168,20 +275,78 @@ __global__ void __launch_bounds__(kBlock) region_scatter_kernel(const int32_t *_
     if (e < n) perm[base[r] + rank] = (uint32_t)e;
 }
 
+// NEXT-4: TOF-based scatter rejection (PAPER.md:63 Fig. 2, :69-71; reading R24, float32 specification F2 in
+// DESIGN.md): keep the event iff the segment {c + u t : |t| <= h} (c = TOF-estimated annihilation point, u = LOR
+// direction, h = 1.96 sigma: the 95 % confidence interval) meets the body outline, a union of ellipsoids.  Every
+// float operation is one IEEE binary32 RN operation in the order of F2, so the flags are bit-exact.
+// Kept events' indices are appended to `perm` (order unspecified) through one atomic per warp.
+__global__ void __launch_bounds__(kBlock) scatter_keep_kernel(EventPtrs ev, uint64_t n, EllipsoidSet es, float h,
+                                                              uint8_t *__restrict__ keep, uint32_t *__restrict__ perm,
+                                                              unsigned long long *__restrict__ counter) {
+    const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    bool hit = false;
+    float c[3], d[3];
+    if (e < n && tof_centre(ev, e, c, d)) {
+        const float xx = __fmul_rn(d[0], d[0]), yy = __fmul_rn(d[1], d[1]), zz = __fmul_rn(d[2], d[2]);
+        const float L = __fsqrt_rn(__fadd_rn(__fadd_rn(xx, yy), zz));
+        const float ux = __fdiv_rn(d[0], L), uy = __fdiv_rn(d[1], L), uz = __fdiv_rn(d[2], L);
+        for (int k = 0; k < es.n && !hit; ++k) {
+            const float *q = es.v + 6 * k;
+            const float rx = __fmul_rn(__fsub_rn(c[0], q[0]), q[3]);
+            const float ry = __fmul_rn(__fsub_rn(c[1], q[1]), q[4]);
+            const float rz = __fmul_rn(__fsub_rn(c[2], q[2]), q[5]);
+            const float wx = __fmul_rn(ux, q[3]), wy = __fmul_rn(uy, q[4]), wz = __fmul_rn(uz, q[5]);
+            const float A = __fadd_rn(__fadd_rn(__fmul_rn(wx, wx), __fmul_rn(wy, wy)), __fmul_rn(wz, wz));
+            const float B = __fadd_rn(__fadd_rn(__fmul_rn(rx, wx), __fmul_rn(ry, wy)), __fmul_rn(rz, wz));
+            float t = -__fdiv_rn(B, A);
+            t = fminf(fmaxf(t, -h), h);
+            const float px = __fadd_rn(rx, __fmul_rn(wx, t));
+            const float py = __fadd_rn(ry, __fmul_rn(wy, t));
+            const float pz = __fadd_rn(rz, __fmul_rn(wz, t));
+            const float Q = __fadd_rn(__fadd_rn(__fmul_rn(px, px), __fmul_rn(py, py)), __fmul_rn(pz, pz));
+            hit = Q <= 1.0f;
+        }
+    }
+    if (e < n) keep[e] = hit ? 1 : 0;
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (m) {
+        const unsigned lane = threadIdx.x & 31u;
+        unsigned long long base = 0;
+        if (lane == (unsigned)(__ffs(m) - 1)) base = atomicAdd(counter, (unsigned long long)__popc(m));
+        base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+        if (hit && perm) perm[base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)e;
+    }
+}
+
 static inline unsigned grid_for(uint64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
 
-void launch_bin_keys(const GridF32 &g, int tile_log2, const EventPtrs &ev, uint64_t n, uint32_t *key, uint32_t *hist,
-                     uint32_t nbins, cudaStream_t s) {
-    if (n) bin_keys_kernel<<<grid_for(n), kBlock, 0, s>>>(g, tile_log2, ev, n, key, hist, nbins);
+void launch_bin_keys(const GridF32 &g, int tile_log2, const SubBin &sb, const EventPtrs &ev, uint64_t n, uint32_t *key,
+                     uint8_t *sub, uint32_t *hist, uint32_t nbins, cudaStream_t s) {
+    if (n) bin_keys_kernel<<<grid_for(n), kBlock, 0, s>>>(g, tile_log2, sb, ev, n, key, sub, hist, nbins);
 }
 
-void launch_exclusive_scan_u32(const uint32_t *in, uint32_t *out, uint32_t *out2, uint32_t n, cudaStream_t s) {
-    if (n) exclusive_scan_kernel<<<1, 1024, 0, s>>>(in, out, out2, n);
+uint32_t scan_tmp_elems(uint32_t n) { return 2 * ((n + kScanChunk - 1) / kScanChunk + 1); }
+
+int launch_exclusive_scan_u32(const uint32_t *in, uint32_t *out, uint32_t *tmp, uint32_t n, cudaStream_t s) {
+    if (!n) return 0;
+    const uint32_t chunks = (n + kScanChunk - 1) / kScanChunk;
+    if (chunks <= 4 || !tmp) {
+        exclusive_scan_kernel<<<1, 1024, 0, s>>>(in, out, nullptr, n);
+        return 1;
+    }
+    scan_chunk_sums_kernel<<<chunks, kBlock, 0, s>>>(in, n, tmp);
+    exclusive_scan_kernel<<<1, 1024, 0, s>>>(tmp, tmp + chunks + 1, nullptr, chunks);
+    scan_chunks_kernel<<<chunks, kBlock, 0, s>>>(in, n, tmp + chunks + 1, out);
+    return 3;
 }
 
-void launch_scatter_perm(const uint32_t *key, uint64_t n, uint32_t nbins, uint32_t *cursor, uint32_t *perm,
-                         cudaStream_t s) {
-    if (n) scatter_perm_kernel<<<grid_for(n), kBlock, 0, s>>>(key, n, nbins, cursor, perm);
+void launch_scatter_perm(const uint32_t *key, const uint8_t *sub, uint32_t S, uint64_t n, uint32_t nbins,
+                         uint32_t *cursor, uint32_t *perm, cudaStream_t s) {
+    if (n) scatter_perm_kernel<<<grid_for(n), kBlock, 0, s>>>(key, sub, S, n, nbins, cursor, perm);
+}
+
+void launch_strided_copy(const uint32_t *fine, uint32_t S, uint32_t count, uint32_t *out, cudaStream_t s) {
+    if (count) strided_copy_kernel<<<(count + kBlock - 1) / kBlock, kBlock, 0, s>>>(fine, S, count, out);
 }
 
 void launch_gather(const float *in, const uint32_t *perm, uint64_t n, float *out, cudaStream_t s) {
@@ -196,6 +361,11 @@ void launch_region_ids(const EventPtrs &ev, uint64_t n, const RegionBounds &rb, 
 void launch_region_scatter(const int32_t *region, uint64_t n, int n_regions, unsigned long long *cursor,
                            uint32_t *perm, cudaStream_t s) {
     if (n) region_scatter_kernel<<<grid_for(n), kBlock, 0, s>>>(region, n, n_regions, cursor, perm);
+}
+
+void launch_scatter_keep(const EventPtrs &ev, uint64_t n, const EllipsoidSet &es, float h, uint8_t *keep,
+                         uint32_t *perm, unsigned long long *counter, cudaStream_t s) {
+    if (n) scatter_keep_kernel<<<grid_for(n), kBlock, 0, s>>>(ev, n, es, h, keep, perm, counter);
 }
 
 }  // namespace tofmlem

@@ -149,3 +149,71 @@ void launch_add(float *dst, const float *src, uint64_t n, cudaStream_t s) {
 }
 
 }  // namespace tofmlem
+
+namespace tofmlem {
+
+// ---------------------------------------------------------------------------------------------------------------
+// NEXT-2: 3x3x3 median filter between iterations ("we introduced a median filter between MLEM
+// iterations"; the size is not stated -> R23: the 27-voxel cube, edges replicated).  One thread per output voxel:
+// 27 loads (neighbouring threads share them through L1) and a forgetful-selection network in registers: keep 15
+// values, drop their minimum and maximum (neither can be the median of 27), take in one more value, repeat; the
+// last three values' middle one is the 14th smallest of the 27.  The result is one of the inputs, so the filter
+// is bit-exact against any correct implementation.
+__device__ __forceinline__ void cmpxchg(float &a, float &b) {
+    const float lo = fminf(a, b), hi = fmaxf(a, b);
+    a = lo;
+    b = hi;
+}
+
+__global__ void __launch_bounds__(kBlock) median3_kernel(const float *__restrict__ in, float *__restrict__ out, int nx,
+                                                         int ny, int nz) {
+    const uint64_t nvox = (uint64_t)nx * ny * nz;
+    const uint64_t j = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (j >= nvox) return;
+    const int x = (int)(j % (uint64_t)nx);
+    const uint64_t t = j / (uint64_t)nx;
+    const int y = (int)(t % (uint64_t)ny), z = (int)(t / (uint64_t)ny);
+    int xo[3], yo[3], zo[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        xo[d] = min(max(x + d - 1, 0), nx - 1);
+        yo[d] = min(max(y + d - 1, 0), ny - 1);
+        zo[d] = min(max(z + d - 1, 0), nz - 1);
+    }
+    float v[27];
+#pragma unroll
+    for (int dz = 0; dz < 3; ++dz)
+#pragma unroll
+        for (int dy = 0; dy < 3; ++dy) {
+            const float *row = in + ((size_t)zo[dz] * ny + yo[dy]) * nx;
+#pragma unroll
+            for (int dx = 0; dx < 3; ++dx) v[(dz * 3 + dy) * 3 + dx] = __ldg(row + xo[dx]);
+        }
+    // working set w = v[0..14]; v[15..26] are fed in one per stage
+#pragma unroll
+    for (int s = 0; s < 13; ++s) {
+#pragma unroll
+        for (int i = s + 1; i <= 14; ++i) cmpxchg(v[s], v[i]);  // minimum of the active range -> v[s]
+#pragma unroll
+        for (int i = s + 1; i < 14; ++i) cmpxchg(v[i], v[14]);  // maximum -> v[14]
+        if (s < 12) v[14] = v[15 + s];                          // forget both, take the next value in
+    }
+    out[j] = v[13];
+}
+
+void launch_median3(const float *in, float *out, int nx, int ny, int nz, cudaStream_t s) {
+    const uint64_t nvox = (uint64_t)nx * ny * nz;
+    median3_kernel<<<(unsigned)((nvox + kBlock - 1) / kBlock), kBlock, 0, s>>>(in, out, nx, ny, nz);
+}
+
+// w <- exp(w)  (NEXT-3: attenuation weight from the line integral of mu, R19); accurate expf
+__global__ void __launch_bounds__(kBlock) exp_kernel(float *__restrict__ w, uint64_t n) {
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) w[i] = expf(w[i]);
+}
+
+void launch_exp(float *w, uint64_t n, cudaStream_t s) {
+    if (n) exp_kernel<<<grid_for(n), kBlock, 0, s>>>(w, n);
+}
+
+}  // namespace tofmlem

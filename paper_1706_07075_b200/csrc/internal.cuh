@@ -31,6 +31,7 @@ struct EventPtrs {
 struct DeviceStats {
     unsigned long long n_valid;
     unsigned long long visits;
+    unsigned long long reds;  // reduction instructions (requests to the L2 atomic units) of the scatter walk
     double sum_image_sens;
 };
 
@@ -48,8 +49,10 @@ void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint
                         float *out, bool vec_ok, cudaStream_t s);
 // queues: kMaxQueues work counters owned by the context (persistent variant), may be NULL
 constexpr int kMaxQueues = 2048;
-void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *image,
-                          float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues, cudaStream_t s);
+// evw: optional per-event weights (NEXT-3), NULL => 1
+void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *evw,
+                          const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,
+                          cudaStream_t s);
 
 // ---- image_ops.cu
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);
@@ -61,14 +64,25 @@ void launch_dot_f64(const float *a, const float *b, uint64_t n, double *d_out /*
                     cudaStream_t s);
 void launch_scale(float *x, float a, uint64_t n, cudaStream_t s);
 void launch_add(float *dst, const float *src, uint64_t n, cudaStream_t s);
+void launch_median3(const float *in, float *out, int nx, int ny, int nz, cudaStream_t s);
+void launch_exp(float *w, uint64_t n, cudaStream_t s);
 
 // ---- binning.cu
-void launch_bin_keys(const GridF32 &g, int tile_log2, const EventPtrs &ev, uint64_t n, uint32_t *key,
-                     uint32_t *hist /* nbins+1, zeroed by caller */, uint32_t nbins, cudaStream_t s);
-void launch_exclusive_scan_u32(const uint32_t *in, uint32_t *out, uint32_t *out2 /* optional copy */, uint32_t n,
-                               cudaStream_t s);
-void launch_scatter_perm(const uint32_t *key, uint64_t n, uint32_t nbins, uint32_t *cursor, uint32_t *perm,
-                         cudaStream_t s);
+// Sub-bins: the events of one locality bin are ordered by predicted visit count (S sub-bins of `quantum` visits;
+// sub-bin 0 = the window misses the grid).  S = 1 switches the ordering off.
+struct SubBin {
+    uint32_t S, quantum;
+    float half_window;  // trunc_sigmas * sigma (mm); 0 for non-TOF
+};
+void launch_bin_keys(const GridF32 &g, int tile_log2, const SubBin &sb, const EventPtrs &ev, uint64_t n, uint32_t *key,
+                     uint8_t *sub /* n, or NULL */, uint32_t *hist /* nbins*S+1, zeroed by caller */, uint32_t nbins,
+                     cudaStream_t s);
+uint32_t scan_tmp_elems(uint32_t n);
+// returns the number of kernels launched; tmp: scan_tmp_elems(n) words (NULL: single-block scan)
+int launch_exclusive_scan_u32(const uint32_t *in, uint32_t *out, uint32_t *tmp, uint32_t n, cudaStream_t s);
+void launch_scatter_perm(const uint32_t *key, const uint8_t *sub, uint32_t S, uint64_t n, uint32_t nbins,
+                         uint32_t *cursor, uint32_t *perm, cudaStream_t s);
+void launch_strided_copy(const uint32_t *fine, uint32_t S, uint32_t count, uint32_t *out, cudaStream_t s);
 void launch_gather(const float *in, const uint32_t *perm, uint64_t n, float *out, cudaStream_t s);
 constexpr int kMaxRegions = 64;
 struct RegionBounds {
@@ -81,6 +95,28 @@ void launch_region_ids(const EventPtrs &ev, uint64_t n, const RegionBounds &rb, 
 void launch_region_scatter(const int32_t *region, uint64_t n, int n_regions,
                            unsigned long long *cursor /* n_regions+1 start offsets, advanced */, uint32_t *perm,
                            cudaStream_t s);
+
+constexpr int kMaxEllipsoids = 64;
+struct EllipsoidSet {
+    float v[6 * kMaxEllipsoids];  // per ellipsoid: centre x, y, z, reciprocal semi-axes 1/ax, 1/ay, 1/az
+    int n;
+};
+void launch_scatter_keep(const EventPtrs &ev, uint64_t n, const EllipsoidSet &es, float h, uint8_t *keep,
+                         uint32_t *perm /* may be NULL */, unsigned long long *counter /* zeroed by caller */,
+                         cudaStream_t s);
+
+// ---- sampled.cu (the paper's K-sample TOF kernel, NEXT-1)
+struct SampleLutEntry {
+    double offset;  // mm along the LOR from the kernel centre
+    float weight;   // Gaussian weight, the K weights sum to one
+    float pad;
+};
+void launch_sampled_forward(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
+                            const float *image, float *fwd, cudaStream_t s);
+void launch_sampled_backproject(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
+                                const float *values, float *out, cudaStream_t s);
+void launch_sampled_em(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
+                       const float *evw, const float *image, float *corr, DeviceStats *stats, cudaStream_t s);
 
 // ---- probe.cu
 int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *ms, cudaStream_t s);

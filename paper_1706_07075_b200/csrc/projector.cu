@@ -43,6 +43,13 @@ __device__ __forceinline__ void red_v4(float *p, float a, float b, float c, floa
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
+__device__ __forceinline__ void red_v4_if(bool p, float *ptr, float a, float b, float c, float d) {
+    asm volatile(
+        "{\n .reg .pred q;\n setp.ne.s32 q, %5, 0;\n @q red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n}" ::"l"(ptr),
+        "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)p)
+        : "memory");
+}
+
 constexpr float kBigT = 1.0e30f;
 
 // Three-way select on the layout index for the pointer triples (a dynamically indexed pointer array in the
@@ -208,34 +215,39 @@ __device__ __forceinline__ float ray_gather(const ProjParams &P, const Ray &r, c
 // VEC: one 16-byte vector reduction per aligned group of 4 voxels (needs a 16-byte aligned `out` whose
 // allocation covers whole groups); otherwise one scalar reduction per voxel.
 template <bool TOF, bool VEC>
-__device__ __forceinline__ void ray_scatter(const ProjParams &P, const Ray &r, float *__restrict__ out, float scale) {
+__device__ __forceinline__ int ray_scatter(const ProjParams &P, const Ray &r, float *__restrict__ out, float scale) {
     Walker<TOF> wk(r);
-    int at;
+    int at, reds = 1;
     bool done;
     if (VEC) {
+        // The flush is a predicated instruction, not a branch: some lane of a warp flushes in nearly every step
+        // (ncu r01b: 97 % of the warp iterations), so a branch only adds its re-convergence overhead.
         int grp = r.idx >> 2;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll 2
         do {
             const float val = wk.step(P, r, at, done) * scale;
             const int g = at >> 2;
-            if (g != grp) {
-                red_v4(out + 4 * (size_t)grp, a0, a1, a2, a3);
-                a0 = a1 = a2 = a3 = 0.f;
-                grp = g;
-            }
+            const bool fl = g != grp;
+            red_v4_if(fl, out + 4 * (size_t)grp, a0, a1, a2, a3);
+            reds += fl;
+            grp = g;
             const int sl = at & 3;  // each voxel is met once per ray: plain writes, no accumulation
-            a0 = sl == 0 ? val : a0;
-            a1 = sl == 1 ? val : a1;
-            a2 = sl == 2 ? val : a2;
-            a3 = sl == 3 ? val : a3;
+            a0 = sl == 0 ? val : (fl ? 0.f : a0);
+            a1 = sl == 1 ? val : (fl ? 0.f : a1);
+            a2 = sl == 2 ? val : (fl ? 0.f : a2);
+            a3 = sl == 3 ? val : (fl ? 0.f : a3);
         } while (!done);
         red_v4(out + 4 * (size_t)grp, a0, a1, a2, a3);
     } else {
+        reds = 0;
         do {
             const float w = wk.step(P, r, at, done);
             atomicAdd(out + at, w * scale);  // zero-length chords (corner crossings) add +0: harmless, rare
+            ++reds;
         } while (!done);
     }
+    return reds;
 }
 
 
@@ -293,17 +305,19 @@ __global__ void __launch_bounds__(kBlock) backproject_kernel(ProjParams P, Event
 // recomputes the weights and scatters w / fwd (the Gaussian normalisation cancels in a_ej / fwd_e).
 template <bool TOF, bool VEC>
 __device__ __forceinline__ void em_event(const ProjParams &P, const EventPtrs &ev, uint64_t e, uint64_t n,
-                                         const float *__restrict__ image, float *__restrict__ corr, int &visits,
-                                         bool &valid) {
+                                         const float *__restrict__ evw, const float *__restrict__ image,
+                                         float *__restrict__ corr, int &visits, bool &valid, int &reds) {
     Ray r;
     int layout;
     visits = 0;
+    reds = 0;
     valid = false;
     if (e < n && load_and_setup<TOF, false>(P, ev, e, r, layout)) {
         const float acc = ray_gather<TOF>(P, r, image, visits);
         if (acc > 0.0f) {  // R9
             valid = true;
-            ray_scatter<TOF, VEC>(P, r, corr, 1.0f / acc);
+            // evw: optional per-event weight (attenuation correction applied to the LOR, R19)
+            reds = ray_scatter<TOF, VEC>(P, r, corr, (evw ? __ldg(evw + e) : 1.0f) / acc);
         }
     }
 }
@@ -311,17 +325,20 @@ __device__ __forceinline__ void em_event(const ProjParams &P, const EventPtrs &e
 // Grid-order form: one CTA per 256-event chunk, chunks interleaved (comment (5) at the top).
 template <bool TOF, bool VEC>
 __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, EventPtrs ev, uint64_t n,
+                                                               const float *__restrict__ evw,
                                                                const float *__restrict__ image,
                                                                float *__restrict__ corr, DeviceStats *stats) {
-    int visits;
+    int visits, reds;
     bool valid;
-    em_event<TOF, VEC>(P, ev, event_index(P.stride), n, image, corr, visits, valid);
+    em_event<TOF, VEC>(P, ev, event_index(P.stride), n, evw, image, corr, visits, valid, reds);
     // per-warp counters -> one atomic per warp
     const unsigned nv = __popc(__ballot_sync(0xffffffffu, valid));
     const unsigned vis = __reduce_add_sync(0xffffffffu, (unsigned)visits);
+    const unsigned nr = __reduce_add_sync(0xffffffffu, (unsigned)reds);
     if ((threadIdx.x & 31) == 0 && stats) {
         if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
         if (vis) atomicAdd(&stats->visits, (unsigned long long)vis);
+        if (nr) atomicAdd(&stats->reds, (unsigned long long)nr);
     }
 }
 
@@ -333,13 +350,14 @@ __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, Eve
 // events sorted to the end of the list make the last segments empty).  Measured at cfg-3: 30.2 -> 25.2 ms.
 template <bool TOF, bool VEC>
 __global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, EventPtrs ev, uint64_t n,
+                                                               const float *__restrict__ evw,
                                                                const float *__restrict__ image,
                                                                float *__restrict__ corr, DeviceStats *stats,
                                                                unsigned *queues, unsigned nseg, unsigned per_seg) {
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
-    unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0;
+    unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
         if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
@@ -349,17 +367,20 @@ __global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, Eve
             seg = (seg + 61u) % nseg;  // 61 is prime: visits every segment for any nseg not a multiple of 61
             continue;
         }
-        int visits;
+        int visits, reds;
         bool valid;
-        em_event<TOF, VEC>(P, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, image, corr, visits, valid);
+        em_event<TOF, VEC>(P, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, visits, valid, reds);
         nv += valid;
         vis += visits;
+        nr += reds;
     }
     nv = __reduce_add_sync(0xffffffffu, nv);
     vis = __reduce_add_sync(0xffffffffu, vis);
+    nr = __reduce_add_sync(0xffffffffu, nr);
     if (lane == 0 && stats) {
         if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
         if (vis) atomicAdd(&stats->visits, (unsigned long long)vis);
+        if (nr) atomicAdd(&stats->reds, (unsigned long long)nr);
     }
 }
 
@@ -396,8 +417,8 @@ void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint
 }
 
 template <bool TOF, bool VEC>
-static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *image, float *corr,
-                      DeviceStats *stats, unsigned *queues, cudaStream_t s) {
+static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
+                      float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
     if (p.variant != 1 && queues) {
         static int n_sm = 0, per_sm = 0;  // per instantiation; one device per process
         if (!n_sm) {
@@ -412,26 +433,27 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         const uint64_t wchunks = (n + 31) / 32;
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
         cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-        em_persistent_kernel<TOF, VEC><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, ev, n, image, corr, stats,
-                                                                                         queues, nseg, per_seg);
+        em_persistent_kernel<TOF, VEC><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, ev, n, evw, image, corr,
+                                                                                         stats, queues, nseg, per_seg);
     } else {
-        em_correction_kernel<TOF, VEC><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, image, corr, stats);
+        em_correction_kernel<TOF, VEC><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
     }
 }
 
-void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *image,
-                          float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
+void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *evw,
+                          const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,
+                          cudaStream_t s) {
     if (n == 0) return;
     if (tof) {
         if (vec_ok)
-            launch_em<true, true>(p, ev, n, image, corr, stats, queues, s);
+            launch_em<true, true>(p, ev, n, evw, image, corr, stats, queues, s);
         else
-            launch_em<true, false>(p, ev, n, image, corr, stats, queues, s);
+            launch_em<true, false>(p, ev, n, evw, image, corr, stats, queues, s);
     } else {
         if (vec_ok)
-            launch_em<false, true>(p, ev, n, image, corr, stats, queues, s);
+            launch_em<false, true>(p, ev, n, evw, image, corr, stats, queues, s);
         else
-            launch_em<false, false>(p, ev, n, image, corr, stats, queues, s);
+            launch_em<false, false>(p, ev, n, evw, image, corr, stats, queues, s);
     }
 }
 

@@ -20,6 +20,9 @@ TOFMLEM_OK, TOFMLEM_EINVAL, TOFMLEM_ENOMEM, TOFMLEM_ECUDA, TOFMLEM_ESTATE, TOFML
 OPT_TRUNC_SIGMAS, OPT_SENS_FLOOR_REL, OPT_TILE_LOG2, OPT_PROJECTOR, OPT_SAMPLES_K, OPT_SHELL_MM = 1, 2, 3, 4, 5, 6
 OPT_CTA_INTERLEAVE = 7
 OPT_EM_VARIANT = 8
+OPT_SUBBINS = 9
+OPT_MEDIAN = 10
+PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = (
@@ -28,6 +31,8 @@ SYMBOLS = (
     "tofmlem_iterate", "tofmlem_iterate_host", "tofmlem_bin_events", "tofmlem_num_bins", "tofmlem_gather_events",
     "tofmlem_split_regions", "tofmlem_region_zbounds", "tofmlem_region_grid", "tofmlem_reconstruct_regions",
     "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
+    "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
+    "tofmlem_gather_f32", "tofmlem_scatter_reject",
 )
 
 
@@ -51,7 +56,7 @@ class Events(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_valid", C.c_uint64), ("n_skipped", C.c_uint64), ("visits", C.c_uint64),
-                ("sum_image_sens", C.c_double)]
+                ("sum_image_sens", C.c_double), ("reductions", C.c_uint64)]
 
 
 class TofMlemError(RuntimeError):
@@ -234,6 +239,50 @@ class Context:
             self._h, C.byref(e), C.c_uint64(n), C.c_int(n_regions), C.c_void_p(zb),
             C.c_void_p(_ptr(image_out, torch.float32, "cuda", self.nvox)),
             C.c_void_p(_ptr(sens, torch.float32, "cuda", self.nvox)), C.c_int(iters)))
+
+    # -- widened rows
+    def median3(self, src: torch.Tensor, dst: torch.Tensor):
+        self._check(self._L.tofmlem_median3(self._h, C.c_void_p(_ptr(src, torch.float32, "cuda", self.nvox)),
+                                            C.c_void_p(_ptr(dst, torch.float32, "cuda", self.nvox))))
+
+    def attenuation_weights(self, lors, n: int, mu: torch.Tensor, weight: torch.Tensor):
+        e = _events({**lors, "dt": None}, n)
+        self._check(self._L.tofmlem_attenuation_weights(self._h, C.byref(e), C.c_uint64(n),
+                                                        C.c_void_p(_ptr(mu, torch.float32, "cuda", self.nvox)),
+                                                        C.c_void_p(_ptr(weight, torch.float32, "cuda", n))))
+
+    def em_correction_weighted(self, ev, n: int, weight: Optional[torch.Tensor], image: torch.Tensor,
+                               corr: torch.Tensor):
+        e = _events(ev, n)
+        self._check(self._L.tofmlem_em_correction_weighted(
+            self._h, C.byref(e), C.c_uint64(n), C.c_void_p(_ptr(weight, torch.float32, "cuda", n)),
+            C.c_void_p(_ptr(image, torch.float32, "cuda", self.nvox)),
+            C.c_void_p(_ptr(corr, torch.float32, "cuda", self.nvox))))
+
+    def iterate_weighted(self, ev, n: int, weight: Optional[torch.Tensor], image: torch.Tensor, sens: torch.Tensor,
+                         iters: int):
+        e = _events(ev, n)
+        self._check(self._L.tofmlem_iterate_weighted(
+            self._h, C.byref(e), C.c_uint64(n), C.c_void_p(_ptr(weight, torch.float32, "cuda", n)),
+            C.c_void_p(_ptr(image, torch.float32, "cuda", self.nvox)),
+            C.c_void_p(_ptr(sens, torch.float32, "cuda", self.nvox)), C.c_int(iters)))
+
+    def gather_f32(self, src: torch.Tensor, perm: torch.Tensor, n: int, dst: torch.Tensor):
+        self._check(self._L.tofmlem_gather_f32(self._h, C.c_void_p(_ptr(src, torch.float32, "cuda", n)),
+                                               C.c_void_p(_ptr(perm, torch.int32, "cuda", n)), C.c_uint64(n),
+                                               C.c_void_p(_ptr(dst, torch.float32, "cuda", n))))
+
+    def scatter_reject(self, ev, n: int, ellipsoids: torch.Tensor, half_width_mm: float, keep: torch.Tensor,
+                       perm: Optional[torch.Tensor]) -> int:
+        """ellipsoids: HOST float32 [n_ell, 6] = centre, reciprocal semi-axes; returns the number of kept events."""
+        e = _events(ev, n)
+        ell = _ptr(ellipsoids, torch.float32, "cpu")
+        kept = C.c_uint64(0)
+        self._check(self._L.tofmlem_scatter_reject(
+            self._h, C.byref(e), C.c_uint64(n), C.c_void_p(ell), C.c_int(ellipsoids.numel() // 6),
+            C.c_float(half_width_mm), C.c_void_p(_ptr(keep, torch.uint8, "cuda", n)),
+            C.c_void_p(_ptr(perm, torch.int32, "cuda", n)), C.byref(kept)))
+        return int(kept.value)
 
     def probe(self, kind: int, buf: torch.Tensor, n_ops: int) -> float:
         """elapsed ms of n_ops float32 REDs (kind 0,1) or gathers (2,3) against buf; see include/tofmlem.h"""
