@@ -126,6 +126,194 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------
+def run_report(args):
+    """Single-GPU reports beside the bench line: cfg-5 sweep, cfg-4 division, widened rows.  Device-timed with CUDA
+    events after a warm-up pass; inputs (>= 280 MB of events) are larger than L2 except where noted."""
+    import torch
+
+    import paper_1706_07075_b200 as pkg
+    import synth
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+
+    def timed(fn, reps=1):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        b.synchronize()
+        return a.elapsed_time(b) / reps
+
+    def binned(ctx, ev, n):
+        key = torch.empty(n, dtype=torch.int32, device=dev)
+        perm = torch.empty(n, dtype=torch.int32, device=dev)
+        sev = {k: torch.empty_like(v) for k, v in ev.items()}
+        ms = timed(lambda: (ctx.bin_events(ev, n, key, perm, None), ctx.gather_events(ev, perm, n, sev)))
+        return sev, perm, ms
+
+    full = synth.FULL
+    g = pkg.make_grid(full.nx, full.ny, full.nz, full.voxel_mm)
+    nvox = g.nvox
+    base = pkg.Context(full.radius_mm, full.axial_mm, g, full.tof_fwhm_ps)
+    m = args.sens_lors or 20_000_000
+    lors = synth.make_sens_lors_chunked(full, m, device=dev)
+    sens = torch.empty(nvox, dtype=torch.float32, device=dev)
+    base.sensitivity(lors, m, sens)
+    del lors
+    probe_buf = torch.zeros(nvox, dtype=torch.float32, device=dev)
+    red_rand = (1 << 30) / (base.probe(0, probe_buf, 1 << 30) * 1e-3)
+    del probe_buf
+    out = {"report": args.report, "data": "synthetic", "dtype": "f32", "sens_lors": m,
+           "red_random_Gps": red_rand / 1e9}
+
+    if args.report == "sweep":
+        # cfg-5: full-body geometry and phantom, 20 % scatter, 3 iterations, seed 5
+        points = []
+        for n in [int(t) for t in args.sweep_events.split(",")]:
+            for fwhm in [float(t) for t in args.sweep_fwhm.split(",")]:
+                cfg = synth.sweep_config(n, fwhm)
+                ev = synth.make_events_chunked(cfg, n, device=dev)
+                if fwhm <= 0:
+                    ev["dt"].zero_()
+                ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
+                sev, _, bin_ms = binned(ctx, ev, n)
+                del ev
+                image = torch.ones(nvox, dtype=torch.float32, device=dev)
+                corr = torch.zeros(nvox, dtype=torch.float32, device=dev)
+
+                def step():
+                    ctx.reset_stats()
+                    ctx.em_correction(sev, n, image, corr)
+                    ctx.update(image, corr, sens)
+
+                step()  # warm-up = iteration 1
+                ms = timed(step, reps=cfg.iters - 1)  # iterations 2..3
+                st = ctx.get_stats()
+                p7 = float((image.double() * sens.double()).sum().item())
+                points.append({
+                    "events": n, "tof_fwhm_ps": fwhm, "ms_per_iteration": ms, "events_per_s": n / (ms * 1e-3),
+                    "n_valid": int(st.n_valid), "visits": int(st.visits), "reductions": int(st.reductions),
+                    "visits_per_valid_event": st.visits / max(1, st.n_valid), "Gvisits_per_s": st.visits / ms / 1e6,
+                    "roofline_frac": st.reductions / (ms * 1e-3) / red_rand, "bin_sort_gather_ms": bin_ms,
+                    "p7_rel_err": abs(p7 - st.n_valid) / max(1, st.n_valid)})
+                print(json.dumps(points[-1]), file=sys.stderr, flush=True)
+                del sev, image, corr, ctx
+                torch.cuda.empty_cache()
+        out["config"] = {"workload": "cfg-5 sweep: 160x160x640 x 3.75 mm, 20% scatter-like, 3 iterations (first = warm-up)"}
+        out["points"] = points
+
+    elif args.report == "division":
+        # cfg-4: the cfg-3 event set split into nine axial regions, each reconstructed on its sub-volume + margin on its
+        # own stream, the extended images summed; compared with the unsplit reconstruction (same x0 = mask).
+        cfg = full
+        n = args.events or cfg.n_events
+        ev = synth.make_events_chunked(cfg, n, device=dev)
+        sev, _, bin_ms = binned(base, ev, n)
+        mx = sens.max()
+        x0 = (sens >= 0.01 * mx).float()
+        whole = x0.clone()
+        base.iterate(sev, n, whole, sens, 1)  # warm-up
+        whole = x0.clone()
+        whole_ms = timed(lambda: base.iterate(sev, n, whole, sens, cfg.iters))
+        del sev
+        split = torch.empty(nvox, dtype=torch.float32, device=dev)
+        base.reconstruct_regions(ev, n, 9, None, split, sens, 1)  # warm-up
+        t0 = time.perf_counter()
+        base.reconstruct_regions(ev, n, 9, None, split, sens, cfg.iters)  # synchronises
+        split_ms = (time.perf_counter() - t0) * 1e3
+        region = torch.empty(n, dtype=torch.int32, device=dev)
+        counts = base.split_regions(ev, n, 9, None, region, None)
+        d = (split.double() - whole.double())
+        big = whole > 0.01 * whole.max()
+        out["config"] = {"workload": f"cfg-4 division: {n} events of cfg-3, 9 regions, {cfg.iters} iterations each"}
+        out.update({
+            "unsplit_ms": whole_ms, "unsplit_bin_ms": bin_ms, "split_total_ms": split_ms,
+            "split_note": "split + permute + nine per-region reconstructions on nine streams + sum, host wall clock of the synchronising call",
+            "region_counts": [int(c) for c in counts],
+            "rel_l2_split_vs_unsplit": float(d.norm() / whole.double().norm()),
+            "max_rel_on_voxels_above_1pct": float((d.abs()[big] / whole.double()[big]).max()),
+            "paper": "PAPER.md:212 'no difference to the whole-body reconstruction' (visual); parity unpinned, no threshold"})
+
+    else:  # widened rows, cfg-3 sizes
+        cfg = full
+        n = args.events or cfg.n_events
+        ev = synth.make_events_chunked(cfg, n, device=dev)
+        res = {}
+        # NEXT-4 first (it is a pre-processing step): TOF scatter rejection against the phantom's body outline
+        import numpy as np
+        ell = np.empty((len(cfg.phantom.parts), 6), np.float32)
+        for i, (c, sa) in enumerate(synth.body_outline(cfg)):
+            ell[i, :3] = c
+            ell[i, 3:] = 1.0 / np.asarray(sa, np.float64)
+        ell_t = torch.from_numpy(ell)
+        keep = torch.empty(n, dtype=torch.uint8, device=dev)
+        perm = torch.empty(n, dtype=torch.int32, device=dev)
+        base.scatter_reject(ev, n, ell_t, 0.0, keep, perm)
+        t0 = time.perf_counter()
+        kept = base.scatter_reject(ev, n, ell_t, 0.0, keep, perm)
+        ms = (time.perf_counter() - t0) * 1e3
+        kinds = synth.event_kinds(cfg, min(n, 4_000_000), device=dev).bool()
+        kk = keep[:kinds.numel()].bool()
+        res["scatter_reject"] = {"ms": ms, "events_per_s": n / (ms * 1e-3), "kept": kept, "kept_fraction": kept / n,
+                                 "hbm_GBs": (28.0 * n + n + 4.0 * kept) / (ms * 1e-3) / 1e9,
+                                 "trues_kept": float(kk[~kinds].float().mean()),
+                                 "scatter_like_kept": float(kk[kinds].float().mean())}
+        del keep, perm
+        # NEXT-3: attenuation weights (non-TOF line integral of a synthetic mu-map) and the weighted EM pass
+        mu = synth.rasterize_mu_map(cfg, device=dev).reshape(-1).contiguous()
+        w = torch.empty(n, dtype=torch.float32, device=dev)
+        base.attenuation_weights(ev, n, mu, w)
+        ms = timed(lambda: base.attenuation_weights(ev, n, mu, w))
+        res["attenuation_weights"] = {"ms": ms, "lors_per_s": n / (ms * 1e-3), "mean_weight": float(w.mean())}
+        sev, perm, _ = binned(base, ev, n)
+        sw = torch.empty_like(w)
+        base.gather_f32(w, perm, n, sw)
+        del ev, w, perm, mu
+        image = torch.ones(nvox, dtype=torch.float32, device=dev)
+        corr = torch.zeros(nvox, dtype=torch.float32, device=dev)
+
+        def pass_w():
+            base.em_correction_weighted(sev, n, sw, image, corr)
+            base.update(image, corr, sens)
+
+        pass_w()
+        ms = timed(pass_w, reps=3)
+        res["weighted_iteration"] = {"ms": ms, "events_per_s": n / (ms * 1e-3)}
+        # NEXT-2: 3x3x3 median filter on the full volume (65.5 MB in + 65.5 MB out: L2-sized, HBM-cold between reps)
+        tmp = torch.empty_like(image)
+        base.median3(image, tmp)
+        ms = timed(lambda: base.median3(image, tmp), reps=5)
+        hbm_peak, _ = load_peaks()
+        res["median3"] = {"ms": ms, "voxels_per_s": nvox / (ms * 1e-3), "algorithmic_GBs": 8.0 * nvox / (ms * 1e-3) / 1e9,
+                          "hbm_frac": 8.0 * nvox / (ms * 1e-3) / 1e9 / hbm_peak}
+        # NEXT-1: the paper's K-sample kernel (K = 32 GPU value, 15 CPU value), fused EM pass + update
+        for K in (32, 15):
+            ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+            ctx.set_option(pkg.OPT_SAMPLES_K, K)
+            ctx.set_option(pkg.OPT_PROJECTOR, pkg.PROJECTOR_SAMPLED)
+            image.fill_(1.0)
+            corr.zero_()
+
+            def pass_k():
+                ctx.reset_stats()
+                ctx.em_correction(sev, n, image, corr)
+                ctx.update(image, corr, sens)
+
+            pass_k()
+            ms = timed(pass_k, reps=3)
+            st = ctx.get_stats()
+            res[f"sampled_K{K}_iteration"] = {"ms": ms, "events_per_s": n / (ms * 1e-3), "samples_kept": int(st.visits),
+                                             "reductions": int(st.reductions), "n_valid": int(st.n_valid),
+                                             "roofline_frac": st.reductions / (ms * 1e-3) / red_rand}
+        out["config"] = {"workload": f"widened rows on cfg-3: {n} events, 160x160x640 x 3.75 mm"}
+        out["results"] = res
+    print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -141,9 +329,16 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-bin", action="store_true", help="skip locality binning (for comparison)")
     ap.add_argument("--subbins", type=int, default=0, help="TOFMLEM_OPT_SUBBINS override (0 = library default)")
+    ap.add_argument("--report", default="", choices=["", "sweep", "division", "next"],
+                    help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
+                         "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
+    ap.add_argument("--sweep-events", default="10000000,146000000,500000000")
+    ap.add_argument("--sweep-fwhm", default="100,300,600,0")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.report:
+        return run_report(args)
 
     import torch
     import torch.distributed as dist
@@ -256,21 +451,27 @@ def main():
     ld_row = n_ops / (ctx.probe(3, probe_buf, n_ops) * 1e-3)
     del probe_buf
     hbm_bytes = 28.0 * n  # algorithmic HBM bytes per launch: 7 float32 per event
+    reds = int(st.reductions)  # reduction instructions of one launch (each is one request to an L2 atomic unit)
     t_hbm = hbm_bytes / (hbm_peak * 1e9)
-    t_red = visits / red_rand  # one RED per visit (events with fwd = 0 do none: a few %)
+    t_red = reds / red_rand
     t_ld = visits / ld_rand
-    t_roof = max(t_hbm, t_red, t_ld)
-    achieved = visits / (kern_ms * 1e-3)
+    achieved = reds / (kern_ms * 1e-3)
     roofline = {
-        "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_rand / 1e9, "unit": "Gvisit/s",
-        "frac": achieved / red_rand, "traffic": None,
-        "kernel": "em_correction_kernel<TOF>", "kernel_ms": kern_ms, "visits_per_launch": visits,
-        "peak_source": "tofmlem_probe kind 0 (random-address RED.ADD.F32 into an L2-resident array of nvox floats), measured in this run",
+        "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_rand / 1e9, "unit": "G reductions/s",
+        "frac": achieved / red_rand,
+        # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3 from the committed ncu --set full capture
+        # (profiles/r01b_em_persistent_ncu_full_metrics.txt); only meaningful for the default full workload
+        "traffic": 8.256535e9 if (args.workload == "full" and not args.events) else None,
+        "kernel": "em_persistent_kernel<TOF, v4>", "kernel_ms": kern_ms, "visits_per_launch": visits,
+        "reductions_per_launch": reds, "visits_per_reduction": visits / max(1, reds),
+        "visits_Gps": visits / (kern_ms * 1e-3) / 1e9,
+        "peak_source": "tofmlem_probe kind 0 (random-address RED.ADD.F32 into an L2-resident array of nvox floats: the "
+                       "request rate of the L2 atomic units), measured in this run",
         "probes_Gops": {"red_random": red_rand / 1e9, "red_row": red_row / 1e9, "gather_random": ld_rand / 1e9,
                         "gather_row": ld_row / 1e9},
         "t_roof_ms": {"hbm": t_hbm * 1e3, "red": t_red * 1e3, "gather": t_ld * 1e3},
         "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_GBs": hbm_bytes / (kern_ms * 1e-3) / 1e9, "peak_GBs": hbm_peak,
-                "peak_source": peak_src},
+                "frac": hbm_bytes / (kern_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src},
     }
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timed region
