@@ -47,6 +47,13 @@ def test_argument_errors_without_gpu():
     assert L.tofmlem_destroy(None) == 0
     assert L.tofmlem_num_bins(None) == 0
     assert L.tofmlem_iterate(None, None, ctypes.c_uint64(0), None, None, 1) == -1
+    # widened rows: a NULL context is rejected by every entry point
+    assert L.tofmlem_iterate_weighted(None, None, ctypes.c_uint64(0), None, None, None, 1) == -1
+    assert L.tofmlem_em_correction_weighted(None, None, ctypes.c_uint64(0), None, None, None) == -1
+    assert L.tofmlem_median3(None, None, None) == -1
+    assert L.tofmlem_attenuation_weights(None, None, ctypes.c_uint64(0), None, None) == -1
+    assert L.tofmlem_gather_f32(None, None, None, ctypes.c_uint64(0), None) == -1
+    assert L.tofmlem_scatter_reject(None, None, ctypes.c_uint64(0), None, 1, ctypes.c_float(0.0), None, None, None) == -1
 
 
 def test_no_cpu_fallback():
