@@ -228,6 +228,18 @@ def run_report(args):
         counts = base.split_regions(ev, n, 9, None, region, None)
         d = (split.double() - whole.double())
         big = whole > 0.01 * whole.max()
+        # where the difference sits: slices within the region margin of an internal border vs the region interiors
+        zb = base.region_zbounds(9)
+        ks = [int(round((float(z) - g.oz) / g.vz)) for z in zb]
+        _, z0r, z1r = base.region_grid(9, None, 1)
+        margin = ks[1] - z0r
+        near = torch.zeros(cfg.nz, dtype=torch.bool, device=dev)
+        for k in ks[1:-1]:
+            near[max(0, k - margin):min(cfg.nz, k + margin)] = True
+        near_v = near.repeat_interleave(cfg.nx * cfg.ny)
+        w2 = whole.double()
+        interior_l2 = float(d[~near_v].norm() / w2[~near_v].norm())
+        border_l2 = float(d[near_v].norm() / w2[near_v].norm())
         out["config"] = {"workload": f"cfg-4 division: {n} events of cfg-3, 9 regions, {cfg.iters} iterations each"}
         out.update({
             "unsplit_ms": whole_ms, "unsplit_bin_ms": bin_ms, "split_total_ms": split_ms,
@@ -235,6 +247,8 @@ def run_report(args):
             "region_counts": [int(c) for c in counts],
             "rel_l2_split_vs_unsplit": float(d.norm() / whole.double().norm()),
             "max_rel_on_voxels_above_1pct": float((d.abs()[big] / whole.double()[big]).max()),
+            "margin_slices": margin, "rel_l2_region_interiors": interior_l2, "rel_l2_within_margin_of_borders": border_l2,
+            "border_slice_fraction": float(near.float().mean()),
             "paper": "PAPER.md:212 'no difference to the whole-body reconstruction' (visual); parity unpinned, no threshold"})
 
     else:  # widened rows, cfg-3 sizes

@@ -176,6 +176,7 @@ int ensure_lut(tofmlem_ctx *ctx) {
         w[k] = exp(-0.5 * r * r);
         sum += w[k];
         ctx->h_lut[k].offset = off;
+        ctx->h_lut[k].offset_f = (float)off;
     }
     for (int k = 0; k < K; ++k) ctx->h_lut[k].weight = (float)(w[k] / sum);
     CU(cudaMalloc(&ctx->d_lut, K * sizeof(SampleLutEntry)));
@@ -193,7 +194,7 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p, const EventPtrs &ev, uint64_t
     if (ctx->projector == 1) {
         int rc = ensure_lut(ctx);
         if (rc) return rc;
-        launch_sampled_em(p, ctx->d_lut, ctx->samples_k, ev, n, evw, d_image, d_corr, ctx->d_stats, s);
+        launch_sampled_em(p, ctx->d_lut, ctx->samples_k, ev, n, evw, d_image, d_corr, ctx->d_stats, ctx->d_queues, s);
     } else {
         launch_em_correction(p, ctx->tof, ev, n, evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, s);
     }
@@ -751,7 +752,7 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
     const size_t slice = (size_t)ctx->grid.nx * ctx->grid.ny;
     int32_t *d_region = nullptr;
     uint32_t *d_perm = nullptr;
-    float *d_sorted = nullptr;
+    float *d_sorted = nullptr, *d_binned = nullptr;
     const uint64_t stride = (n + 3) & ~3ull;
     std::vector<uint64_t> counts(n_regions);
     std::vector<tofmlem_ctx *> subs(n_regions, nullptr);
@@ -772,6 +773,7 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         cudaFree(d_region);
         cudaFree(d_perm);
         cudaFree(d_sorted);
+        cudaFree(d_binned);
     };
 #define RCU(call)                                          \
     do {                                                   \
@@ -795,6 +797,7 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
     RCU(cudaMalloc(&d_region, n * sizeof(int32_t)));
     RCU(cudaMalloc(&d_perm, n * sizeof(uint32_t)));
     RCU(cudaMalloc(&d_sorted, 7 * stride * sizeof(float)));
+    RCU(cudaMalloc(&d_binned, 7 * stride * sizeof(float)));
     RRC(tofmlem_split_regions(ctx, ev, n, n_regions, h_zbounds, d_region, d_perm, counts.data()));
     tofmlem_events_mut sorted{d_sorted, d_sorted + stride, d_sorted + 2 * stride, d_sorted + 3 * stride,
                               d_sorted + 4 * stride, d_sorted + 5 * stride, ev->dt ? d_sorted + 6 * stride : nullptr};
@@ -828,7 +831,23 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         sc->launches += 1;
         tofmlem_events sub_ev{sorted.x1 + off, sorted.y1 + off, sorted.z1 + off, sorted.x2 + off, sorted.y2 + off,
                               sorted.z2 + off, sorted.dt ? sorted.dt + off : nullptr};
-        rc = iterate_device(sc, counts[r] ? ev_ptrs(&sub_ev) : EventPtrs{}, counts[r], nullptr, images[r], sens_r, iters, false);
+        // locality binning inside the region (on its own grid and stream); the region-id and region-permutation buffers
+        // are free again by now (the region streams start after `ready`) and serve as key / permutation scratch
+        tofmlem_events_mut bin_ev{d_binned + off, d_binned + stride + off, d_binned + 2 * stride + off,
+                                  d_binned + 3 * stride + off, d_binned + 4 * stride + off, d_binned + 5 * stride + off,
+                                  sorted.dt ? d_binned + 6 * stride + off : nullptr};
+        if (counts[r]) {
+            rc = tofmlem_bin_events(sc, &sub_ev, counts[r], reinterpret_cast<uint32_t *>(d_region) + off, d_perm + off, nullptr);
+            if (rc == TOFMLEM_OK) rc = tofmlem_gather_events(sc, &sub_ev, d_perm + off, counts[r], &bin_ev);
+            if (rc != TOFMLEM_OK) {
+                ctx->err = sc->err;
+                cudaDeviceSynchronize();
+                cleanup();
+                return rc;
+            }
+        }
+        tofmlem_events run_ev{bin_ev.x1, bin_ev.y1, bin_ev.z1, bin_ev.x2, bin_ev.y2, bin_ev.z2, bin_ev.dt};
+        rc = iterate_device(sc, counts[r] ? ev_ptrs(&run_ev) : EventPtrs{}, counts[r], nullptr, images[r], sens_r, iters, false);
         if (rc != TOFMLEM_OK) {
             ctx->err = sc->err;
             cudaDeviceSynchronize();

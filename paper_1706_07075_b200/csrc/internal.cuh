@@ -109,14 +109,15 @@ void launch_scatter_keep(const EventPtrs &ev, uint64_t n, const EllipsoidSet &es
 struct SampleLutEntry {
     double offset;  // mm along the LOR from the kernel centre
     float weight;   // Gaussian weight, the K weights sum to one
-    float pad;
+    float offset_f; // offset rounded to float32 (fast path of the voxel decision)
 };
 void launch_sampled_forward(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
                             const float *image, float *fwd, cudaStream_t s);
 void launch_sampled_backproject(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
                                 const float *values, float *out, cudaStream_t s);
 void launch_sampled_em(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
-                       const float *evw, const float *image, float *corr, DeviceStats *stats, cudaStream_t s);
+                       const float *evw, const float *image, float *corr, DeviceStats *stats,
+                       unsigned *queues /* kMaxQueues work counters */, cudaStream_t s);
 
 // ---- probe.cu
 int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *ms, cudaStream_t s);

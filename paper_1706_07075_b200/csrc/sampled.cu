@@ -12,6 +12,12 @@
 // floating point: it is taken in fp64 with the oracle's expression floor((p1 + u s - o) / v) (single rounded
 // operations, no contraction), evaluated as a multiplication by 1/v and re-done with the exact division only when
 // the product is within 1e-9 of an integer (the only case where the two can differ).
+//
+// Fast path: that fp64 expression is only evaluated for samples that come close to a voxel plane.  Per axis the
+// position of sample k in voxel units is q0 + offset_k * (u / v) with q0 the position of the kernel centre; relative to
+// floor(q0) this is a float32 fma whose error is below 1e-5 voxel for any window up to a few hundred voxels, so when
+// the float32 value is farther than `guard` = 1e-4 + 1e-5 |q| from an integer its floor IS the fp64 decision; otherwise
+// (about one sample in a thousand) the exact fp64 path decides.  Results are identical to the all-fp64 kernel.
 #include "internal.cuh"
 
 namespace tofmlem {
@@ -25,6 +31,9 @@ __device__ __forceinline__ bool finite_f(float x) { return fabsf(x) <= 3.4028234
 struct SampledRay {
     double p1[3], u[3];
     double s_c, L;
+    int base[3];   // floor of the kernel centre's position in voxel units, per axis
+    float f0[3];   // its fractional part
+    float du[3];   // u / v: voxels per mm along the LOR
 };
 
 __device__ __forceinline__ bool sampled_setup(const EventPtrs &ev, uint64_t e, SampledRay &r) {
@@ -59,13 +68,36 @@ __device__ __forceinline__ int sample_voxel(double p1, double u, double s, doubl
     return (int)f;
 }
 
+__device__ __forceinline__ void sampled_fast_setup(const ProjParams &P, SampledRay &r) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double q0 = ((r.p1[a] + r.u[a] * r.s_c) - P.o[a]) * P.iv[a];
+        const double fl = floor(q0);
+        // a centre far outside the grid cannot produce an in-grid sample through the fast path: clamp the base so that
+        // the int conversion is defined; such samples fail the bounds test either way
+        r.base[a] = (int)fmax(-1.0e9, fmin(1.0e9, fl));
+        r.f0[a] = (float)(q0 - fl);
+        r.du[a] = (float)(r.u[a] * P.iv[a]);
+    }
+}
+
+// voxel index along one axis through the float32 fast path; falls back to the exact fp64 decision near a voxel plane
+__device__ __forceinline__ int sample_voxel_fast(const ProjParams &P, const SampledRay &r, int a, float off, double s) {
+    const float qf = fmaf(off, r.du[a], r.f0[a]);
+    const float guard = fmaf(1.0e-5f, fabsf(qf), 1.0e-4f);
+    if (fabsf(qf - rintf(qf)) < guard || !(fabsf(qf) < 1.0e6f))
+        return sample_voxel(r.p1[a], r.u[a], s, P.o[a], P.v[a], P.iv[a], P.n[a]);
+    const int i = r.base[a] + (int)floorf(qf);
+    return (i < 0 || i >= P.n[a]) ? -1 : i;
+}
+
 // flat voxel index of sample k, or -1 when the sample is dropped
-__device__ __forceinline__ int sample_index(const ProjParams &P, const SampledRay &r, double offset) {
-    const double s = __dadd_rn(r.s_c, offset);
+__device__ __forceinline__ int sample_index(const ProjParams &P, const SampledRay &r, const SampleLutEntry &l) {
+    const double s = __dadd_rn(r.s_c, l.offset);
     if (s < 0.0 || s > r.L) return -1;
-    const int ix = sample_voxel(r.p1[0], r.u[0], s, P.o[0], P.v[0], P.iv[0], P.n[0]);
-    const int iy = sample_voxel(r.p1[1], r.u[1], s, P.o[1], P.v[1], P.iv[1], P.n[1]);
-    const int iz = sample_voxel(r.p1[2], r.u[2], s, P.o[2], P.v[2], P.iv[2], P.n[2]);
+    const int ix = sample_voxel_fast(P, r, 0, l.offset_f, s);
+    const int iy = sample_voxel_fast(P, r, 1, l.offset_f, s);
+    const int iz = sample_voxel_fast(P, r, 2, l.offset_f, s);
     if ((ix | iy | iz) < 0) return -1;
     return (iz * P.n[1] + iy) * P.n[0] + ix;
 }
@@ -79,9 +111,10 @@ __global__ void __launch_bounds__(kBlock) sampled_forward_kernel(ProjParams P, c
     SampledRay r;
     float acc = 0.0f;
     if (sampled_setup(ev, e, r)) {
+        sampled_fast_setup(P, r);
         for (int k = 0; k < K; ++k) {
             const SampleLutEntry s = lut[k];
-            const int j = sample_index(P, r, s.offset);
+            const int j = sample_index(P, r, s);
             if (j >= 0) acc = fmaf(s.weight, __ldg(image + j), acc);
         }
     }
@@ -97,32 +130,34 @@ __global__ void __launch_bounds__(kBlock) sampled_backproject_kernel(ProjParams 
     if (e >= n) return;
     SampledRay r;
     if (!sampled_setup(ev, e, r)) return;
+    sampled_fast_setup(P, r);
     const float val = values ? __ldg(values + e) : 1.0f;
     if (val == 0.0f) return;
     for (int k = 0; k < K; ++k) {
         const SampleLutEntry s = lut[k];
-        const int j = sample_index(P, r, s.offset);
+        const int j = sample_index(P, r, s);
         if (j >= 0) atomicAdd(out + j, s.weight * val);
     }
 }
 
-// Fused EM pass: pass 1 gathers (the forward value stays in a register), pass 2 recomputes the sample voxels and
-// scatters evw * w_k / fwd.  Consecutive samples of one event often fall into the same voxel (the sample spacing
-// 6 sigma/(K-1) = 3.7 mm at 300 ps, K = 32 is about one 3.75 mm voxel): equal neighbours are merged into one
+// Fused EM pass of one event: pass 1 gathers (the forward value stays in a register), pass 2 recomputes the sample
+// voxels and scatters evw * w_k / fwd.  Consecutive samples of one event often fall into the same voxel (the sample
+// spacing 6 sigma/(K-1) = 3.7 mm at 300 ps, K = 32 is about one 3.75 mm voxel): equal neighbours are merged into one
 // reduction.
-__global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const SampleLutEntry *__restrict__ lut, int K,
-                                                            EventPtrs ev, uint64_t n, const float *__restrict__ evw,
-                                                            const float *__restrict__ image, float *__restrict__ corr,
-                                                            DeviceStats *stats) {
-    const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+__device__ __forceinline__ void sampled_em_event(const ProjParams &P, const SampleLutEntry *__restrict__ lut, int K,
+                                                 const EventPtrs &ev, uint64_t e, uint64_t n,
+                                                 const float *__restrict__ evw, const float *__restrict__ image,
+                                                 float *__restrict__ corr, unsigned &visits, unsigned &reds,
+                                                 bool &valid) {
     SampledRay r;
-    bool valid = false;
-    unsigned visits = 0, reds = 0;
+    valid = false;
+    visits = reds = 0;
     if (e < n && sampled_setup(ev, e, r)) {
+        sampled_fast_setup(P, r);
         float acc = 0.0f;
         for (int k = 0; k < K; ++k) {
             const SampleLutEntry s = lut[k];
-            const int j = sample_index(P, r, s.offset);
+            const int j = sample_index(P, r, s);
             if (j >= 0) {
                 acc = fmaf(s.weight, __ldg(image + j), acc);
                 ++visits;
@@ -135,7 +170,7 @@ __global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const 
             float pw = 0.0f;
             for (int k = 0; k < K; ++k) {
                 const SampleLutEntry s = lut[k];
-                const int j = sample_index(P, r, s.offset);
+                const int j = sample_index(P, r, s);
                 if (j < 0) continue;
                 if (j != pend) {
                     if (pend >= 0) {
@@ -153,10 +188,42 @@ __global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const 
             }
         }
     }
-    const unsigned nv = __popc(__ballot_sync(0xffffffffu, valid));
-    const unsigned vis = __reduce_add_sync(0xffffffffu, visits);
-    const unsigned nr = __reduce_add_sync(0xffffffffu, reds);
-    if ((threadIdx.x & 31) == 0 && stats) {
+}
+
+// Persistent scheduling as in projector.cu's em_persistent_kernel: the (locality-binned) list is cut into one segment
+// per SM, every warp takes 32-event chunks from the queue of the SM it runs on and steals from other segments when
+// its own is exhausted, so that co-resident warps share L1 while different SMs reduce into different parts of the
+// volume.
+__global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const SampleLutEntry *__restrict__ lut, int K,
+                                                            EventPtrs ev, uint64_t n, const float *__restrict__ evw,
+                                                            const float *__restrict__ image, float *__restrict__ corr,
+                                                            DeviceStats *stats, unsigned *queues, unsigned nseg,
+                                                            unsigned per_seg) {
+    unsigned smid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    const unsigned lane = threadIdx.x & 31u;
+    unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0, nr = 0;
+    while (true) {
+        unsigned c = per_seg;
+        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= per_seg) {
+            if (++tries >= nseg) break;
+            seg = (seg + 61u) % nseg;
+            continue;
+        }
+        unsigned visits, reds;
+        bool valid;
+        sampled_em_event(P, lut, K, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, visits, reds,
+                         valid);
+        nv += valid;
+        vis += visits;
+        nr += reds;
+    }
+    nv = __reduce_add_sync(0xffffffffu, nv);
+    vis = __reduce_add_sync(0xffffffffu, vis);
+    nr = __reduce_add_sync(0xffffffffu, nr);
+    if (lane == 0 && stats) {
         if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
         if (vis) atomicAdd(&stats->visits, (unsigned long long)vis);
         if (nr) atomicAdd(&stats->reds, (unsigned long long)nr);
@@ -178,8 +245,24 @@ void launch_sampled_backproject(const ProjParams &p, const SampleLutEntry *lut, 
 }
 
 void launch_sampled_em(const ProjParams &p, const SampleLutEntry *lut, int K, const EventPtrs &ev, uint64_t n,
-                       const float *evw, const float *image, float *corr, DeviceStats *stats, cudaStream_t s) {
-    if (n) sampled_em_kernel<<<grid_for(n), kBlock, 0, s>>>(p, lut, K, ev, n, evw, image, corr, stats);
+                       const float *evw, const float *image, float *corr, DeviceStats *stats, unsigned *queues,
+                       cudaStream_t s) {
+    if (!n) return;
+    static int n_sm = 0, per_sm = 0;  // one device per process
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sampled_em_kernel, kBlock, 0);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    unsigned nseg = (unsigned)n_sm;
+    if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
+    if (nseg % 61u == 0) nseg -= 1;
+    const uint64_t wchunks = (n + 31) / 32;
+    const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
+    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    sampled_em_kernel<<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, lut, K, ev, n, evw, image, corr, stats,
+                                                                        queues, nseg, per_seg);
 }
 
 }  // namespace tofmlem
