@@ -343,6 +343,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-bin", action="store_true", help="skip locality binning (for comparison)")
     ap.add_argument("--subbins", type=int, default=0, help="TOFMLEM_OPT_SUBBINS override (0 = library default)")
+    ap.add_argument("--em-variant", type=int, default=-1, help="TOFMLEM_OPT_EM_VARIANT override (-1 = library default)")
+    ap.add_argument("--cache-share", type=int, default=-1, help="TOFMLEM_OPT_CACHE_SHARE override")
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next"],
                     help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
                          "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
@@ -377,6 +379,10 @@ def main():
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
     if args.subbins:
         ctx.set_option(pkg.OPT_SUBBINS, args.subbins)
+    if args.em_variant >= 0:
+        ctx.set_option(pkg.OPT_EM_VARIANT, args.em_variant)
+    if args.cache_share >= 0:
+        ctx.set_option(pkg.OPT_CACHE_SHARE, args.cache_share)
     nvox = g.nvox
 
     def timed(fn):

@@ -78,10 +78,14 @@ enum {
     TOFMLEM_OPT_SAMPLES_K = 5,      /* K of the sampled projector, default 32 */
     TOFMLEM_OPT_SHELL_MM = 6,       /* extra shell added to the region margin, default 6 mm */
     TOFMLEM_OPT_EM_VARIANT = 8,     /* fused EM pass scheduling (performance only): 0 = persistent kernel with one work
-                                       queue per SM (default), 1 = one CTA per 256-event chunk in grid order */
+                                       queue per SM (default), 1 = one CTA per 256-event chunk in grid order, 2 = one
+                                       1024-thread CTA per SM whose warps reduce partly through a shared-memory
+                                       write-back cache (see TOFMLEM_OPT_CACHE_SHARE) */
     TOFMLEM_OPT_CTA_INTERLEAVE = 7, /* scatter kernels: number of list segments advanced in parallel (default 64;
                                        1 = natural order).  Performance only, results are the same up to the
                                        order of the float32 reductions. */
+    TOFMLEM_OPT_CACHE_SHARE = 11,   /* EM variant 2 (performance only): how many warps of every 8 reduce through the
+                                       shared-memory write-back cache (0..8); the others reduce at L2 directly */
     TOFMLEM_OPT_MEDIAN = 10,        /* 1: tofmlem_iterate applies the 3x3x3 median filter to the image estimate after
                                        every update (R23); default 0 */
     TOFMLEM_OPT_SUBBINS = 9         /* tofmlem_bin_events: order the events INSIDE each locality bin by predicted

@@ -23,6 +23,7 @@ struct tofmlem_ctx {
     float *d_corr = nullptr;  // padded to whole groups of 4 voxels
     unsigned cta_interleave = 64;
     int em_variant = 0;
+    int cache_share = 4;
     float *d_max = nullptr;          // max(sens) of the current iterate call
     const float *d_max_ext = nullptr;  // region sub-contexts use the parent's global max
     DeviceStats *d_stats = nullptr;
@@ -102,6 +103,7 @@ ProjParams make_params(const tofmlem_ctx *c, bool tof) {
     }
     p.stride = c->cta_interleave;
     p.variant = c->em_variant;
+    p.cache_share = c->cache_share;
     return p;
 }
 
@@ -341,8 +343,12 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             ctx->cta_interleave = (unsigned)value;
             return TOFMLEM_OK;
         case TOFMLEM_OPT_EM_VARIANT:
-            if (value < 0 || value > 1 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "em_variant in 0..1");
+            if (value < 0 || value > 2 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "em_variant in 0..2");
             ctx->em_variant = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_CACHE_SHARE:
+            if (value < 0 || value > 8 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "cache_share in 0..8");
+            ctx->cache_share = (int)value;
             return TOFMLEM_OK;
         case TOFMLEM_OPT_MEDIAN:
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "median is 0 or 1");

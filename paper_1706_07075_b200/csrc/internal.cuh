@@ -21,7 +21,8 @@ struct ProjParams {
     float gauss_a;         // -log2(e) / (2 sigma^2): weight = l * 2^(gauss_a * t^2)
     float gauss_norm;      // 1 / (sigma sqrt(2 pi))
     unsigned stride;       // CTA interleave of the scatter kernels (<= 1: natural order)
-    int variant;           // fused EM pass: 0 = persistent per-SM queues (default), 1 = grid order
+    int variant;           // fused EM pass: 0 = persistent per-SM queues (default), 1 = grid order, 2 = smem cache
+    int cache_share;       // variant 2: warps (of every 8) that reduce through the shared-memory cache
 };
 
 struct EventPtrs {

@@ -384,6 +384,122 @@ __global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, Eve
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Variant 2 of the fused pass: the reductions go through a software WRITE-BACK CACHE in shared memory.
+// ncu (profiles/r02_*): after the sub-bin ordering the pass is bound by the request rate of the L2 atomic units (tag
+// requests 77 % on average, 92 % on the busiest slice) with the issue slots 64 % busy.  The 1024 events in flight on
+// an SM come from one or two locality bins, so they hit the same few thousand voxels over and over: a direct-mapped
+// table of (voxel index, partial sum) pairs, 8 bytes each, updated with one 64-bit compare-and-swap, absorbs the
+// repeats; only an entry that is displaced (or left at the end) costs a reduction at L2.
+constexpr int kCacheLog2 = 14;  // 16384 entries = 128 KB of the SM's shared memory
+constexpr unsigned kCacheEmpty = 0xFFFFFFFFu;
+constexpr int kCachedBlock = 1024;
+
+__device__ __forceinline__ int cache_add(unsigned long long *cache, float *__restrict__ out, int at, float val) {
+    unsigned long long *slot = cache + (at & ((1 << kCacheLog2) - 1));
+    unsigned long long old = *slot;
+    while (true) {
+        const unsigned tag = (unsigned)(old >> 32);
+        const float cur = __uint_as_float((unsigned)old);
+        const float sum = tag == (unsigned)at ? cur + val : val;
+        const unsigned long long upd = ((unsigned long long)(unsigned)at << 32) | __float_as_uint(sum);
+        const unsigned long long prev = atomicCAS(slot, old, upd);
+        if (prev == old) {
+            if (tag != (unsigned)at && tag != kCacheEmpty) {  // displaced entry: write it back
+                atomicAdd(out + tag, cur);
+                return 1;
+            }
+            return 0;
+        }
+        old = prev;
+    }
+}
+
+template <bool TOF>
+__global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P, EventPtrs ev, uint64_t n,
+                                                                    const float *__restrict__ evw,
+                                                                    const float *__restrict__ image,
+                                                                    float *__restrict__ corr, DeviceStats *stats,
+                                                                    unsigned *queues, unsigned nseg, unsigned per_seg) {
+    extern __shared__ unsigned long long cache[];
+    for (int i = threadIdx.x; i < (1 << kCacheLog2); i += kCachedBlock) cache[i] = (unsigned long long)kCacheEmpty << 32;
+    __syncthreads();
+    const unsigned lane = threadIdx.x & 31u;
+    // the shared-memory atomics and the L2 atomic units are two separate pipes: `cache_share` of every 8 warps reduce
+    // through the cache, the others send their 16-byte reductions straight to L2, so that both pipes work in parallel
+    const bool use_cache = ((threadIdx.x >> 5) & 7u) < (unsigned)P.cache_share;
+    unsigned seg = blockIdx.x % nseg, tries = 0, nv = 0, vis = 0, nr = 0;
+    while (true) {
+        unsigned c = per_seg;
+        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= per_seg) {
+            if (++tries >= nseg) break;
+            seg = (seg + 61u) % nseg;
+            continue;
+        }
+        const uint64_t e = ((uint64_t)seg * per_seg + c) * 32u + lane;
+        Ray r;
+        int layout;
+        if (e < n && load_and_setup<TOF, false>(P, ev, e, r, layout)) {
+            int visits;
+            const float acc = ray_gather<TOF>(P, r, image, visits);
+            vis += visits;
+            if (acc > 0.0f) {  // R9
+                ++nv;
+                const float scale = (evw ? __ldg(evw + e) : 1.0f) / acc;
+                if (use_cache) {
+                    Walker<TOF> wk(r);
+                    int at;
+                    bool done;
+                    do {
+                        const float w = wk.step(P, r, at, done);
+                        nr += cache_add(cache, corr, at, w * scale);
+                    } while (!done);
+                } else {
+                    nr += ray_scatter<TOF, true>(P, r, corr, scale);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < (1 << kCacheLog2); i += kCachedBlock) {
+        const unsigned long long v = cache[i];
+        if ((unsigned)(v >> 32) != kCacheEmpty) {
+            atomicAdd(corr + (unsigned)(v >> 32), __uint_as_float((unsigned)v));
+            ++nr;
+        }
+    }
+    nv = __reduce_add_sync(0xffffffffu, nv);
+    vis = __reduce_add_sync(0xffffffffu, vis);
+    nr = __reduce_add_sync(0xffffffffu, nr);
+    if (lane == 0 && stats) {
+        if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
+        if (vis) atomicAdd(&stats->visits, (unsigned long long)vis);
+        if (nr) atomicAdd(&stats->reds, (unsigned long long)nr);
+    }
+}
+
+template <bool TOF>
+static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
+                             float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
+    static int n_sm = 0;
+    const size_t smem = sizeof(unsigned long long) << kCacheLog2;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        cudaFuncSetAttribute(em_cached_kernel<TOF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    }
+    unsigned nseg = (unsigned)n_sm;
+    if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
+    if (nseg % 61u == 0) nseg -= 1;
+    const uint64_t wchunks = (n + 31) / 32;
+    const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
+    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    em_cached_kernel<TOF><<<n_sm, kCachedBlock, smem, s>>>(p, ev, n, evw, image, corr, stats, queues, nseg, per_seg);
+}
+
 static inline unsigned grid_for(uint64_t n, unsigned stride) {
     const unsigned nb = (unsigned)((n + kBlock - 1) / kBlock);
     if (stride <= 1) return nb;
@@ -444,6 +560,13 @@ void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, ui
                           const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,
                           cudaStream_t s) {
     if (n == 0) return;
+    if (p.variant == 2 && queues && vec_ok) {
+        if (tof)
+            launch_em_cached<true>(p, ev, n, evw, image, corr, stats, queues, s);
+        else
+            launch_em_cached<false>(p, ev, n, evw, image, corr, stats, queues, s);
+        return;
+    }
     if (tof) {
         if (vec_ok)
             launch_em<true, true>(p, ev, n, evw, image, corr, stats, queues, s);

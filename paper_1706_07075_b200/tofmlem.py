@@ -22,6 +22,7 @@ OPT_CTA_INTERLEAVE = 7
 OPT_EM_VARIANT = 8
 OPT_SUBBINS = 9
 OPT_MEDIAN = 10
+OPT_CACHE_SHARE = 11
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)

@@ -228,3 +228,21 @@ def test_subbins_keep_keys_offsets_membership(pkg, subbins):
     assert np.all(np.diff(sorted_keys.astype(np.int64)) >= 0)  # sorted by key, invalid (0xFFFFFFFF) last
     ref_offs = np.searchsorted(sorted_keys, np.arange(nb + 1, dtype=np.uint64), side="left")
     assert np.array_equal(offs.cpu().numpy().view(np.uint32).astype(np.int64), ref_offs)
+
+
+# ------------------------------------------------------------------ scheduling variants of the fused EM pass
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_em_variants_parity(pkg, tiny, variant):
+    """TOFMLEM_OPT_EM_VARIANT changes scheduling / accumulation only: same image within the north_star tolerance."""
+    cfg, n, ev, ev_np, g, og, sens = tiny
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ctx.set_option(pkg.OPT_EM_VARIANT, variant)
+    sens_np = sens.cpu().numpy()
+    mask = oracle.mask_f32(sens_np)
+    img = torch.from_numpy(mask.astype(np.float32)).cuda()
+    ctx.iterate(ev, n, img, sens, 2)
+    st = ctx.get_stats()
+    ref, ost = oracle.mlem(og, oracle.sigma_mm(cfg.tof_fwhm_ps), ev_np, mask.astype(np.float64), sens_np, 2)
+    check_image(img.cpu().numpy(), ref)
+    assert st.n_valid == ost.n_valid and st.visits == ost.visits
+    assert abs(st.sum_image_sens - st.n_valid) <= 1e-4 * st.n_valid  # P7
