@@ -151,7 +151,7 @@ def run_report(args):
         key = torch.empty(n, dtype=torch.int32, device=dev)
         perm = torch.empty(n, dtype=torch.int32, device=dev)
         sev = {k: torch.empty_like(v) for k, v in ev.items()}
-        ms = timed(lambda: (ctx.bin_events(ev, n, key, perm, None), ctx.gather_events(ev, perm, n, sev)))
+        ms = timed(lambda: (ctx.bin_events(ev, n, key, perm, None), ctx.permute_events(ev, perm, n, sev)))
         return sev, perm, ms
 
     full = synth.FULL
@@ -409,7 +409,7 @@ def main():
 
         def do_bin():
             ctx.bin_events(ev, n, key, perm, None)
-            ctx.gather_events(ev, perm, n, sev)
+            ctx.permute_events(ev, perm, n, sev)
 
         bin_ms = timed(do_bin)
         n_valid_keys = int((key != -1).sum().item())

@@ -150,9 +150,15 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_events, uint6
 int tofmlem_bin_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, uint32_t *d_key, uint32_t *d_perm,
                        uint32_t *d_bin_offsets);
 uint32_t tofmlem_num_bins(const tofmlem_ctx *ctx);
-/* out[i] = in[d_perm[i]] for every member (dt skipped if either dt pointer is NULL).  in/out must not alias. */
+/* out[i] = in[d_perm[i]], i < n, for every member (dt skipped if either dt pointer is NULL).  in/out must not alias.
+ * tofmlem_gather_events accepts any index list (e.g. the kept events of tofmlem_scatter_reject, whose indices exceed
+ * n); tofmlem_permute_events REQUIRES d_perm to be a permutation of 0..n-1 (what tofmlem_bin_events and
+ * tofmlem_split_regions produce) and is 4x faster: it interleaves the members into 32-byte records first, in scratch
+ * of 32 B per event that the context keeps until tofmlem_destroy. */
 int tofmlem_gather_events(tofmlem_ctx *ctx, const tofmlem_events *in, const uint32_t *d_perm, uint64_t n,
                           const tofmlem_events_mut *out);
+int tofmlem_permute_events(tofmlem_ctx *ctx, const tofmlem_events *in, const uint32_t *d_perm, uint64_t n,
+                           const tofmlem_events_mut *out);
 
 /* TOF-assisted data division (R12, R13): d_region[e] = #{ j in 1..R-1 : zb[j] <= cz_e } with
  * cz_e the z of the TOF kernel centre (float32, F1); invalid events get -1.  h_zbounds: n_regions+1 ascending

@@ -85,6 +85,9 @@ void launch_scatter_perm(const uint32_t *key, const uint8_t *sub, uint32_t S, ui
                          uint32_t *cursor, uint32_t *perm, cudaStream_t s);
 void launch_strided_copy(const uint32_t *fine, uint32_t S, uint32_t count, uint32_t *out, cudaStream_t s);
 void launch_gather(const float *in, const uint32_t *perm, uint64_t n, float *out, cudaStream_t s);
+// all members at once through 32-byte records; rec: 8 n floats of scratch (16-byte aligned); out[6] may be NULL
+void launch_gather_packed(const EventPtrs &in, const uint32_t *perm, uint64_t n, float *rec, float *const out[7],
+                          cudaStream_t s);
 constexpr int kMaxRegions = 64;
 struct RegionBounds {
     float zb[kMaxRegions + 1];

@@ -33,7 +33,7 @@ SYMBOLS = (
     "tofmlem_split_regions", "tofmlem_region_zbounds", "tofmlem_region_grid", "tofmlem_reconstruct_regions",
     "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
     "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
-    "tofmlem_gather_f32", "tofmlem_scatter_reject",
+    "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events",
 )
 
 
@@ -207,6 +207,12 @@ class Context:
         a, b = _events(ev, n), _events(out, n)
         self._check(self._L.tofmlem_gather_events(self._h, C.byref(a), C.c_void_p(_ptr(perm, torch.int32, "cuda", n)),
                                                   C.c_uint64(n), C.byref(b)))
+
+    def permute_events(self, ev, perm: torch.Tensor, n: int, out):
+        """gather_events for a perm that is a permutation of 0..n-1 (bin_events / split_regions): packed fast path"""
+        a, b = _events(ev, n), _events(out, n)
+        self._check(self._L.tofmlem_permute_events(self._h, C.byref(a), C.c_void_p(_ptr(perm, torch.int32, "cuda", n)),
+                                                   C.c_uint64(n), C.byref(b)))
 
     def region_zbounds(self, n_regions: int = 9) -> torch.Tensor:
         zb = torch.empty(n_regions + 1, dtype=torch.float32)

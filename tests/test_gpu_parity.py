@@ -338,6 +338,11 @@ def test_bin_events_bit_exact(pkg, cfg_name, n):
     for k in synth.EVENT_FIELDS:
         a, b = out[k].cpu().numpy(), ev_np[k][p]
         assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+    # the packed fast path for full permutations gives the same bits
+    out2 = {k: torch.zeros_like(v) for k, v in ev.items()}
+    ctx.permute_events(ev, perm, n, out2)
+    for k in synth.EVENT_FIELDS:
+        assert torch.equal(out[k].view(torch.int32), out2[k].view(torch.int32))
 
 
 def test_split_regions_bit_exact(pkg):

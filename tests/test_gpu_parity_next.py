@@ -163,7 +163,7 @@ def test_attenuation_weights_and_weighted_iterate(pkg):
     perm = torch.empty(n, dtype=torch.int32, device="cuda")
     ctx.bin_events(ev, n, key, perm, None)
     sev = {k: torch.empty_like(v) for k, v in ev.items()}
-    ctx.gather_events(ev, perm, n, sev)
+    ctx.permute_events(ev, perm, n, sev)
     sw = torch.empty_like(w)
     ctx.gather_f32(w, perm, n, sw)
     img2 = torch.from_numpy(mask.astype(np.float32)).cuda()
@@ -197,6 +197,12 @@ def test_scatter_reject_bit_exact(pkg, cfg_name, n):
     assert not ref_keep[[5, 17, 29]].any()
     got_idx = np.sort(perm[:kept].cpu().numpy().astype(np.int64))
     assert np.array_equal(got_idx, np.nonzero(ref_keep)[0])
+    # compaction: gather_events takes the kept indices (a subset whose indices exceed the output length)
+    out = {k: torch.empty(kept, dtype=torch.float32, device="cuda") for k in ev}
+    ctx.gather_events(ev, perm, kept, out)
+    order = perm[:kept].cpu().numpy().astype(np.int64)
+    for k in synth.EVENT_FIELDS:
+        assert np.array_equal(out[k].cpu().numpy().view(np.uint32), ev_np[k][order].view(np.uint32))
     # default half width (<= 0) = 1.959964 sigma rounded to float32: the same flags
     keep2 = torch.empty_like(keep)
     assert ctx.scatter_reject(ev, n, torch.from_numpy(ell), 0.0, keep2, None) == ref_cnt
