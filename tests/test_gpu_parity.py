@@ -430,3 +430,65 @@ def test_reconstruct_regions_parity(pkg):
     ctx.iterate(ev, n, x, sens, iters)
     d = (out - x).double().norm() / x.double().norm()
     print(f"split-vs-unsplit rel-L2 = {d.item():.3e} (no threshold: parity unpinned)")
+
+
+def test_full_size_bench_configuration(pkg):
+    """BASELINE.json cfg-3 at FULL size (146 M events, 160x160x640) in the launch configuration bench.py times
+    (sub-binned permutation, persistent fused EM pass, update).  The oracle cannot run 146 M events, so:
+      - sampled outputs it CAN compute one by one: forward values of every 1000th event of the full set, rel <= 1e-4;
+      - properties that hold at any size: the binned pass and the unbinned pass give the same correction image up to
+        the float32 summation order; sum(sens * x) = n_valid after the iteration (P7); n_valid = #{fwd > 0};
+        the permutation is a bijection that sorts the keys."""
+    cfg = synth.FULL
+    n = cfg.n_events
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40e9:
+        pytest.skip("needs 40 GB of free device memory")
+    g, og = grids(pkg, cfg)
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ev = synth.make_events_chunked(cfg, n, device="cuda")
+    img = synth.random_image((g.nvox,), 41, device="cuda")
+    # sampled forward values against the oracle
+    fwd = torch.empty(n, dtype=torch.float32, device="cuda")
+    ctx.forward(ev, n, img, fwd)
+    sub = {k: v[::1000].contiguous() for k, v in ev.items()}
+    ref = oracle.forward(og, oracle.sigma_mm(cfg.tof_fwhm_ps), to_np(sub), img.cpu().numpy())
+    err = fwd_rel_err(fwd[::1000].cpu().numpy(), ref)
+    assert err.max() <= FWD_RTOL, err.max()
+    n_pos = int((fwd > 0).sum().item())
+    del fwd
+    # unbinned pass (grid-order kernel on the raw order) vs binned pass (persistent kernel on the permuted set)
+    corr_a = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.set_option(pkg.OPT_EM_VARIANT, 1)
+    ctx.reset_stats()
+    ctx.em_correction(ev, n, img, corr_a)
+    st_a = ctx.get_stats()
+    key = torch.empty(n, dtype=torch.int32, device="cuda")
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    ctx.bin_events(ev, n, key, perm, None)
+    sev = {k: torch.empty_like(v) for k, v in ev.items()}
+    ctx.permute_events(ev, perm, n, sev)
+    skey = key[perm.long()].view(torch.int32)  # sorted as unsigned: compare through int64
+    sk = skey.long() & 0xFFFFFFFF
+    assert bool((sk[1:] >= sk[:-1]).all())
+    del ev, key, skey, sk
+    seen = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    seen[perm.long()] = 1
+    assert int(seen.sum().item()) == n  # a bijection
+    del seen, perm
+    ctx.set_option(pkg.OPT_EM_VARIANT, 0)
+    corr_b = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.reset_stats()
+    ctx.em_correction(sev, n, img, corr_b)
+    st_b = ctx.get_stats()
+    assert st_a.n_valid == st_b.n_valid == n_pos and st_a.visits == st_b.visits
+    d = (corr_a.double() - corr_b.double()).norm() / corr_a.double().norm()
+    assert float(d) <= 1e-5, float(d)
+    big = corr_a > 0.01 * corr_a.max()
+    assert float(((corr_a - corr_b).abs()[big] / corr_a[big]).max()) <= 1e-3
+    # P7 at full size: after the update sum(sens * x) = n_valid (sens = any positive image; mask = all voxels)
+    sens = torch.full((g.nvox,), 0.25, dtype=torch.float32, device="cuda")
+    ctx.update(img, corr_b, sens)
+    p7 = float((img.double() * sens.double()).sum().item())
+    # sum_j x_j corr_j = n_valid holds for the image the pass was run on: rel 1e-5 covers float32 products
+    assert abs(p7 - st_b.n_valid) <= 1e-5 * st_b.n_valid, (p7, st_b.n_valid)
