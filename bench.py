@@ -533,7 +533,7 @@ def main():
             c_ref, nv_ref, vis_ref = oracle.em_correction(og, oracle.sigma_mm(cfg.tof_fwhm_ps), sub, x)
             oracle.update(x.copy(), c_ref, sens_np, ones)
             dt = time.perf_counter() - tt
-            ns2 = min(max(n // 4, 1), int(ns * args.cpu_seconds / max(dt, 1e-3)))
+            ns2 = min(n, int(ns * args.cpu_seconds / max(dt, 1e-3)))
             if attempt == 2 or ns2 <= 1.5 * ns:
                 break
             ns = ns2
