@@ -84,6 +84,15 @@ enum {
     TOFMLEM_OPT_CTA_INTERLEAVE = 7, /* scatter kernels: number of list segments advanced in parallel (default 64;
                                        1 = natural order).  Performance only, results are the same up to the
                                        order of the float32 reductions. */
+    TOFMLEM_OPT_CORR_BRICKS = 12,   /* 1 (default): correction images of the fused pass are kept in the context's internal
+                                       order (2x2x1-voxel bricks per 16 bytes: 11 % fewer reductions at L2).  This
+                                       concerns d_corr of tofmlem_em_correction[_weighted] and tofmlem_update: between
+                                       those calls it may be zeroed, copied, or summed element-wise with the d_corr of
+                                       an equally configured context (multi-GPU), but not read as an image.  0: d_corr
+                                       is a plain image (x fastest).  Applies when nx and ny are even, the Siddon
+                                       projector is selected and d_corr is 16-byte aligned;
+                                       otherwise d_corr is a plain image anyway.  Do not change options between a pass
+                                       and its update. */
     TOFMLEM_OPT_CACHE_SHARE = 11,   /* EM variant 2 (performance only): how many warps of every 8 reduce through the
                                        shared-memory write-back cache (0..8); the others reduce at L2 directly */
     TOFMLEM_OPT_MEDIAN = 10,        /* 1: tofmlem_iterate applies the 3x3x3 median filter to the image estimate after

@@ -24,6 +24,7 @@ struct tofmlem_ctx {
     unsigned cta_interleave = 64;
     int em_variant = 0;
     int cache_share = 4;
+    int corr_bricks = 1;  // correction images of the fused pass in the 2x2x1 brick layout (TOFMLEM_OPT_CORR_BRICKS)
     float *d_max = nullptr;          // max(sens) of the current iterate call
     const float *d_max_ext = nullptr;  // region sub-contexts use the parent's global max
     DeviceStats *d_stats = nullptr;
@@ -106,12 +107,26 @@ ProjParams make_params(const tofmlem_ctx *c, bool tof) {
     p.stride = c->cta_interleave;
     p.variant = c->em_variant;
     p.cache_share = c->cache_share;
+    p.brick = 0;
     return p;
 }
 
 // 16-byte vector reductions need an aligned array made of whole groups of 4 voxels
 bool vec_ok(const tofmlem_ctx *c, const float *out) {
     return (c->nvox & 3) == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+}
+
+// Is the correction image `corr` of this context's fused pass / update in the brick layout?  Depends only on the
+// context's options and the pointer, so tofmlem_em_correction and tofmlem_update agree without further state.
+bool bricks_on(const tofmlem_ctx *c, const float *corr) {
+    return c->corr_bricks && c->projector == 0 && (c->grid.nx & 1) == 0 && (c->grid.ny & 1) == 0 && vec_ok(c, corr);
+}
+
+void update_any(const tofmlem_ctx *c, float *image, float *corr, const float *sens, const float *dmax, cudaStream_t s) {
+    if (bricks_on(c, corr))
+        launch_update_brick(image, corr, sens, dmax, (float)c->sens_floor_rel, c->grid.nx, c->grid.ny, c->grid.nz, s);
+    else
+        launch_update(image, corr, sens, dmax, (float)c->sens_floor_rel, c->nvox, s);
 }
 
 EventPtrs ev_ptrs(const tofmlem_events *e, uint64_t off = 0) {
@@ -192,9 +207,11 @@ int ensure_lut(tofmlem_ctx *ctx) {
 }
 
 // One fused EM pass with the context's projector (0 = Siddon x Gaussian, 1 = K-sample kernel).
-int em_pass(tofmlem_ctx *ctx, const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw,
+int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint64_t n, const float *evw,
             const float *d_image, float *d_corr, bool vec, cudaStream_t s) {
     if (n == 0) return TOFMLEM_OK;
+    ProjParams p = p_in;
+    p.brick = bricks_on(ctx, d_corr) ? 1 : 0;
     if (ctx->projector == 1) {
         int rc = ensure_lut(ctx);
         if (rc) return rc;
@@ -229,7 +246,7 @@ int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, const floa
         CU(cudaMemsetAsync(ctx->d_stats, 0, 3 * sizeof(unsigned long long), ctx->stream));
         rc = em_pass(ctx, p, ev, n, evw, d_image, ctx->d_corr, true, ctx->stream);
         if (rc) return rc;
-        launch_update(d_image, ctx->d_corr, d_sens, dmax, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
+        update_any(ctx, d_image, ctx->d_corr, d_sens, dmax, ctx->stream);
         CHECK_LAUNCH(1);
         if (ctx->median) {  // the filter is applied to the image estimate after each iteration (R23)
             rc = median_in_place(ctx, d_image, ctx->stream);
@@ -349,6 +366,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             if (value < 0 || value > 2 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "em_variant in 0..2");
             ctx->em_variant = (int)value;
             return TOFMLEM_OK;
+        case TOFMLEM_OPT_CORR_BRICKS:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "corr_bricks is 0 or 1");
+            ctx->corr_bricks = (int)value;
+            return TOFMLEM_OK;
         case TOFMLEM_OPT_CACHE_SHARE:
             if (value < 0 || value > 8 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "cache_share in 0..8");
             ctx->cache_share = (int)value;
@@ -443,7 +464,7 @@ int tofmlem_update(tofmlem_ctx *ctx, float *d_image, float *d_corr, const float 
     if (!d_image || !d_corr || !d_sens) return fail(ctx, TOFMLEM_EINVAL, "update: NULL argument");
     launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, ctx->stream);
     CHECK_LAUNCH(1);
-    launch_update(d_image, d_corr, d_sens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, ctx->stream);
+    update_any(ctx, d_image, d_corr, d_sens, ctx->d_max, ctx->stream);
     CHECK_LAUNCH(1);
     return TOFMLEM_OK;
 }
@@ -571,20 +592,20 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
             rc = em_pass(ctx, p, ev_ptrs(&dev, off), m, nullptr, ctx->d_himg, ctx->d_corr, true, s);
             if (rc) return rc;
         }
-        launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
+        update_any(ctx, ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, s);
         CHECK_LAUNCH(1);
         if (ctx->median && (rc = median_in_place(ctx, ctx->d_himg, s))) return rc;
         for (int it = 1; it < iters; ++it) {
             CU(cudaMemsetAsync(ctx->d_stats, 0, 3 * sizeof(unsigned long long), s));
             rc = em_pass(ctx, p, ev_ptrs(&dev), n, nullptr, ctx->d_himg, ctx->d_corr, true, s);
             if (rc) return rc;
-            launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
+            update_any(ctx, ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, s);
             CHECK_LAUNCH(1);
             if (ctx->median && (rc = median_in_place(ctx, ctx->d_himg, s))) return rc;
         }
     } else if (iters > 0) {
         for (int it = 0; it < iters; ++it) {
-            launch_update(ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, (float)ctx->sens_floor_rel, ctx->nvox, s);
+            update_any(ctx, ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, s);
             CHECK_LAUNCH(1);
         }
     }
@@ -860,6 +881,9 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         sc->projector = ctx->projector;
         sc->samples_k = ctx->samples_k;
         sc->median = ctx->median;
+        sc->corr_bricks = ctx->corr_bricks;
+        sc->em_variant = ctx->em_variant;
+        sc->cache_share = ctx->cache_share;
         sc->d_max_ext = ctx->d_max;
         const uint64_t nv = sc->nvox;
         RCU(cudaMalloc(&images[r], nv * sizeof(float)));

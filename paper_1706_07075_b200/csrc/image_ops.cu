@@ -76,6 +76,35 @@ __global__ void __launch_bounds__(kBlock) update_kernel(float *__restrict__ imag
     }
 }
 
+// update with the correction image in the 2x2x1 brick layout (projector.cu, ray_scatter<BRICK>): one thread per
+// brick = one float4 of corr, two float2 of image and of sens.
+__global__ void __launch_bounds__(kBlock) update_brick_kernel(float *__restrict__ image, float *__restrict__ corr,
+                                                              const float *__restrict__ sens,
+                                                              const float *__restrict__ d_max, float floor_rel, int nx,
+                                                              int ny, int nz) {
+    const float thr = __fmul_rn(floor_rel, *d_max);
+    const uint64_t hx = (uint64_t)(nx >> 1), hy = (uint64_t)(ny >> 1);
+    const uint64_t nb = hx * hy * (uint64_t)nz;
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    float4 *cor4 = reinterpret_cast<float4 *>(corr);
+    for (uint64_t b = (uint64_t)blockIdx.x * kBlock + threadIdx.x; b < nb; b += stride) {
+        const uint64_t bx = b % hx, t = b / hx;
+        const uint64_t by = t % hy, z = t / hy;
+        const uint64_t lo = (z * (uint64_t)ny + 2 * by) * (uint64_t)nx + 2 * bx, hi = lo + (uint64_t)nx;
+        const float4 c = cor4[b];
+        float2 x0 = *reinterpret_cast<float2 *>(image + lo), x1 = *reinterpret_cast<float2 *>(image + hi);
+        const float2 s0 = __ldg(reinterpret_cast<const float2 *>(sens + lo));
+        const float2 s1 = __ldg(reinterpret_cast<const float2 *>(sens + hi));
+        x0.x = update_one(x0.x, c.x, s0.x, thr);
+        x0.y = update_one(x0.y, c.y, s0.y, thr);
+        x1.x = update_one(x1.x, c.z, s1.x, thr);
+        x1.y = update_one(x1.y, c.w, s1.y, thr);
+        *reinterpret_cast<float2 *>(image + lo) = x0;
+        *reinterpret_cast<float2 *>(image + hi) = x1;
+        cor4[b] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
 // x0 = mask (the harness' initial image, R15)
 __global__ void __launch_bounds__(kBlock) mask_init_kernel(float *__restrict__ image, const float *__restrict__ sens,
                                                            const float *__restrict__ d_max, float floor_rel,
@@ -199,6 +228,12 @@ __global__ void __launch_bounds__(kBlock) median3_kernel(const float *__restrict
         if (s < 12) v[14] = v[15 + s];                          // forget both, take the next value in
     }
     out[j] = v[13];
+}
+
+void launch_update_brick(float *image, float *corr, const float *sens, const float *d_max, float floor_rel, int nx,
+                         int ny, int nz, cudaStream_t s) {
+    const uint64_t nb = (uint64_t)(nx >> 1) * (ny >> 1) * nz;
+    update_brick_kernel<<<grid_for(nb), kBlock, 0, s>>>(image, corr, sens, d_max, floor_rel, nx, ny, nz);
 }
 
 void launch_median3(const float *in, float *out, int nx, int ny, int nz, cudaStream_t s) {

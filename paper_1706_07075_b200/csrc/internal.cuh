@@ -23,6 +23,7 @@ struct ProjParams {
     unsigned stride;       // CTA interleave of the scatter kernels (<= 1: natural order)
     int variant;           // fused EM pass: 0 = persistent per-SM queues (default), 1 = grid order, 2 = smem cache
     int cache_share;       // variant 2: warps (of every 8) that reduce through the shared-memory cache
+    int brick;             // fused EM pass: the correction image is in the 2x2x1 brick layout (needs even nx, ny)
 };
 
 struct EventPtrs {
@@ -59,6 +60,9 @@ void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, ui
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);
 void launch_update(float *image, float *corr, const float *sens, const float *d_max, float floor_rel, uint64_t n,
                    cudaStream_t s);
+// corr in the brick layout: index = ((z * ny/2 + y/2) * nx/2 + x/2) * 4 + (y & 1) * 2 + (x & 1); nx, ny even
+void launch_update_brick(float *image, float *corr, const float *sens, const float *d_max, float floor_rel, int nx,
+                         int ny, int nz, cudaStream_t s);
 void launch_mask_init(float *image, const float *sens, const float *d_max, float floor_rel, uint64_t n,
                       cudaStream_t s);
 void launch_dot_f64(const float *a, const float *b, uint64_t n, double *d_out /* zeroed by the call */,

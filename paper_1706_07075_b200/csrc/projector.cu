@@ -29,6 +29,10 @@ struct Ray {
     float tdx, tdy, tdz;
     int idx;            // flat index of the first voxel (in the lane's layout)
     int dxi, dyi, dzi;  // flat-index increments of a step along each (permuted) axis, 0 when parallel
+    // brick layout of the correction image (2x2x1 voxels per 16-byte group, see ProjParams::brick):
+    int bidx;        // brick-layout index of the first voxel
+    int bdx0, bdxs;  // x step: increment for the first step, and the sum of the two alternating increments
+    int bdy0, bdys;  // y step: likewise
 };
 
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -149,17 +153,30 @@ __device__ __forceinline__ bool ray_setup(const ProjParams &P, float fx1, float 
     const float ec = axis_setup(z1, uz, s_lo, oC, vC, ivC, nC, nA * nB, ic, r.dzi, r.t0z, r.tdz);
     r.t_end = fminf(fminf((float)(s_hi - s_lo), ea), fminf(eb, ec));
     r.idx = (ic * nB + ib) * nA + ia;
+    if (!LAYOUTS && P.brick) {
+        // index = (brick number) * 4 + (iy & 1) * 2 + (ix & 1): a step in x alternates between +-1 (inside the brick)
+        // and +-3 (into the neighbouring brick), a step in y between +-2 and +-(2 nx - 2); z steps are unchanged
+        r.bidx = ((ic * (nB >> 1) + (ib >> 1)) * (nA >> 1) + (ia >> 1)) * 4 + ((ib & 1) << 1) + (ia & 1);
+        const int xa = r.dxi > 0 ? 1 : (r.dxi < 0 ? -3 : 0), xb = r.dxi > 0 ? 3 : (r.dxi < 0 ? -1 : 0);
+        r.bdx0 = (ia & 1) ? xb : xa;
+        r.bdxs = xa + xb;
+        const int yo = 2 * nA - 2;
+        const int ya = r.dyi > 0 ? 2 : (r.dyi < 0 ? -yo : 0), yb = r.dyi > 0 ? yo : (r.dyi < 0 ? -2 : 0);
+        r.bdy0 = (ib & 1) ? yb : ya;
+        r.bdys = ya + yb;
+    }
     return true;
 }
 
 // Branch-free incremental walk.  step() returns the un-normalised weight of the current clipped chord and its
 // flat voxel index, and advances; `done` is set on the last chord.
-template <bool TOF>
+template <bool TOF, bool BRICK = false>
 struct Walker {
     float tx, ty, tz, kx, ky, kz, t;
-    int idx;
+    int idx, dxc, dyc;
     __device__ __forceinline__ explicit Walker(const Ray &r)
-        : tx(r.t0x), ty(r.t0y), tz(r.t0z), kx(0.f), ky(0.f), kz(0.f), t(0.f), idx(r.idx) {}
+        : tx(r.t0x), ty(r.t0y), tz(r.t0z), kx(0.f), ky(0.f), kz(0.f), t(0.f), idx(BRICK ? r.bidx : r.idx),
+          dxc(BRICK ? r.bdx0 : r.dxi), dyc(BRICK ? r.bdy0 : r.dyi) {}
     __device__ __forceinline__ float step(const ProjParams &P, const Ray &r, int &at, bool &done) {
         const float tn = fminf(fminf(tx, ty), fminf(tz, r.t_end));
         const float l = tn - t;
@@ -170,8 +187,16 @@ struct Walker {
         }
         at = idx;
         done = tn >= r.t_end;
-        if (tx <= tn) { kx += 1.0f; idx += r.dxi; }
-        if (ty <= tn) { ky += 1.0f; idx += r.dyi; }
+        if (tx <= tn) {
+            kx += 1.0f;
+            idx += dxc;
+            if (BRICK) dxc = r.bdxs - dxc;
+        }
+        if (ty <= tn) {
+            ky += 1.0f;
+            idx += dyc;
+            if (BRICK) dyc = r.bdys - dyc;
+        }
         if (tz <= tn) { kz += 1.0f; idx += r.dzi; }
         tx = fmaf(kx, r.tdx, r.t0x);
         ty = fmaf(ky, r.tdy, r.t0y);
@@ -216,15 +241,17 @@ __device__ __forceinline__ float ray_gather(const ProjParams &P, const Ray &r, c
 // out[j] += w_j * scale over the window: float32 reductions at L2, fire and forget.
 // VEC: one 16-byte vector reduction per aligned group of 4 voxels (needs a 16-byte aligned `out` whose
 // allocation covers whole groups); otherwise one scalar reduction per voxel.
-template <bool TOF, bool VEC>
+// BRICK (with VEC): `out` is in the brick layout, whose 16-byte groups are 2x2x1 voxels: a line that meets a group meets
+// 1.50 of its voxels on average against 1.34 for 4x1x1 groups (Cauchy: 4 * 6 / surface), i.e. 11 % fewer reductions.
+template <bool TOF, bool VEC, bool BRICK = false>
 __device__ __forceinline__ int ray_scatter(const ProjParams &P, const Ray &r, float *__restrict__ out, float scale) {
-    Walker<TOF> wk(r);
+    Walker<TOF, BRICK> wk(r);
     int at, reds = 1;
     bool done;
     if (VEC) {
         // The flush is a predicated instruction, not a branch: some lane of a warp flushes in nearly every step
         // (ncu r01b: 97 % of the warp iterations), so a branch only adds its re-convergence overhead.
-        int grp = r.idx >> 2;
+        int grp = (BRICK ? r.bidx : r.idx) >> 2;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
 #pragma unroll 2
         do {
@@ -305,7 +332,7 @@ __global__ void __launch_bounds__(kBlock) backproject_kernel(ProjParams P, Event
 
 // One event of the fused EM pass: walk 1 gathers the image (the forward value stays in a register), walk 2
 // recomputes the weights and scatters w / fwd (the Gaussian normalisation cancels in a_ej / fwd_e).
-template <bool TOF, bool VEC>
+template <bool TOF, bool VEC, bool BRICK>
 __device__ __forceinline__ void em_event(const ProjParams &P, const EventPtrs &ev, uint64_t e, uint64_t n,
                                          const float *__restrict__ evw, const float *__restrict__ image,
                                          float *__restrict__ corr, int &visits, bool &valid, int &reds) {
@@ -319,20 +346,20 @@ __device__ __forceinline__ void em_event(const ProjParams &P, const EventPtrs &e
         if (acc > 0.0f) {  // R9
             valid = true;
             // evw: optional per-event weight (attenuation correction applied to the LOR, R19)
-            reds = ray_scatter<TOF, VEC>(P, r, corr, (evw ? __ldg(evw + e) : 1.0f) / acc);
+            reds = ray_scatter<TOF, VEC, BRICK>(P, r, corr, (evw ? __ldg(evw + e) : 1.0f) / acc);
         }
     }
 }
 
 // Grid-order form: one CTA per 256-event chunk, chunks interleaved (comment (5) at the top).
-template <bool TOF, bool VEC>
+template <bool TOF, bool VEC, bool BRICK>
 __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, EventPtrs ev, uint64_t n,
                                                                const float *__restrict__ evw,
                                                                const float *__restrict__ image,
                                                                float *__restrict__ corr, DeviceStats *stats) {
     int visits, reds;
     bool valid;
-    em_event<TOF, VEC>(P, ev, event_index(P.stride), n, evw, image, corr, visits, valid, reds);
+    em_event<TOF, VEC, BRICK>(P, ev, event_index(P.stride), n, evw, image, corr, visits, valid, reds);
     // per-warp counters -> one atomic per warp
     const unsigned nv = __popc(__ballot_sync(0xffffffffu, valid));
     const unsigned vis = __reduce_add_sync(0xffffffffu, (unsigned)visits);
@@ -350,7 +377,7 @@ __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, Eve
 // CTAs of the grid-order form come from 8 unrelated places and thrash it), while different SMs reduce into different
 // parts of the volume.  A warp whose segment is exhausted moves on to other segments (work stealing; the invalid
 // events sorted to the end of the list make the last segments empty).  Measured at cfg-3: 30.2 -> 25.2 ms.
-template <bool TOF, bool VEC>
+template <bool TOF, bool VEC, bool BRICK>
 __global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, EventPtrs ev, uint64_t n,
                                                                const float *__restrict__ evw,
                                                                const float *__restrict__ image,
@@ -371,7 +398,8 @@ __global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, Eve
         }
         int visits, reds;
         bool valid;
-        em_event<TOF, VEC>(P, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, visits, valid, reds);
+        em_event<TOF, VEC, BRICK>(P, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, visits, valid,
+                                  reds);
         nv += valid;
         vis += visits;
         nr += reds;
@@ -417,7 +445,7 @@ __device__ __forceinline__ int cache_add(unsigned long long *cache, float *__res
     }
 }
 
-template <bool TOF>
+template <bool TOF, bool BRICK>
 __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P, EventPtrs ev, uint64_t n,
                                                                     const float *__restrict__ evw,
                                                                     const float *__restrict__ image,
@@ -451,7 +479,7 @@ __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P
                 ++nv;
                 const float scale = (evw ? __ldg(evw + e) : 1.0f) / acc;
                 if (use_cache) {
-                    Walker<TOF> wk(r);
+                    Walker<TOF, BRICK> wk(r);
                     int at;
                     bool done;
                     do {
@@ -459,7 +487,7 @@ __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P
                         nr += cache_add(cache, corr, at, w * scale);
                     } while (!done);
                 } else {
-                    nr += ray_scatter<TOF, true>(P, r, corr, scale);
+                    nr += ray_scatter<TOF, true, BRICK>(P, r, corr, scale);
                 }
             }
         }
@@ -482,7 +510,7 @@ __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P
     }
 }
 
-template <bool TOF>
+template <bool TOF, bool BRICK>
 static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
                              float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
     static int n_sm = 0;
@@ -491,7 +519,7 @@ static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t 
         int dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(em_cached_kernel<TOF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(em_cached_kernel<TOF, BRICK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     }
     unsigned nseg = (unsigned)n_sm;
     if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
@@ -499,7 +527,8 @@ static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t 
     const uint64_t wchunks = (n + 31) / 32;
     const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
     cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-    em_cached_kernel<TOF><<<n_sm, kCachedBlock, smem, s>>>(p, ev, n, evw, image, corr, stats, queues, nseg, per_seg);
+    em_cached_kernel<TOF, BRICK><<<n_sm, kCachedBlock, smem, s>>>(p, ev, n, evw, image, corr, stats, queues, nseg,
+                                                                 per_seg);
 }
 
 static inline unsigned grid_for(uint64_t n, unsigned stride) {
@@ -534,7 +563,7 @@ void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint
     }
 }
 
-template <bool TOF, bool VEC>
+template <bool TOF, bool VEC, bool BRICK>
 static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
                       float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
     if (p.variant != 1 && queues) {
@@ -542,7 +571,7 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         if (!n_sm) {
             int dev = 0;
             cudaGetDevice(&dev);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_persistent_kernel<TOF, VEC>, kBlock, 0);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
             cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         }
         unsigned nseg = (unsigned)n_sm;
@@ -551,10 +580,10 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         const uint64_t wchunks = (n + 31) / 32;
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
         cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-        em_persistent_kernel<TOF, VEC><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, ev, n, evw, image, corr,
+        em_persistent_kernel<TOF, VEC, BRICK><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, ev, n, evw, image, corr,
                                                                                          stats, queues, nseg, per_seg);
     } else {
-        em_correction_kernel<TOF, VEC><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
+        em_correction_kernel<TOF, VEC, BRICK><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
     }
 }
 
@@ -563,22 +592,36 @@ void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, ui
                           cudaStream_t s) {
     if (n == 0) return;
     if (p.variant == 2 && queues && vec_ok) {
+        if (tof) {
+            if (p.brick)
+                launch_em_cached<true, true>(p, ev, n, evw, image, corr, stats, queues, s);
+            else
+                launch_em_cached<true, false>(p, ev, n, evw, image, corr, stats, queues, s);
+        } else {
+            if (p.brick)
+                launch_em_cached<false, true>(p, ev, n, evw, image, corr, stats, queues, s);
+            else
+                launch_em_cached<false, false>(p, ev, n, evw, image, corr, stats, queues, s);
+        }
+        return;
+    }
+    if (p.brick && vec_ok) {  // the brick layout exists only together with the 16-byte reductions
         if (tof)
-            launch_em_cached<true>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<true, true, true>(p, ev, n, evw, image, corr, stats, queues, s);
         else
-            launch_em_cached<false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<false, true, true>(p, ev, n, evw, image, corr, stats, queues, s);
         return;
     }
     if (tof) {
         if (vec_ok)
-            launch_em<true, true>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<true, true, false>(p, ev, n, evw, image, corr, stats, queues, s);
         else
-            launch_em<true, false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<true, false, false>(p, ev, n, evw, image, corr, stats, queues, s);
     } else {
         if (vec_ok)
-            launch_em<false, true>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<false, true, false>(p, ev, n, evw, image, corr, stats, queues, s);
         else
-            launch_em<false, false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<false, false, false>(p, ev, n, evw, image, corr, stats, queues, s);
     }
 }
 

@@ -23,6 +23,7 @@ OPT_EM_VARIANT = 8
 OPT_SUBBINS = 9
 OPT_MEDIAN = 10
 OPT_CACHE_SHARE = 11
+OPT_CORR_BRICKS = 12
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)

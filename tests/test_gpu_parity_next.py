@@ -252,3 +252,35 @@ def test_em_variants_parity(pkg, tiny, variant):
     check_image(img.cpu().numpy(), ref)
     assert st.n_valid == ost.n_valid and st.visits == ost.visits
     assert abs(st.sum_image_sens - st.n_valid) <= 1e-4 * st.n_valid  # P7
+
+
+# ------------------------------------------------------------------ layout of the correction image
+def test_correction_layouts(pkg, tiny):
+    """TOFMLEM_OPT_CORR_BRICKS: with 0 the correction image of tofmlem_em_correction is a plain image and matches the
+    oracle's element by element; with 1 (default) it is in the context's internal order, the same multiset of values,
+    and em_correction + update gives the same image either way (and the same as the oracle)."""
+    cfg, n, ev, ev_np, g, og, sens = tiny
+    sig = oracle.sigma_mm(cfg.tof_fwhm_ps)
+    x = synth.random_image((g.nvox,), 13, device="cuda")
+    ref_corr, nv, _ = oracle.em_correction(og, sig, ev_np, x.cpu().numpy())
+    sens_np = sens.cpu().numpy()
+    ref_img = oracle.update(x.cpu().numpy().astype(np.float64), ref_corr, sens_np, oracle.mask_f32(sens_np))
+    images = {}
+    for bricks in (0, 1):
+        ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+        ctx.set_option(pkg.OPT_CORR_BRICKS, bricks)
+        corr = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+        ctx.em_correction(ev, n, x, corr)
+        c = corr.cpu().numpy().astype(np.float64)
+        if bricks == 0:
+            check_image(c, ref_corr)
+        else:
+            # 2x2x1 bricks: value of voxel (x, y, z) sits at ((z*ny/2 + y/2)*nx/2 + x/2)*4 + (y&1)*2 + (x&1)
+            lin = c.reshape(g.nz, g.ny // 2, g.nx // 2, 2, 2).transpose(0, 1, 3, 2, 4).reshape(-1)
+            check_image(lin, ref_corr)
+        img = x.clone()
+        ctx.update(img, corr, sens)
+        assert not corr.any()  # zeroed for the next pass
+        images[bricks] = img.cpu().numpy()
+        check_image(images[bricks], ref_img)
+    assert np.allclose(images[0], images[1], rtol=1e-4, atol=0)
