@@ -337,7 +337,9 @@ def main():
     ap.add_argument("--workload", default="full", choices=["full", "mid", "tiny"])
     ap.add_argument("--events", type=int, default=0, help="override the event count (debugging only)")
     ap.add_argument("--sens-lors", type=int, default=0, help="override the number of sensitivity LORs")
-    ap.add_argument("--ref-events", type=int, default=1_000_000, help="events per step of the oracle legs")
+    ap.add_argument("--ref-events", type=int, default=8_000_000,
+                    help="events per step of --impl reference (the oracle's per-call cost of ~0.75 s -- one private fp64 "
+                         "correction image per thread -- is amortised from a few million events on)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target duration of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -480,9 +482,9 @@ def main():
         "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_rand / 1e9, "unit": "G reductions/s",
         "frac": achieved / red_rand,
         # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3 from the committed ncu --set full capture
-        # (profiles/r02_em_persistent_ncu_full_metrics.txt: 6.916 GB read + 1.254 GB written); default full workload only
-        "traffic": 8.170312e9 if (args.workload == "full" and not args.events) else None,
-        "kernel": "em_persistent_kernel<TOF, v4>", "kernel_ms": kern_ms, "visits_per_launch": visits,
+        # (profiles/r03_em_persistent_ncu_full_metrics.txt: 7.108 GB read + 1.348 GB written); default full workload only
+        "traffic": 8.456278e9 if (args.workload == "full" and not args.events) else None,
+        "kernel": "em_persistent_kernel<TOF, v4, BRICK>", "kernel_ms": kern_ms, "visits_per_launch": visits,
         "reductions_per_launch": reds, "visits_per_reduction": visits / max(1, reds),
         "visits_Gps": visits / (kern_ms * 1e-3) / 1e9,
         "peak_source": "tofmlem_probe kind 0 (random-address RED.ADD.F32 into an L2-resident array of nvox floats: the "
@@ -538,7 +540,7 @@ def main():
                 break
             ns = ns2
         cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{ns} events (every {stride}th of the binned set), one EM pass + update on the full grid, {dt:.1f} s"}
+               "sample": f"{ns} events (stride {stride} through the binned set), one EM pass + update on the full grid, {dt:.1f} s"}
 
     if rank == 0:
         line = {
