@@ -34,6 +34,8 @@ struct SampledRay {
     int base[3];   // floor of the kernel centre's position in voxel units, per axis
     float f0[3];   // its fractional part
     float du[3];   // u / v: voxels per mm along the LOR
+    float guard;   // fast path: distance from a voxel plane (voxels) below which the fp64 expression decides
+    int k0, k1;    // samples k0 <= k < k1 lie between the LOR's end points (the others are dropped, R8)
 };
 
 __device__ __forceinline__ bool sampled_setup(const EventPtrs &ev, uint64_t e, SampledRay &r) {
@@ -68,7 +70,9 @@ __device__ __forceinline__ int sample_voxel(double p1, double u, double s, doubl
     return (int)f;
 }
 
-__device__ __forceinline__ void sampled_fast_setup(const ProjParams &P, SampledRay &r) {
+__device__ __forceinline__ void sampled_fast_setup(const ProjParams &P, const SampleLutEntry *__restrict__ lut, int K,
+                                                   SampledRay &r) {
+    float span = 0.0f;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double q0 = ((r.p1[a] + r.u[a] * r.s_c) - P.o[a]) * P.iv[a];
@@ -78,23 +82,43 @@ __device__ __forceinline__ void sampled_fast_setup(const ProjParams &P, SampledR
         r.base[a] = (int)fmax(-1.0e9, fmin(1.0e9, fl));
         r.f0[a] = (float)(q0 - fl);
         r.du[a] = (float)(r.u[a] * P.iv[a]);
+        span = fmaxf(span, fabsf(r.du[a]));
     }
+    // |q| <= 1 + half window * |du|: the float32 error of the fma is below 1e-5 voxel per 100 voxels of |q|
+    r.guard = 1.0e-4f + 1.0e-5f * (1.0f + (float)P.half_window * span);
+    // The offsets increase with k, so the samples between the end points (0 <= s_c + offset_k <= L, evaluated in
+    // fp64 exactly as the per-sample test would be) form one interval [k0, k1): found by scanning from both ends
+    // (no iteration at all unless the kernel centre is within 3 sigma of a detector).
+    int k0 = 0, k1 = K;
+    while (k0 < K) {
+        const double s = __dadd_rn(r.s_c, lut[k0].offset);
+        if (!(s < 0.0 || s > r.L)) break;
+        ++k0;
+    }
+    while (k1 > k0) {
+        const double s = __dadd_rn(r.s_c, lut[k1 - 1].offset);
+        if (!(s < 0.0 || s > r.L)) break;
+        --k1;
+    }
+    r.k0 = k0;
+    r.k1 = k1;
 }
 
 // voxel index along one axis through the float32 fast path; falls back to the exact fp64 decision near a voxel plane
 __device__ __forceinline__ int sample_voxel_fast(const ProjParams &P, const SampledRay &r, int a, float off, double s) {
     const float qf = fmaf(off, r.du[a], r.f0[a]);
-    const float guard = fmaf(1.0e-5f, fabsf(qf), 1.0e-4f);
-    if (fabsf(qf - rintf(qf)) < guard || !(fabsf(qf) < 1.0e6f))
+    const int fl = __float2int_rd(qf);
+    const float d = qf - (float)fl;  // distance to the voxel plane below, in voxels
+    if (fminf(d, 1.0f - d) < r.guard || !(fabsf(qf) < 1.0e6f))
         return sample_voxel(r.p1[a], r.u[a], s, P.o[a], P.v[a], P.iv[a], P.n[a]);
-    const int i = r.base[a] + (int)floorf(qf);
-    return (i < 0 || i >= P.n[a]) ? -1 : i;
+    const int i = r.base[a] + fl;
+    return (unsigned)i < (unsigned)P.n[a] ? i : -1;
 }
 
 // flat voxel index of sample k, or -1 when the sample is dropped
+// (for k0 <= k < k1; the end-point test was done by sampled_fast_setup)
 __device__ __forceinline__ int sample_index(const ProjParams &P, const SampledRay &r, const SampleLutEntry &l) {
-    const double s = __dadd_rn(r.s_c, l.offset);
-    if (s < 0.0 || s > r.L) return -1;
+    const double s = __dadd_rn(r.s_c, l.offset);  // only used by the fp64 fallback
     const int ix = sample_voxel_fast(P, r, 0, l.offset_f, s);
     const int iy = sample_voxel_fast(P, r, 1, l.offset_f, s);
     const int iz = sample_voxel_fast(P, r, 2, l.offset_f, s);
@@ -111,8 +135,8 @@ __global__ void __launch_bounds__(kBlock) sampled_forward_kernel(ProjParams P, c
     SampledRay r;
     float acc = 0.0f;
     if (sampled_setup(ev, e, r)) {
-        sampled_fast_setup(P, r);
-        for (int k = 0; k < K; ++k) {
+        sampled_fast_setup(P, lut, K, r);
+        for (int k = r.k0; k < r.k1; ++k) {
             const SampleLutEntry s = lut[k];
             const int j = sample_index(P, r, s);
             if (j >= 0) acc = fmaf(s.weight, __ldg(image + j), acc);
@@ -130,34 +154,39 @@ __global__ void __launch_bounds__(kBlock) sampled_backproject_kernel(ProjParams 
     if (e >= n) return;
     SampledRay r;
     if (!sampled_setup(ev, e, r)) return;
-    sampled_fast_setup(P, r);
+    sampled_fast_setup(P, lut, K, r);
     const float val = values ? __ldg(values + e) : 1.0f;
     if (val == 0.0f) return;
-    for (int k = 0; k < K; ++k) {
+    for (int k = r.k0; k < r.k1; ++k) {
         const SampleLutEntry s = lut[k];
         const int j = sample_index(P, r, s);
         if (j >= 0) atomicAdd(out + j, s.weight * val);
     }
 }
 
-// Fused EM pass of one event: pass 1 gathers (the forward value stays in a register), pass 2 recomputes the sample
-// voxels and scatters evw * w_k / fwd.  Consecutive samples of one event often fall into the same voxel (the sample
-// spacing 6 sigma/(K-1) = 3.7 mm at 300 ps, K = 32 is about one 3.75 mm voxel): equal neighbours are merged into one
-// reduction.
+// Fused EM pass of one event: pass 1 gathers (the forward value stays in a register) and keeps the voxel index of
+// each of the first kSampleCache samples in shared memory; pass 2 replays them (samples beyond the cache are recomputed)
+// and scatters evw * w_k / fwd.  Consecutive samples of one event often fall into the same voxel (the sample spacing
+// 6 sigma/(K-1) = 3.7 mm at 300 ps, K = 32 is about one 3.75 mm voxel): equal neighbours are merged into one reduction.
+// (Merging further into 16-byte reductions on a brick layout was measured: 3.64e9 -> 2.90e9 reductions but 28.0 ->
+// 30.0 ms at K = 32 -- this pass is bound by its instruction count, not by the L2 atomic units.)
+constexpr int kSampleCache = 32;
+
 __device__ __forceinline__ void sampled_em_event(const ProjParams &P, const SampleLutEntry *__restrict__ lut, int K,
                                                  const EventPtrs &ev, uint64_t e, uint64_t n,
                                                  const float *__restrict__ evw, const float *__restrict__ image,
-                                                 float *__restrict__ corr, unsigned &visits, unsigned &reds,
-                                                 bool &valid) {
+                                                 float *__restrict__ corr, int (*jcache)[kBlock], unsigned &visits,
+                                                 unsigned &reds, bool &valid) {
     SampledRay r;
     valid = false;
     visits = reds = 0;
     if (e < n && sampled_setup(ev, e, r)) {
-        sampled_fast_setup(P, r);
+        sampled_fast_setup(P, lut, K, r);
         float acc = 0.0f;
-        for (int k = 0; k < K; ++k) {
+        for (int k = r.k0; k < r.k1; ++k) {
             const SampleLutEntry s = lut[k];
             const int j = sample_index(P, r, s);
+            if (k < kSampleCache) jcache[k][threadIdx.x] = j;
             if (j >= 0) {
                 acc = fmaf(s.weight, __ldg(image + j), acc);
                 ++visits;
@@ -168,9 +197,8 @@ __device__ __forceinline__ void sampled_em_event(const ProjParams &P, const Samp
             const float scale = (evw ? __ldg(evw + e) : 1.0f) / acc;
             int pend = -1;
             float pw = 0.0f;
-            for (int k = 0; k < K; ++k) {
-                const SampleLutEntry s = lut[k];
-                const int j = sample_index(P, r, s);
+            for (int k = r.k0; k < r.k1; ++k) {
+                const int j = k < kSampleCache ? jcache[k][threadIdx.x] : sample_index(P, r, lut[k]);
                 if (j < 0) continue;
                 if (j != pend) {
                     if (pend >= 0) {
@@ -180,7 +208,7 @@ __device__ __forceinline__ void sampled_em_event(const ProjParams &P, const Samp
                     pend = j;
                     pw = 0.0f;
                 }
-                pw += s.weight;
+                pw += lut[k].weight;
             }
             if (pend >= 0) {
                 atomicAdd(corr + pend, pw * scale);
@@ -199,6 +227,7 @@ __global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const 
                                                             const float *__restrict__ image, float *__restrict__ corr,
                                                             DeviceStats *stats, unsigned *queues, unsigned nseg,
                                                             unsigned per_seg) {
+    __shared__ int jcache[kSampleCache][kBlock];  // voxel index of sample k of this thread's event (thread-private column)
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
@@ -214,8 +243,8 @@ __global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const 
         }
         unsigned visits, reds;
         bool valid;
-        sampled_em_event(P, lut, K, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, visits, reds,
-                         valid);
+        sampled_em_event(P, lut, K, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, jcache, visits,
+                         reds, valid);
         nv += valid;
         vis += visits;
         nr += reds;
