@@ -2,7 +2,7 @@
  * tofmlem.h -- C ABI of libtofmlem: list-mode TOF-weighted MLEM hot path on one NVIDIA B200 (sm_100a).
  *
  * Source of every operation: arxiv 1706.07075 ("PAPER.md" = /root/reference/PAPER.md) as read in
- * DESIGN.md (readings R1..R22).  The paper states the problem in prose only (events with a TOF time
+ * DESIGN.md (readings R1..R26).  The paper states the problem in prose only (events with a TOF time
  * difference -> image by TOF-weighted list-mode MLEM; nine-region TOF-assisted
  * data division); the call list follows BASELINE.json's north_star.
  *
