@@ -471,25 +471,27 @@ def main():
     red_row = n_ops / (ctx.probe(1, probe_buf, n_ops) * 1e-3)
     ld_rand = n_ops / (ctx.probe(2, probe_buf, n_ops) * 1e-3)
     ld_row = n_ops / (ctx.probe(3, probe_buf, n_ops) * 1e-3)
+    red_rand_v4 = n_ops / (ctx.probe(5, probe_buf, n_ops) * 1e-3)  # the kernel's own instruction: 16-byte reductions
+    red_peak = max(red_rand, red_rand_v4)  # the roofline uses the HIGHER of the two request rates
     del probe_buf
     hbm_bytes = 28.0 * n  # algorithmic HBM bytes per launch: 7 float32 per event
     reds = int(st.reductions)  # reduction instructions of one launch (each is one request to an L2 atomic unit)
     t_hbm = hbm_bytes / (hbm_peak * 1e9)
-    t_red = reds / red_rand
+    t_red = reds / red_peak
     t_ld = visits / ld_rand
     achieved = reds / (kern_ms * 1e-3)
     roofline = {
-        "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_rand / 1e9, "unit": "G reductions/s",
-        "frac": achieved / red_rand,
+        "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_peak / 1e9, "unit": "G reductions/s",
+        "frac": achieved / red_peak,
         # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3 from the committed ncu --set full capture
         # (profiles/r03_em_persistent_ncu_full_metrics.txt: 7.108 GB read + 1.348 GB written); default full workload only
         "traffic": 8.456278e9 if (args.workload == "full" and not args.events) else None,
         "kernel": "em_persistent_kernel<TOF, v4, BRICK>", "kernel_ms": kern_ms, "visits_per_launch": visits,
         "reductions_per_launch": reds, "visits_per_reduction": visits / max(1, reds),
         "visits_Gps": visits / (kern_ms * 1e-3) / 1e9,
-        "peak_source": "tofmlem_probe kind 0 (random-address RED.ADD.F32 into an L2-resident array of nvox floats: the "
-                       "request rate of the L2 atomic units), measured in this run",
-        "probes_Gops": {"red_random": red_rand / 1e9, "red_row": red_row / 1e9, "gather_random": ld_rand / 1e9,
+        "peak_source": "tofmlem_probe: random-address reductions into an L2-resident array of nvox floats, the higher of "
+                       "the 4-byte (kind 0) and the 16-byte (kind 5) request rates, measured in this run",
+        "probes_Gops": {"red_random": red_rand / 1e9, "red_random_v4": red_rand_v4 / 1e9, "red_row": red_row / 1e9, "gather_random": ld_rand / 1e9,
                         "gather_row": ld_row / 1e9},
         "t_roof_ms": {"hbm": t_hbm * 1e3, "red": t_red * 1e3, "gather": t_ld * 1e3},
         "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_GBs": hbm_bytes / (kern_ms * 1e-3) / 1e9, "peak_GBs": hbm_peak,

@@ -233,8 +233,9 @@ int tofmlem_scatter_reject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t 
 /* Roofline probe (measurement aid; north_star asks for the MEASURED atomic / L2 roofline): issues n_ops float32
  * operations against d_buf[0..n_elems) and returns the elapsed milliseconds in *h_ms (second of two passes, so
  * the array is L2-resident when it fits).  kind 0: RED.ADD.F32 to unrelated random elements per lane; 1: RED to
- * 32 consecutive elements of a random row per warp; 2 / 3: the same two patterns with 4-byte loads.
- * d_buf is modified by kinds 0, 1.  SYNCHRONISES. */
+ * 32 consecutive elements of a random row per warp; 2 / 3: the same two patterns with 4-byte loads; 4 / 5: random
+ * 8-byte / 16-byte vector reductions (one n_ops unit = one instruction per lane).
+ * d_buf is modified by kinds 0, 1, 4, 5.  SYNCHRONISES. */
 int tofmlem_probe(tofmlem_ctx *ctx, int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *h_ms);
 
 /* Copies the counters of the last pass to *h_out.  SYNCHRONISES the context's stream. */

@@ -19,17 +19,18 @@ __global__ void __launch_bounds__(256) probe_kernel(float *buf, uint32_t n, int 
     const uint32_t tid = blockIdx.x * 256u + threadIdx.x;
     const uint32_t lane = threadIdx.x & 31u, warp = tid >> 5;
     float acc = 0.0f;
-    uint32_t h = mix32(((KIND & 1) ? warp : tid) * 2654435761u + 12345u);
+    constexpr bool kRow = KIND == 1 || KIND == 3;  // lanes of a warp on 32 consecutive elements of a random row
+    uint32_t h = mix32((kRow ? warp : tid) * 2654435761u + 12345u);
 #pragma unroll 4
     for (int i = 0; i < ops; ++i) {
         h = mix32(h + 0x9e3779b9u);
         uint32_t a;
-        if (KIND & 1)
+        if (kRow)
             a = ((h % (n >> 5)) << 5) + lane;
         else
             a = h % n;
         if (KIND < 2)
-            atomicAdd(buf + a, 1.0f);
+            atomicAdd(buf + a, 1.0f);  // result unused: RED.E.ADD.F32
         else if (KIND == 4)
             asm volatile("red.global.add.v2.f32 [%0], {%1, %1};" ::"l"(buf + (a & ~1u)), "f"(1.0f) : "memory");
         else if (KIND == 5)
