@@ -27,8 +27,8 @@ struct Ray {
     float t_end, tc;
     float t0x, t0y, t0z;
     float tdx, tdy, tdz;
-    int idx;            // flat index of the first voxel (in the lane's layout)
-    int dxi, dyi, dzi;  // flat-index increments of a step along each (permuted) axis, 0 when parallel
+    int idx;            // flat index of the first voxel
+    int dxi, dyi, dzi;  // flat-index increments of a step along each axis, 0 when parallel
     // brick layout of the correction image (2x2x1 voxels per 16-byte group, see ProjParams::brick):
     int bidx;        // brick-layout index of the first voxel
     int bdx0, bdxs;  // x step: increment for the first step, and the sum of the two alternating increments
@@ -55,13 +55,6 @@ __device__ __forceinline__ void red_v4_if(bool p, float *ptr, float a, float b, 
 }
 
 constexpr float kBigT = 1.0e30f;
-
-// Three-way select on the layout index for the pointer triples (a dynamically indexed pointer array in the
-// kernel parameters would be copied to local memory).
-template <class T>
-__device__ __forceinline__ T sel3(int a, T v0, T v1, T v2) {
-    return a == 0 ? v0 : (a == 1 ? v1 : v2);
-}
 
 // Per-axis set-up; returns the parameter at which the ray leaves the grid through this axis.
 __device__ __forceinline__ float axis_setup(double p1, double u, double s_lo, double o, double v, double iv, int n,
@@ -98,31 +91,14 @@ __device__ __forceinline__ bool axis_clip(double p1, double u, double lo, double
     return true;
 }
 
-// LAYOUTS: permute the axes per lane so that axis "A" (fastest in memory) is the ray's dominant axis;
-// `layout` receives 0/1/2 = which of x/y/z that is.  Without LAYOUTS the canonical order is used.
-// (LAYOUTS = true was measured and is NOT used by any kernel at present: DESIGN.md "What was tried".)
-template <bool TOF, bool LAYOUTS>
+// Ray set-up in fp64 (comment (1) at the top); false when the event is skipped or its window misses the grid.
+template <bool TOF>
 __device__ __forceinline__ bool ray_setup(const ProjParams &P, float fx1, float fy1, float fz1, float fx2, float fy2,
-                                          float fz2, float fdt, Ray &r, int &layout) {
-    layout = 0;
+                                          float fz2, float fdt, Ray &r) {
     if (!(finite_f(fx1) && finite_f(fy1) && finite_f(fz1) && finite_f(fx2) && finite_f(fy2) && finite_f(fz2)))
         return false;
     if (TOF && !finite_f(fdt)) return false;
-    int A = 0, B = 1, C = 2;
-    if (LAYOUTS) {
-        const float ax = fabsf(fx2 - fx1), ay = fabsf(fy2 - fy1), az = fabsf(fz2 - fz1);
-        const int a = (ay > ax) ? ((az > ay) ? 2 : 1) : ((az > ax) ? 2 : 0);
-        layout = a;
-        // cyclic permutation (A,B,C) = (a, a+1, a+2) mod 3, applied to the six coordinates
-        const float ta1 = a == 0 ? fx1 : (a == 1 ? fy1 : fz1), ta2 = a == 0 ? fx2 : (a == 1 ? fy2 : fz2);
-        const float tb1 = a == 0 ? fy1 : (a == 1 ? fz1 : fx1), tb2 = a == 0 ? fy2 : (a == 1 ? fz2 : fx2);
-        const float tc1 = a == 0 ? fz1 : (a == 1 ? fx1 : fy1), tc2 = a == 0 ? fz2 : (a == 1 ? fx2 : fy2);
-        fx1 = ta1; fx2 = ta2; fy1 = tb1; fy2 = tb2; fz1 = tc1; fz2 = tc2;
-        A = a;
-        B = a == 2 ? 0 : a + 1;
-        C = a == 0 ? 2 : a - 1;
-    }
-    // dynamically indexed kernel parameters: ptxas turns these into indexed constant-bank loads
+    constexpr int A = 0, B = 1, C = 2;
     const int nA = P.n[A], nB = P.n[B], nC = P.n[C];
     const double oA = P.o[A], oB = P.o[B], oC = P.o[C];
     const double hA = P.h[A], hB = P.h[B], hC = P.h[C];
@@ -153,7 +129,7 @@ __device__ __forceinline__ bool ray_setup(const ProjParams &P, float fx1, float 
     const float ec = axis_setup(z1, uz, s_lo, oC, vC, ivC, nC, nA * nB, ic, r.dzi, r.t0z, r.tdz);
     r.t_end = fminf(fminf((float)(s_hi - s_lo), ea), fminf(eb, ec));
     r.idx = (ic * nB + ib) * nA + ia;
-    if (!LAYOUTS && P.brick) {
+    if (P.brick) {
         // index = (brick number) * 4 + (iy & 1) * 2 + (ix & 1): a step in x alternates between +-1 (inside the brick)
         // and +-3 (into the neighbouring brick), a step in y between +-2 and +-(2 nx - 2); z steps are unchanged
         r.bidx = ((ic * (nB >> 1) + (ib >> 1)) * (nA >> 1) + (ia >> 1)) * 4 + ((ib & 1) << 1) + (ia & 1);
@@ -282,13 +258,12 @@ __device__ __forceinline__ int ray_scatter(const ProjParams &P, const Ray &r, fl
 
 constexpr int kBlock = 256;
 
-template <bool TOF, bool LAYOUTS>
-__device__ __forceinline__ bool load_and_setup(const ProjParams &P, const EventPtrs &ev, uint64_t e, Ray &r,
-                                               int &layout) {
+template <bool TOF>
+__device__ __forceinline__ bool load_and_setup(const ProjParams &P, const EventPtrs &ev, uint64_t e, Ray &r) {
     const float x1 = __ldg(ev.x1 + e), y1 = __ldg(ev.y1 + e), z1 = __ldg(ev.z1 + e);
     const float x2 = __ldg(ev.x2 + e), y2 = __ldg(ev.y2 + e), z2 = __ldg(ev.z2 + e);
     const float dt = (TOF && ev.dt) ? __ldg(ev.dt + e) : 0.0f;
-    return ray_setup<TOF, LAYOUTS>(P, x1, y1, z1, x2, y2, z2, dt, r, layout);
+    return ray_setup<TOF>(P, x1, y1, z1, x2, y2, z2, dt, r);
 }
 
 // Event index of this thread under the interleaved chunk order (comment (5) at the top).
@@ -305,9 +280,8 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(ProjParams P, EventPtrs
     const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
     if (e >= n) return;
     Ray r;
-    int layout;
     float acc = 0.0f;
-    if (load_and_setup<TOF, false>(P, ev, e, r, layout)) {
+    if (load_and_setup<TOF>(P, ev, e, r)) {
         int visits;
         acc = ray_gather<TOF>(P, r, image, visits);
         if (TOF) acc *= P.gauss_norm;
@@ -322,8 +296,7 @@ __global__ void __launch_bounds__(kBlock) backproject_kernel(ProjParams P, Event
     const uint64_t e = event_index(P.stride);
     if (e >= n) return;
     Ray r;
-    int layout;
-    if (!load_and_setup<TOF, false>(P, ev, e, r, layout)) return;
+    if (!load_and_setup<TOF>(P, ev, e, r)) return;
     float val = values ? __ldg(values + e) : 1.0f;
     if (TOF) val *= P.gauss_norm;
     if (val == 0.0f) return;
@@ -337,11 +310,10 @@ __device__ __forceinline__ void em_event(const ProjParams &P, const EventPtrs &e
                                          const float *__restrict__ evw, const float *__restrict__ image,
                                          float *__restrict__ corr, int &visits, bool &valid, int &reds) {
     Ray r;
-    int layout;
     visits = 0;
     reds = 0;
     valid = false;
-    if (e < n && load_and_setup<TOF, false>(P, ev, e, r, layout)) {
+    if (e < n && load_and_setup<TOF>(P, ev, e, r)) {
         const float acc = ray_gather<TOF>(P, r, image, visits);
         if (acc > 0.0f) {  // R9
             valid = true;
@@ -470,8 +442,7 @@ __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P
         }
         const uint64_t e = ((uint64_t)seg * per_seg + c) * 32u + lane;
         Ray r;
-        int layout;
-        if (e < n && load_and_setup<TOF, false>(P, ev, e, r, layout)) {
+            if (e < n && load_and_setup<TOF>(P, ev, e, r)) {
             int visits;
             const float acc = ray_gather<TOF>(P, r, image, visits);
             vis += visits;
