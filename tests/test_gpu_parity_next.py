@@ -284,3 +284,58 @@ def test_correction_layouts(pkg, tiny):
         images[bricks] = img.cpu().numpy()
         check_image(images[bricks], ref_img)
     assert np.allclose(images[0], images[1], rtol=1e-4, atol=0)
+
+
+# ------------------------------------------------------------------ the paper's whole chain (Table 2)
+def test_paper_pipeline_parity(pkg):
+    """Pre-processing (TOF scatter rejection, attenuation weights), starting backprojection as x0,
+    then MLEM iterations with the per-event weights and the median filter after each iteration,
+    on locality-binned events: the CUDA chain against the same chain of oracle calls."""
+    cfg = synth.MID
+    n, m, iters = 120_000, 500_000, 3
+    ev = synth.make_events(cfg, n, device="cuda")
+    ev_np = to_np(ev)
+    g, og = grids(pkg, cfg)
+    sig = oracle.sigma_mm(cfg.tof_fwhm_ps)
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ctx.set_option(pkg.OPT_MEDIAN, 1)
+    # 1. scatter rejection against the body outline, compaction
+    ell = oracle.ellipsoids_f32(synth.body_outline(cfg))
+    h = oracle.scatter_half_width_f32(sig)
+    keep = torch.empty(n, dtype=torch.uint8, device="cuda")
+    perm = torch.empty(n, dtype=torch.int32, device="cuda")
+    kept = ctx.scatter_reject(ev, n, torch.from_numpy(ell), float(h), keep, perm)
+    ref_keep, ref_cnt = oracle.scatter_keep(ev_np, ell, h)
+    assert kept == ref_cnt and np.array_equal(keep.cpu().numpy(), ref_keep)
+    kev = {k: torch.empty(kept, dtype=torch.float32, device="cuda") for k in ev}
+    ctx.gather_events(ev, perm, kept, kev)
+    kev_np = to_np(kev)  # the oracle works on the same compacted order
+    # 2. attenuation weights
+    mu = synth.rasterize_mu_map(cfg, device="cuda").reshape(-1).contiguous()
+    w = torch.empty(kept, dtype=torch.float32, device="cuda")
+    ctx.attenuation_weights(kev, kept, mu, w)
+    # 3. sensitivity, 4. starting backprojection
+    lors = synth.make_sens_lors(cfg, m, device="cuda")
+    sens = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.sensitivity(lors, m, sens)
+    x0 = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.backproject(kev, kept, None, x0)
+    ref_x0 = oracle.backproject(og, sig, kev_np)
+    check_image(x0.cpu().numpy(), ref_x0)
+    # 5. locality binning of events and weights, 6. iterations
+    key = torch.empty(kept, dtype=torch.int32, device="cuda")
+    bperm = torch.empty(kept, dtype=torch.int32, device="cuda")
+    ctx.bin_events(kev, kept, key, bperm, None)
+    sev = {k: torch.empty_like(v) for k, v in kev.items()}
+    ctx.permute_events(kev, bperm, kept, sev)
+    sw = torch.empty_like(w)
+    ctx.gather_f32(w, bperm, kept, sw)
+    img = x0.clone()
+    ctx.iterate_weighted(sev, kept, sw, img, sens, iters)
+    # the oracle chain starts from the SAME float32 x0, weights and sensitivity (so that only the iterations differ)
+    ref, _ = oracle.mlem(og, sig, kev_np, x0.cpu().numpy().astype(np.float64), sens.cpu().numpy(), iters,
+                         weights=w.cpu().numpy(), median=True)
+    gpu = img.cpu().numpy().astype(np.float64)
+    rel_l2 = np.linalg.norm(gpu - ref) / np.linalg.norm(ref)
+    big = ref > 0.01 * ref.max()
+    assert rel_l2 <= 1e-3 and np.max(np.abs(gpu[big] - ref[big]) / ref[big]) <= 1e-2, rel_l2
