@@ -285,18 +285,17 @@ def run_report(args):
             kev = {k: torch.empty(kept, dtype=torch.float32, device=dev) for k in ev}
             stage("compaction", lambda: base.gather_events(ev, perm, kept, kev))
             del keep, perm
-            w = torch.empty(kept, dtype=torch.float32, device=dev)
-            stage("attenuation_weights", lambda: base.attenuation_weights(kev, kept, mu, w))
             x = torch.zeros(nvox, dtype=torch.float32, device=dev)
             stage("starting_backprojection", lambda: base.backproject(kev, kept, None, x))
             key = torch.empty(kept, dtype=torch.int32, device=dev)
             bperm = torch.empty(kept, dtype=torch.int32, device=dev)
             sev = {k: torch.empty_like(v) for k, v in kev.items()}
-            sw = torch.empty_like(w)
             stage("binning_and_permutation", lambda: (base.bin_events(kev, kept, key, bperm, None),
-                                                      base.permute_events(kev, bperm, kept, sev),
-                                                      base.gather_f32(w, bperm, kept, sw)))
-            del kev, w, key, bperm
+                                                      base.permute_events(kev, bperm, kept, sev)))
+            del kev, key, bperm
+            # on the binned events: neighbouring LORs are nearly parallel and close, so the mu-map gathers hit L1
+            sw = torch.empty(kept, dtype=torch.float32, device=dev)
+            stage("attenuation_weights", lambda: base.attenuation_weights(sev, kept, mu, sw))
             stage("mlem_20_iterations_with_median", lambda: base.iterate_weighted(sev, kept, sw, x, sens, iters))
             return kept, x
 
