@@ -260,9 +260,9 @@ constexpr int kBlock = 256;
 
 template <bool TOF>
 __device__ __forceinline__ bool load_and_setup(const ProjParams &P, const EventPtrs &ev, uint64_t e, Ray &r) {
-    const float x1 = __ldg(ev.x1 + e), y1 = __ldg(ev.y1 + e), z1 = __ldg(ev.z1 + e);
-    const float x2 = __ldg(ev.x2 + e), y2 = __ldg(ev.y2 + e), z2 = __ldg(ev.z2 + e);
-    const float dt = (TOF && ev.dt) ? __ldg(ev.dt + e) : 0.0f;
+    const float x1 = __ldcs(ev.x1 + e), y1 = __ldcs(ev.y1 + e), z1 = __ldcs(ev.z1 + e);
+    const float x2 = __ldcs(ev.x2 + e), y2 = __ldcs(ev.y2 + e), z2 = __ldcs(ev.z2 + e);
+    const float dt = (TOF && ev.dt) ? __ldcs(ev.dt + e) : 0.0f;
     return ray_setup<TOF>(P, x1, y1, z1, x2, y2, z2, dt, r);
 }
 

@@ -39,9 +39,9 @@ struct SampledRay {
 };
 
 __device__ __forceinline__ bool sampled_setup(const EventPtrs &ev, uint64_t e, SampledRay &r) {
-    const float x1 = __ldg(ev.x1 + e), y1 = __ldg(ev.y1 + e), z1 = __ldg(ev.z1 + e);
-    const float x2 = __ldg(ev.x2 + e), y2 = __ldg(ev.y2 + e), z2 = __ldg(ev.z2 + e);
-    const float dt = ev.dt ? __ldg(ev.dt + e) : 0.0f;
+    const float x1 = __ldcs(ev.x1 + e), y1 = __ldcs(ev.y1 + e), z1 = __ldcs(ev.z1 + e);
+    const float x2 = __ldcs(ev.x2 + e), y2 = __ldcs(ev.y2 + e), z2 = __ldcs(ev.z2 + e);
+    const float dt = ev.dt ? __ldcs(ev.dt + e) : 0.0f;
     if (!(finite_f(x1) && finite_f(y1) && finite_f(z1) && finite_f(x2) && finite_f(y2) && finite_f(z2) && finite_f(dt)))
         return false;
     r.p1[0] = x1;
