@@ -19,6 +19,8 @@
 //      advance in parallel): each CTA stays local for its gathers, while the reductions of the ~900
 //      co-resident CTAs spread over the whole volume instead of serialising on a few hot L2 sectors
 //      (measured: 47.8 -> 35.7 ms per pass at cfg-3).
+#include <math.h>
+
 #include "internal.cuh"
 
 namespace tofmlem {
@@ -344,7 +346,7 @@ __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, Eve
 }
 
 // Persistent form of the fused pass (the default): the locality-binned event list is cut into `nseg` contiguous
-// segments, one per SM; every warp takes 32-event chunks from the queue of the SM it runs on (%smid), so the warps
+// segments, two per SM; every warp takes 32-event chunks from the queue of the SM it runs on (%smid), so the warps
 // resident on an SM work on neighbouring events and share that SM's L1 for their image gathers (the 8 co-resident
 // CTAs of the grid-order form come from 8 unrelated places and thrash it), while different SMs reduce into different
 // parts of the volume.  A warp whose segment is exhausted moves on to other segments (work stealing; the invalid
@@ -354,11 +356,14 @@ __global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, Eve
                                                                const float *__restrict__ evw,
                                                                const float *__restrict__ image,
                                                                float *__restrict__ corr, DeviceStats *stats,
-                                                               unsigned *queues, unsigned nseg, unsigned per_seg) {
+                                                               unsigned *queues, unsigned nseg, unsigned per_seg,
+                                                               unsigned segs_per_sm) {
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
-    unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0, nr = 0;
+    // nseg = segs_per_sm * base segments: the warps of an SM start on segs_per_sm of them (base apart in the list)
+    const unsigned base = nseg / segs_per_sm;
+    unsigned seg = smid % base + base * ((threadIdx.x >> 5) % segs_per_sm), tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
         if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
@@ -545,14 +550,18 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
             cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         }
-        unsigned nseg = (unsigned)n_sm;
-        if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
-        if (nseg % 61u == 0) nseg -= 1;
+        // Short windows: two segments per SM (measured at cfg-3, 300 ps: 1 / 2 / 4 / 8 segments per SM -> 21.47 / 21.17 /
+        // 22.25 / 23.54 ms; 100 ps: 11.35 -> 9.69 ms).  Long walks (600 ps: 43.3 -> 45.1 ms, non-TOF: 203 -> 218 ms) keep one.
+        const double reach = 2.0 * p.half_window * sqrt(p.iv[0] * p.iv[0] + p.iv[1] * p.iv[1] + p.iv[2] * p.iv[2]);
+        const unsigned kSegsPerSm = (TOF && reach <= 80.0) ? 2u : 1u;  // reach = largest visit count of a window
+        unsigned nseg = (unsigned)n_sm * kSegsPerSm;
+        if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / kSegsPerSm * kSegsPerSm;
+        if (nseg % 61u == 0) nseg -= kSegsPerSm;  // the stealing stride 61 must not divide the number of segments
         const uint64_t wchunks = (n + 31) / 32;
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
         cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-        em_persistent_kernel<TOF, VEC, BRICK><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, ev, n, evw, image, corr,
-                                                                                         stats, queues, nseg, per_seg);
+        em_persistent_kernel<TOF, VEC, BRICK><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(
+            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, kSegsPerSm);
     } else {
         em_correction_kernel<TOF, VEC, BRICK><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
     }
