@@ -226,12 +226,13 @@ __global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const 
                                                             EventPtrs ev, uint64_t n, const float *__restrict__ evw,
                                                             const float *__restrict__ image, float *__restrict__ corr,
                                                             DeviceStats *stats, unsigned *queues, unsigned nseg,
-                                                            unsigned per_seg) {
+                                                            unsigned per_seg, unsigned segs_per_sm) {
     __shared__ int jcache[kSampleCache][kBlock];  // voxel index of sample k of this thread's event (thread-private column)
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
-    unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0, nr = 0;
+    const unsigned base = nseg / segs_per_sm;  // the warps of an SM start on segs_per_sm segments, base apart
+    unsigned seg = smid % base + base * ((threadIdx.x >> 5) % segs_per_sm), tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
         if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
@@ -284,14 +285,15 @@ void launch_sampled_em(const ProjParams &p, const SampleLutEntry *lut, int K, co
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sampled_em_kernel, kBlock, 0);
         cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     }
-    unsigned nseg = (unsigned)n_sm;
-    if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
-    if (nseg % 61u == 0) nseg -= 1;
+    constexpr unsigned kSegsPerSm = 2;  // as in projector.cu's persistent pass for short windows
+    unsigned nseg = (unsigned)n_sm * kSegsPerSm;
+    if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / kSegsPerSm * kSegsPerSm;
+    if (nseg % 61u == 0) nseg -= kSegsPerSm;
     const uint64_t wchunks = (n + 31) / 32;
     const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
     cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
     sampled_em_kernel<<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, lut, K, ev, n, evw, image, corr, stats,
-                                                                        queues, nseg, per_seg);
+                                                                        queues, nseg, per_seg, kSegsPerSm);
 }
 
 }  // namespace tofmlem
