@@ -352,7 +352,7 @@ __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, Eve
 // parts of the volume.  A warp whose segment is exhausted moves on to other segments (work stealing; the invalid
 // events sorted to the end of the list make the last segments empty).  Measured at cfg-3: 30.2 -> 25.2 ms.
 template <bool TOF, bool VEC, bool BRICK>
-__global__ void __launch_bounds__(kBlock) em_persistent_kernel(ProjParams P, EventPtrs ev, uint64_t n,
+__global__ void __launch_bounds__(kBlock, 5) em_persistent_kernel(ProjParams P, EventPtrs ev, uint64_t n,
                                                                const float *__restrict__ evw,
                                                                const float *__restrict__ image,
                                                                float *__restrict__ corr, DeviceStats *stats,
