@@ -550,10 +550,11 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
             cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         }
-        // Short windows: two segments per SM (measured at cfg-3, 300 ps: 1 / 2 / 4 / 8 segments per SM -> 21.47 / 21.17 /
-        // 22.25 / 23.54 ms; 100 ps: 11.35 -> 9.69 ms).  Long walks (600 ps: 43.3 -> 45.1 ms, non-TOF: 203 -> 218 ms) keep one.
+        // Short windows: the warps of an SM spread over several list segments (measured at 146 M events: 300 ps, 1 / 2 /
+        // 3 / 4 / 8 segments per SM -> 21.47 / 21.04 / 20.75 / 22.25 / 23.54 ms; 100 ps, 1 / 2 / 3 / 4 -> 11.35 / 9.57 /
+        // 9.44 / 9.32 ms).  Long walks (600 ps: 43.3 -> 45.1 ms, non-TOF: 203 -> 218 ms with 2) keep one.
         const double reach = 2.0 * p.half_window * sqrt(p.iv[0] * p.iv[0] + p.iv[1] * p.iv[1] + p.iv[2] * p.iv[2]);
-        const unsigned kSegsPerSm = (TOF && reach <= 80.0) ? 2u : 1u;  // reach = largest visit count of a window
+        const unsigned kSegsPerSm = !TOF || reach > 80.0 ? 1u : (reach > 30.0 ? 3u : 4u);  // reach = largest visit count
         unsigned nseg = (unsigned)n_sm * kSegsPerSm;
         if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / kSegsPerSm * kSegsPerSm;
         if (nseg % 61u == 0) nseg -= kSegsPerSm;  // the stealing stride 61 must not divide the number of segments
