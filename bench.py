@@ -544,8 +544,8 @@ def main():
         "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_peak / 1e9, "unit": "G reductions/s",
         "frac": achieved / red_peak,
         # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3 from the committed ncu --set full capture
-        # (profiles/r04_em_persistent_ncu_full_metrics.txt: 6.529 GB read + 1.120 GB written); default full workload only
-        "traffic": 7.648770e9 if (args.workload == "full" and not args.events) else None,
+        # (profiles/r04_em_persistent_ncu_full_metrics.txt: 6.894 GB read + 1.283 GB written); default full workload only
+        "traffic": 8.177348e9 if (args.workload == "full" and not args.events) else None,
         "kernel": "em_persistent_kernel<TOF, v4, BRICK>", "kernel_ms": kern_ms, "visits_per_launch": visits,
         "reductions_per_launch": reds, "visits_per_reduction": visits / max(1, reds),
         "visits_Gps": visits / (kern_ms * 1e-3) / 1e9,
