@@ -31,6 +31,12 @@ struct tofmlem_ctx {
     unsigned *d_queues = nullptr;  // work counters of the persistent EM kernel
     uint32_t *d_hist = nullptr, *d_cursor = nullptr, *d_scan_tmp = nullptr;
     size_t hist_cap = 0;
+    // scratch of tofmlem_reconstruct_regions, kept between calls (64 B per event): region ids / keys, permutation,
+    // region-sorted and region-binned event copies
+    int32_t *d_rg_region = nullptr;
+    uint32_t *d_rg_perm = nullptr;
+    float *d_rg_sorted = nullptr, *d_rg_binned = nullptr;
+    size_t rg_cap = 0;
     float *d_pack = nullptr;   // 32-byte event records of tofmlem_gather_events
     size_t pack_cap = 0;
     uint8_t *d_sub = nullptr;  // sub-bin of every event of the last tofmlem_bin_events
@@ -320,6 +326,10 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_scan_tmp);
     cudaFree(ctx->d_sub);
     cudaFree(ctx->d_pack);
+    cudaFree(ctx->d_rg_region);
+    cudaFree(ctx->d_rg_perm);
+    cudaFree(ctx->d_rg_sorted);
+    cudaFree(ctx->d_rg_binned);
     cudaFree(ctx->d_tmp_image);
     cudaFree(ctx->d_lut);
     cudaFree(ctx->d_rcounts);
@@ -829,10 +839,6 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
             cudaFree(images[r]);
         }
         if (ready) cudaEventDestroy(ready);
-        cudaFree(d_region);
-        cudaFree(d_perm);
-        cudaFree(d_sorted);
-        cudaFree(d_binned);
     };
 #define RCU(call)                                          \
     do {                                                   \
@@ -853,10 +859,25 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
             return rc;                 \
         }                              \
     } while (0)
-    RCU(cudaMalloc(&d_region, n * sizeof(int32_t)));
-    RCU(cudaMalloc(&d_perm, n * sizeof(uint32_t)));
-    RCU(cudaMalloc(&d_sorted, 7 * stride * sizeof(float)));
-    RCU(cudaMalloc(&d_binned, 7 * stride * sizeof(float)));
+    if (ctx->rg_cap < stride) {  // event scratch is kept by the context: repeated calls do not allocate 64 B per event again
+        cudaFree(ctx->d_rg_region);
+        cudaFree(ctx->d_rg_perm);
+        cudaFree(ctx->d_rg_sorted);
+        cudaFree(ctx->d_rg_binned);
+        ctx->d_rg_region = nullptr;
+        ctx->d_rg_perm = nullptr;
+        ctx->d_rg_sorted = ctx->d_rg_binned = nullptr;
+        ctx->rg_cap = 0;
+        RCU(cudaMalloc(&ctx->d_rg_region, stride * sizeof(int32_t)));
+        RCU(cudaMalloc(&ctx->d_rg_perm, stride * sizeof(uint32_t)));
+        RCU(cudaMalloc(&ctx->d_rg_sorted, 7 * stride * sizeof(float)));
+        RCU(cudaMalloc(&ctx->d_rg_binned, 7 * stride * sizeof(float)));
+        ctx->rg_cap = stride;
+    }
+    d_region = ctx->d_rg_region;
+    d_perm = ctx->d_rg_perm;
+    d_sorted = ctx->d_rg_sorted;
+    d_binned = ctx->d_rg_binned;
     RRC(tofmlem_split_regions(ctx, ev, n, n_regions, h_zbounds, d_region, d_perm, counts.data()));
     tofmlem_events_mut sorted{d_sorted, d_sorted + stride, d_sorted + 2 * stride, d_sorted + 3 * stride,
                               d_sorted + 4 * stride, d_sorted + 5 * stride, ev->dt ? d_sorted + 6 * stride : nullptr};
@@ -900,7 +921,14 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
                                   sorted.dt ? d_binned + 6 * stride + off : nullptr};
         if (counts[r]) {
             rc = tofmlem_bin_events(sc, &sub_ev, counts[r], reinterpret_cast<uint32_t *>(d_region) + off, d_perm + off, nullptr);
-            if (rc == TOFMLEM_OK) rc = tofmlem_permute_events(sc, &sub_ev, d_perm + off, counts[r], &bin_ev);
+            if (rc == TOFMLEM_OK && ctx->pack_cap >= n) {
+                // permutation through 32-byte records in the parent's record scratch (free again after the region split)
+                float *dst[7] = {bin_ev.x1, bin_ev.y1, bin_ev.z1, bin_ev.x2, bin_ev.y2, bin_ev.z2, bin_ev.dt};
+                launch_gather_packed(ev_ptrs(&sub_ev), d_perm + off, counts[r], ctx->d_pack + 8 * off, dst, streams[r]);
+                sc->launches += 2;
+            } else if (rc == TOFMLEM_OK) {
+                rc = tofmlem_gather_events(sc, &sub_ev, d_perm + off, counts[r], &bin_ev);
+            }
             if (rc != TOFMLEM_OK) {
                 ctx->err = sc->err;
                 cudaDeviceSynchronize();
