@@ -97,6 +97,10 @@ enum {
                                        shared-memory write-back cache (0..8); the others reduce at L2 directly */
     TOFMLEM_OPT_MEDIAN = 10,        /* 1: tofmlem_iterate applies the 3x3x3 median filter to the image estimate after
                                        every update (R23); default 0 */
+    TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
+                                       generated an identically reconstructed image").  0 (default) is accepted; 1
+                                       returns TOFMLEM_EUNSUPPORTED: the correction image is summed with float32
+                                       reductions whose order is not fixed (run-to-run differences ~1e-7 relative) */
     TOFMLEM_OPT_SUBBINS = 9         /* tofmlem_bin_events: order the events INSIDE each locality bin by predicted
                                        voxel-visit count, in `value` sub-bins (1..64, default 16; 1 = off), so that
                                        the events of a warp walk windows of nearly equal length.  Keys, bin offsets
@@ -113,6 +117,16 @@ int tofmlem_destroy(tofmlem_ctx *ctx);
 int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value);
 /* sigma along the LOR in mm for this context (0 for non-TOF). */
 double tofmlem_sigma_mm(const tofmlem_ctx *ctx);
+/* Scratch memory.  The context allocates device scratch at first use and keeps it until tofmlem_destroy: the
+ * correction image of tofmlem_iterate (4 B per voxel), the histogram of tofmlem_bin_events (8 B per locality bin and
+ * sub-bin, 1 B per event), the records of tofmlem_permute_events (32 B per event), the event copies of
+ * tofmlem_reconstruct_regions (64 B per event), the staging buffers of tofmlem_iterate_host.  cudaMalloc inside a
+ * call synchronises the device, so a caller who times calls or runs several contexts concurrently reserves first:
+ * tofmlem_reserve allocates what iterate / bin_events / permute_events need for up to n_events events under the
+ * context's CURRENT options (call it after tofmlem_set_option).  tofmlem_trim SYNCHRONISES and releases every
+ * per-event scratch buffer (they are allocated again on demand); ENOMEM / ECUDA as usual. */
+int tofmlem_reserve(tofmlem_ctx *ctx, uint64_t n_events);
+int tofmlem_trim(tofmlem_ctx *ctx);
 
 /* Sensitivity image (north_star; R10): d_sens[j] = (1/m) sum_i l_ij over m detector-pair LORs
  * (non-TOF chords over the whole grid).  d_sens (nvox floats) is overwritten.  lors->dt is ignored. */

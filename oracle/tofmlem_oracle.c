@@ -34,7 +34,8 @@
  * Pins (tests/test_oracle_pins.py): P1 sigma; P2 uniform-box line integral = analytic chord;
  * P3 axis-aligned / diagonal chords; P4 TOF weights sum to erf(3/sqrt 2); P5 closed-form weights;
  * P6 sigma->inf reduces to non-TOF; P7 sum(x*sens)=n_valid; P8 one-voxel MLEM; P9 brute-force
- * quadrature on 8^3; P10 adjointness; P11 region partition 200+8x100; P12 hand-built keys.
+ * quadrature on 8^3; P10 adjointness; P11 region partition 200+8x100; P12 hand-built keys;
+ * P17 the float32 mask rule (orc_mask_f32) on a hand-written array with the expected bytes typed in.
  * Unpinned: the image after N iterations on realistic data has no independent pin beyond
  * P7/P8/P10 ("parity unpinned" for image values on realistic data is NOT claimed pinned);
  * split-vs-unsplit agreement is parity unpinned (PAPER.md:212 is visual only).

@@ -165,6 +165,52 @@ int ensure_corr(tofmlem_ctx *ctx) {
     return TOFMLEM_OK;
 }
 
+// Scratch of tofmlem_bin_events: fine histogram, cursors and scan space for `nfine` counters, one sub-bin byte per
+// event (n_sub = 0: none).  Grows only; cudaFree synchronises the device, so no launch can still be using the old one.
+int ensure_bin_scratch(tofmlem_ctx *ctx, size_t nfine, uint64_t n_sub) {
+    if (ctx->hist_cap < nfine) {
+        cudaFree(ctx->d_hist);
+        cudaFree(ctx->d_cursor);
+        cudaFree(ctx->d_scan_tmp);
+        ctx->d_hist = ctx->d_cursor = ctx->d_scan_tmp = nullptr;
+        ctx->hist_cap = 0;
+        CU(cudaMalloc(&ctx->d_hist, nfine * sizeof(uint32_t)));
+        CU(cudaMalloc(&ctx->d_cursor, nfine * sizeof(uint32_t)));
+        CU(cudaMalloc(&ctx->d_scan_tmp, (size_t)scan_tmp_elems((uint32_t)nfine) * sizeof(uint32_t)));
+        ctx->hist_cap = nfine;
+    }
+    if (ctx->sub_cap < n_sub) {
+        cudaFree(ctx->d_sub);
+        ctx->d_sub = nullptr;
+        ctx->sub_cap = 0;
+        CU(cudaMalloc(&ctx->d_sub, n_sub));
+        ctx->sub_cap = n_sub;
+    }
+    return TOFMLEM_OK;
+}
+
+// 32-byte event records of tofmlem_permute_events (grows only).  false: not enough memory (the caller falls back).
+bool ensure_pack(tofmlem_ctx *ctx, uint64_t n) {
+    if (ctx->pack_cap >= n) return true;
+    cudaFree(ctx->d_pack);
+    ctx->d_pack = nullptr;
+    ctx->pack_cap = 0;
+    if (cudaMalloc(&ctx->d_pack, n * 8 * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    ctx->pack_cap = n;
+    return true;
+}
+
+// number of sub-bins tofmlem_bin_events uses for a sorting call (the fine histogram must fit 32-bit indices)
+uint32_t effective_subbins(const tofmlem_ctx *c) {
+    uint32_t S = (uint32_t)c->subbins;
+    const uint32_t nb = num_bins(c);
+    while (S > 1 && (uint64_t)nb * S + 1 > 0x7FFFFFFFull) S >>= 1;
+    return S;
+}
+
 void default_region_slices(int nz, int R, std::vector<int32_t> &k) {
     k.resize(R + 1);
     k[0] = 0;
@@ -392,12 +438,59 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             if (value < 1 || value > 64 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "subbins in 1..64");
             ctx->subbins = (int)value;
             return TOFMLEM_OK;
+        case TOFMLEM_OPT_DETERMINISTIC:
+            // the paper's LUT kernel "always generated an identically reconstructed image".  Here the
+            // accumulation is a float32 reduction at L2 / in shared memory whose order is not fixed, so a run-to-run
+            // bit-identical image cannot be promised: the key exists, 0 is accepted, 1 is refused.
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "deterministic is 0 or 1");
+            if (value == 1.0)
+                return fail(ctx, TOFMLEM_EUNSUPPORTED,
+                            "deterministic accumulation is not available: float32 reductions are unordered");
+            return TOFMLEM_OK;
         default:
             return fail(ctx, TOFMLEM_EINVAL, "unknown option key");
     }
 }
 
 double tofmlem_sigma_mm(const tofmlem_ctx *ctx) { return ctx ? ctx->sigma : 0.0; }
+
+int tofmlem_reserve(tofmlem_ctx *ctx, uint64_t n_events) {
+    if (!ctx || n_events > 0xFFFFFFFFull) return TOFMLEM_EINVAL;
+    int rc = ensure_corr(ctx);
+    if (rc) return rc;
+    if (n_events) {
+        const uint32_t S = effective_subbins(ctx);
+        rc = ensure_bin_scratch(ctx, (size_t)num_bins(ctx) * S + 1, S > 1 ? n_events : 0);
+        if (rc) return rc;
+        if (!ensure_pack(ctx, n_events)) return fail(ctx, TOFMLEM_ENOMEM, "reserve: no memory for the 32-byte event records");
+    }
+    return TOFMLEM_OK;
+}
+
+int tofmlem_trim(tofmlem_ctx *ctx) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->copy_stream) CU(cudaStreamSynchronize(ctx->copy_stream));
+    cudaFree(ctx->d_pack);
+    cudaFree(ctx->d_sub);
+    cudaFree(ctx->d_rg_region);
+    cudaFree(ctx->d_rg_perm);
+    cudaFree(ctx->d_rg_sorted);
+    cudaFree(ctx->d_rg_binned);
+    cudaFree(ctx->d_tmp_image);
+    cudaFree(ctx->d_hev);
+    cudaFree(ctx->d_himg);
+    cudaFree(ctx->d_hsens);
+    ctx->d_pack = nullptr;
+    ctx->d_sub = nullptr;
+    ctx->d_rg_region = nullptr;
+    ctx->d_rg_perm = nullptr;
+    ctx->d_rg_sorted = ctx->d_rg_binned = nullptr;
+    ctx->d_tmp_image = nullptr;
+    ctx->d_hev = ctx->d_himg = ctx->d_hsens = nullptr;
+    ctx->pack_cap = ctx->sub_cap = ctx->rg_cap = ctx->hev_cap = 0;
+    return TOFMLEM_OK;
+}
 
 int tofmlem_sensitivity(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t m, float *d_sens) {
     if (!ctx) return TOFMLEM_EINVAL;
@@ -637,28 +730,10 @@ int tofmlem_bin_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, u
     const uint32_t nb = num_bins(ctx);
     const bool sort = d_perm != nullptr;
     // sub-bins only matter for the permutation; the fine histogram must still fit 32-bit indices
-    uint32_t S = sort ? (uint32_t)ctx->subbins : 1u;
-    while (S > 1 && (uint64_t)nb * S + 1 > 0x7FFFFFFFull) S >>= 1;
+    const uint32_t S = sort ? effective_subbins(ctx) : 1u;
     const size_t nfine = (size_t)nb * S + 1;
-    if (ctx->hist_cap < nfine) {
-        cudaFree(ctx->d_hist);
-        cudaFree(ctx->d_cursor);
-        cudaFree(ctx->d_scan_tmp);
-        ctx->d_hist = ctx->d_cursor = ctx->d_scan_tmp = nullptr;
-        ctx->hist_cap = 0;
-        CU(cudaMalloc(&ctx->d_hist, nfine * sizeof(uint32_t)));
-        CU(cudaMalloc(&ctx->d_cursor, nfine * sizeof(uint32_t)));
-        CU(cudaMalloc(&ctx->d_scan_tmp, (size_t)scan_tmp_elems((uint32_t)nfine) * sizeof(uint32_t)));
-        ctx->hist_cap = nfine;
-    }
-    if (S > 1 && ctx->sub_cap < n) {
-        cudaFree(ctx->d_sub);
-    cudaFree(ctx->d_pack);
-        ctx->d_sub = nullptr;
-        ctx->sub_cap = 0;
-        CU(cudaMalloc(&ctx->d_sub, n));
-        ctx->sub_cap = n;
-    }
+    int rc = ensure_bin_scratch(ctx, nfine, S > 1 ? n : 0);
+    if (rc) return rc;
     SubBin sb;
     sb.S = S;
     sb.half_window = ctx->tof ? (float)(ctx->trunc_sigmas * ctx->sigma) : 0.0f;
@@ -705,14 +780,7 @@ static int gather_events_impl(tofmlem_ctx *ctx, const tofmlem_events *in, const 
     // kept by the context until tofmlem_destroy), gather one sector per event instead of one per member
     // (measured at 146 M events: 19.5 -> 5.2 ms).
     if (full_permutation && (src[6] != nullptr) == (dst[6] != nullptr)) {
-        if (ctx->pack_cap < n) {
-            cudaFree(ctx->d_pack);
-            ctx->d_pack = nullptr;
-            ctx->pack_cap = 0;
-            if (cudaMalloc(&ctx->d_pack, n * 8 * sizeof(float)) == cudaSuccess) ctx->pack_cap = n;
-            else cudaGetLastError();  // not enough memory for the records: member-by-member gathers below
-        }
-        if (ctx->pack_cap >= n) {
+        if (ensure_pack(ctx, n)) {  // else not enough memory for the records: member-by-member gathers below
             launch_gather_packed(ev_ptrs(in), d_perm, n, ctx->d_pack, dst, ctx->stream);
             CHECK_LAUNCH(2);
             return TOFMLEM_OK;

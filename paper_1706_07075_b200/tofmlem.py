@@ -24,6 +24,7 @@ OPT_SUBBINS = 9
 OPT_MEDIAN = 10
 OPT_CACHE_SHARE = 11
 OPT_CORR_BRICKS = 12
+OPT_DETERMINISTIC = 13
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
@@ -34,7 +35,7 @@ SYMBOLS = (
     "tofmlem_split_regions", "tofmlem_region_zbounds", "tofmlem_region_grid", "tofmlem_reconstruct_regions",
     "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
     "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
-    "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events",
+    "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events", "tofmlem_reserve", "tofmlem_trim",
 )
 
 
@@ -147,6 +148,12 @@ class Context:
 
     def sigma_mm(self) -> float:
         return float(self._L.tofmlem_sigma_mm(self._h))
+
+    def reserve(self, n_events: int):
+        self._check(self._L.tofmlem_reserve(self._h, C.c_uint64(n_events)))
+
+    def trim(self):
+        self._check(self._L.tofmlem_trim(self._h))
 
     def sensitivity(self, lors: Dict[str, torch.Tensor], m: int, sens: torch.Tensor):
         e = _events({**lors, "dt": None}, m)

@@ -433,3 +433,34 @@ def test_bin_keys_in_range_on_synthetic_events():
     T = 20 * 20 * 80
     assert oracle.num_bins(g) == 12 * T and key.max() < 12 * T
     assert len(np.unique(key // T)) == 12  # the long scanner accepts every direction class
+
+
+# ---------------------------------------------------------------- P17
+def test_p17_mask_rule_float32():
+    """R11: mask_j = (sens_j >= floor_rel * max_k sens_k) and sens_j > 0, decided in FLOAT32, default
+    floor 1e-2.  The expected bytes below are typed by hand from IEEE binary32 arithmetic, not computed by any code:
+      max = 100 -> thr = fl32(0.01f * 100f): 0.01f = 0.00999999977648..., the product 0.99999997765 lies between the
+      neighbouring floats 0.99999994 and 1.0 and rounds to 1.0f exactly;
+      max = 3 -> thr = fl32(0.01f * 3f) = 0.0299999993294... = 0.03f, whereas a double-precision threshold 0.01 * 3.0
+      = 0.03 > 0.03f would reject the voxel that holds 0.03f."""
+    one = np.float32(1.0)
+    below, above = np.nextafter(one, np.float32(0.0)), np.nextafter(one, np.float32(2.0))
+    sens = np.array([100.0, 1.0, below, above, 0.0, -5.0, np.nan, 0.5, 2.0, -0.0, 99.0],
+                    np.float32)
+    #                100   at  below  above  0   neg  NaN  0.5  2.0  -0   99
+    want = np.array([1,    1,  0,     1,     0,  0,   0,   0,   1,   0,   1], np.uint8)
+    assert np.array_equal(oracle.mask_f32(sens), want)  # default floor_rel = 1e-2
+    assert np.array_equal(oracle.mask_f32(sens, 1e-2), want)
+    # '>' instead of '>=' would drop element 1; a threshold taken relative to the mean or the sum instead of the max
+    # would move it far from 1.0 and flip elements 7 and 8.
+    # float32 product, not double: the voxel holding exactly 0.03f survives with max = 3
+    s3 = np.array([3.0, np.float32(0.03), np.nextafter(np.float32(0.03), np.float32(0.0))], np.float32)
+    assert np.array_equal(oracle.mask_f32(s3), np.array([1, 1, 0], np.uint8))
+    # another floor: 0.5 * 100 = 50 exactly
+    assert np.array_equal(oracle.mask_f32(sens, 0.5), np.array([1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1], np.uint8))
+    # floor 0 keeps every strictly positive voxel and nothing else (sens > 0 is part of the rule)
+    assert np.array_equal(oracle.mask_f32(sens, 0.0), np.array([1, 1, 1, 1, 0, 0, 0, 1, 1, 0, 1], np.uint8))
+    # all-zero sensitivity: max = 0 -> thr = 0, and 0 >= 0 must NOT make a voxel exist
+    assert not oracle.mask_f32(np.zeros(7, np.float32)).any()
+    # the maximum is taken over the whole array, wherever it sits (last element here)
+    assert np.array_equal(oracle.mask_f32(np.array([0.9, 1.0, 100.0], np.float32)), np.array([0, 1, 1], np.uint8))
