@@ -67,7 +67,18 @@ typedef struct {
     double sum_image_sens; /* sum_j image_j * sens_j after the last tofmlem_iterate (= n_valid, P7) */
     uint64_t reductions;   /* reduction instructions (scalar or 16-byte) the scatter walk of that pass sent to the L2
                               atomic units: the unit of the l2_atomic roofline */
+    uint64_t tile_events;  /* of n_valid: events accumulated through a shared-memory tile (tofmlem_plan_events) */
+    uint64_t tile_oob;     /* TOFMLEM_OPT_TILE_CHECK: tile accesses found out of range; must be 0 */
 } tofmlem_stats;
+
+/* What tofmlem_plan_events decided (tofmlem_plan_info). */
+typedef struct {
+    int32_t active;           /* 1: the fused pass of the planned list runs in tile mode */
+    int32_t sorted;           /* 1: the list was sorted by locality key */
+    uint32_t n_tile_items;    /* pieces of locality bins that are accumulated in shared-memory tiles */
+    uint32_t n_direct_chunks; /* 32-event pieces left to the direct pass */
+    uint64_t n_tile_events, n_direct_events;
+} tofmlem_plan;
 
 /* Option keys for tofmlem_set_option. */
 enum {
@@ -97,6 +108,11 @@ enum {
                                        shared-memory write-back cache (0..8); the others reduce at L2 directly */
     TOFMLEM_OPT_MEDIAN = 10,        /* 1: tofmlem_iterate applies the 3x3x3 median filter to the image estimate after
                                        every update (R23); default 0 */
+    TOFMLEM_OPT_TILE_MIN_EVENTS = 14, /* tofmlem_plan_events: a locality bin with at least this many events is
+                                       accumulated in a shared-memory tile (default 1024; performance only) */
+    TOFMLEM_OPT_TILE_MAX_EVENTS = 16, /* ... in pieces of at most this many events per CTA (default 8192) */
+    TOFMLEM_OPT_TILE_CHECK = 15,    /* 1: bounds-test every access to the shared-memory tiles and count violations in
+                                       tofmlem_stats.tile_oob (a debugging aid; default 0) */
     TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
                                        generated an identically reconstructed image").  0 (default) is accepted; 1
                                        returns TOFMLEM_EUNSUPPORTED: the correction image is summed with float32
@@ -147,6 +163,19 @@ int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, 
  * Updates the context's n_valid / visits counters (reset them with tofmlem_reset_stats). */
 int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr);
 int tofmlem_reset_stats(tofmlem_ctx *ctx);
+
+/* Tile mode of the fused pass (north_star bullet 4: "shared-memory tile accumulation rather than naive global atomics";
+ * the paper's "direct technique for voxel filling").  ev must be a list sorted by locality key (the
+ * output of tofmlem_bin_events + tofmlem_permute_events) on a TOF context with the Siddon projector.  The call looks at
+ * the keys once and remembers, for THIS list (its x1 pointer and n), which bins are populous enough to be walked with
+ * the image and the correction image of the bin's +-T sigma neighbourhood held in shared memory; later
+ * tofmlem_em_correction[_weighted] / tofmlem_iterate[_weighted] calls with the same list run those bins in tile mode
+ * and the remaining events through the direct pass.  Results are the same up to the order of the float32 sums.  The
+ * plan is an optimisation only: every event is checked against its tile inside the kernel, so a list that was changed
+ * in place after the call still gives correct results.  A list that is not sorted, a non-TOF context or a window whose
+ * tiles do not fit in shared memory leave the plan inactive (no error).  Replaces any earlier plan.  SYNCHRONISES. */
+int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n);
+int tofmlem_plan_info(const tofmlem_ctx *ctx, tofmlem_plan *h_out);
 
 /* Multiplicative update (R1, R11): d_image[j] = mask_j ? d_image[j] * d_corr[j] / d_sens[j] : 0 with
  * mask_j = d_sens[j] >= sens_floor_rel * max_k d_sens[k] (and d_sens[j] > 0), decided in float32.

@@ -11,6 +11,7 @@
 using namespace tofmlem;
 
 struct tofmlem_ctx {
+    tofmlem_ctx() { memset(&h_geom_sent, 0xff, sizeof h_geom_sent); }
     tofmlem_scanner scanner;
     tofmlem_grid grid;
     bool tof;
@@ -57,6 +58,26 @@ struct tofmlem_ctx {
     cudaEvent_t chunk_done[2] = {nullptr, nullptr};
     uint64_t last_n = 0;
     uint64_t launches = 0;
+    // tile-mode plan of the fused pass (tofmlem_plan_events; tile.cu)
+    int tile_min_events = 1024, tile_max_events = 8192, tile_check = 0;
+    int n_sm = 0;
+    size_t smem_optin = 0;  // largest dynamic shared memory a CTA may opt in to on this device
+    TileGeom *d_geom = nullptr;
+    TileGeom h_geom_sent;   // what d_geom currently holds (valid when d_geom != nullptr)
+    TileItem *d_items = nullptr;
+    size_t items_cap = 0;
+    uint2 *d_chunks = nullptr;
+    size_t chunks_cap = 0;
+    unsigned *d_plan_flags = nullptr;  // [0] tile work counter, [1] "keys not sorted" flag
+    struct {
+        bool valid = false;
+        const float *x1 = nullptr;  // the plan describes THIS event list (first member array) ...
+        uint64_t n = 0;             // ... of this length, binned with
+        int tile_log2 = 0;          // ... this cube size
+        uint32_t n_items = 0, n_chunks = 0;
+        uint64_t tile_events = 0, direct_events = 0;
+        int sorted = 0;
+    } plan;
     std::string err;
 };
 
@@ -268,6 +289,31 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         int rc = ensure_lut(ctx);
         if (rc) return rc;
         launch_sampled_em(p, ctx->d_lut, ctx->samples_k, ev, n, evw, d_image, d_corr, ctx->d_stats, ctx->d_queues, s);
+    } else if (ctx->plan.valid && ctx->plan.x1 == ev.x1 && ctx->plan.n == n && ctx->plan.tile_log2 == ctx->tile_log2 &&
+               ctx->tof && vec && ctx->em_variant == 0 && ctx->plan.n_items > 0) {
+        // Tile mode (tile.cu): the list is the one tofmlem_plan_events looked at.  The geometry of the tiles follows the
+        // CURRENT window (trunc_sigmas may have changed since the plan, which only depends on the keys).
+        TileGeom g;
+        build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);
+        if (!g.ok) {
+            launch_em_correction(p, ctx->tof, ev, n, evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, s);
+            CHECK_LAUNCH(1);
+            return TOFMLEM_OK;
+        }
+        if (!ctx->d_geom) CU(cudaMalloc(&ctx->d_geom, sizeof(TileGeom)));
+        if (memcmp(&g, &ctx->h_geom_sent, sizeof g) != 0) {
+            ctx->h_geom_sent = g;
+            CU(cudaMemcpyAsync(ctx->d_geom, &ctx->h_geom_sent, sizeof g, cudaMemcpyHostToDevice, s));
+        }
+        launch_em_tile(p, g, ctx->d_geom, ctx->tile_log2, ev, evw, d_image, d_corr, ctx->d_stats, ctx->d_items,
+                       ctx->plan.n_items, ctx->d_plan_flags, ctx->n_sm > 0 ? ctx->n_sm : 1, ctx->tile_check != 0, s);
+        CHECK_LAUNCH(1);
+        if (ctx->plan.n_chunks) {
+            launch_em_correction_chunks(p, true, ev, n, ctx->d_chunks, ctx->plan.n_chunks, evw, d_image, d_corr, vec,
+                                        ctx->d_stats, ctx->d_queues, s);
+            CHECK_LAUNCH(1);
+        }
+        return TOFMLEM_OK;
     } else {
         launch_em_correction(p, ctx->tof, ev, n, evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, s);
     }
@@ -295,7 +341,7 @@ int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, const floa
     }
     CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
     for (int it = 0; it < iters; ++it) {
-        CU(cudaMemsetAsync(ctx->d_stats, 0, 3 * sizeof(unsigned long long), ctx->stream));
+        CU(cudaMemsetAsync(ctx->d_stats, 0, kStatsCounters * sizeof(unsigned long long), ctx->stream));
         rc = em_pass(ctx, p, ev, n, evw, d_image, ctx->d_corr, true, ctx->stream);
         if (rc) return rc;
         update_any(ctx, d_image, ctx->d_corr, d_sens, dmax, ctx->stream);
@@ -335,10 +381,19 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
     ctx->sigma = ctx->tof ? sigma_from_fwhm(tof_fwhm_ps) : 0.0;
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->nvox = nvox;
+    {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) {
+            if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) ctx->n_sm = v;
+            if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess) ctx->smem_optin = (size_t)v;
+        }
+        cudaGetLastError();
+    }
     cudaError_t e = cudaMalloc(&ctx->d_max, sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, sizeof(DeviceStats));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_queues, kMaxQueues * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_rcounts, 2 * (kMaxRegions + 1) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_flags, 2 * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_stats, 0, sizeof(DeviceStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_max, 0, sizeof(float), ctx->stream);
     if (e != cudaSuccess) {
@@ -347,6 +402,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
         cudaFree(ctx->d_stats);
         cudaFree(ctx->d_queues);
         cudaFree(ctx->d_rcounts);
+        cudaFree(ctx->d_plan_flags);
         delete ctx;
         return rc;
     }
@@ -382,6 +438,10 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_hev);
     cudaFree(ctx->d_himg);
     cudaFree(ctx->d_hsens);
+    cudaFree(ctx->d_plan_flags);
+    cudaFree(ctx->d_geom);
+    cudaFree(ctx->d_items);
+    cudaFree(ctx->d_chunks);
     delete ctx;
     return TOFMLEM_OK;
 }
@@ -437,6 +497,18 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
         case TOFMLEM_OPT_SUBBINS:
             if (value < 1 || value > 64 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "subbins in 1..64");
             ctx->subbins = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_TILE_MIN_EVENTS:
+            if (value < 1 || value > 1e9 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "tile_min_events in 1..1e9");
+            ctx->tile_min_events = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_TILE_MAX_EVENTS:
+            if (value < 32 || value > 1e9 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "tile_max_events in 32..1e9");
+            ctx->tile_max_events = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_TILE_CHECK:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "tile_check is 0 or 1");
+            ctx->tile_check = (int)value;
             return TOFMLEM_OK;
         case TOFMLEM_OPT_DETERMINISTIC:
             // the paper's LUT kernel "always generated an identically reconstructed image".  Here the
@@ -699,7 +771,7 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
         CHECK_LAUNCH(1);
         if (ctx->median && (rc = median_in_place(ctx, ctx->d_himg, s))) return rc;
         for (int it = 1; it < iters; ++it) {
-            CU(cudaMemsetAsync(ctx->d_stats, 0, 3 * sizeof(unsigned long long), s));
+            CU(cudaMemsetAsync(ctx->d_stats, 0, kStatsCounters * sizeof(unsigned long long), s));
             rc = em_pass(ctx, p, ev_ptrs(&dev), n, nullptr, ctx->d_himg, ctx->d_corr, true, s);
             if (rc) return rc;
             update_any(ctx, ctx->d_himg, ctx->d_corr, ctx->d_hsens, ctx->d_max, s);
@@ -717,6 +789,106 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
     CU(cudaMemcpyAsync(h_image, ctx->d_himg, vbytes, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     ctx->last_n = n;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    ctx->plan.valid = false;
+    ctx->plan.n_items = ctx->plan.n_chunks = 0;
+    ctx->plan.tile_events = ctx->plan.direct_events = 0;
+    ctx->plan.sorted = 0;
+    if (n == 0) return TOFMLEM_OK;
+    if (!ev_ok(ev, ctx->tof) || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "plan_events: bad argument");
+    if (!ctx->tof || ctx->projector != 0) return TOFMLEM_OK;  // tile mode exists for the TOF Siddon pass only
+    {
+        TileGeom g;
+        build_tile_geom(make_params(ctx, true), ctx->tile_log2, ctx->smem_optin, g);
+        if (!g.ok) return TOFMLEM_OK;  // the tiles of this window do not fit in shared memory: direct pass
+    }
+    const uint32_t nb = num_bins(ctx);
+    int rc = ensure_bin_scratch(ctx, (size_t)nb + 1, 0);
+    if (rc) return rc;
+    cudaStream_t s = ctx->stream;
+    CU(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)nb + 1) * sizeof(uint32_t), s));
+    CU(cudaMemsetAsync(ctx->d_plan_flags, 0, 2 * sizeof(unsigned), s));
+    launch_plan_hist(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, ctx->d_hist, nb, ctx->d_plan_flags + 1, s);
+    CHECK_LAUNCH(1);
+    std::vector<uint32_t> cnt(nb);
+    unsigned flags[2] = {0, 0};
+    CU(cudaMemcpyAsync(cnt.data(), ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    CU(cudaMemcpyAsync(flags, ctx->d_plan_flags, sizeof flags, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    ctx->plan.sorted = flags[1] ? 0 : 1;
+    if (flags[1]) return TOFMLEM_OK;  // not sorted by key: the bins are not contiguous, direct pass
+    // bins with at least tile_min_events events become tile work (pieces of at most tile_max_events, whole warps);
+    // maximal runs of the other bins are cut into 32-event pieces for the direct pass
+    std::vector<TileItem> items;
+    std::vector<uint2> chunks;
+    const uint32_t thr = (uint32_t)ctx->tile_min_events, mx = (uint32_t)ctx->tile_max_events;
+    uint64_t off = 0, run_lo = 0, run_hi = 0, n_tile = 0, n_direct = 0;
+    auto flush_run = [&]() {
+        for (uint64_t a = run_lo; a < run_hi; a += 32)
+            chunks.push_back(make_uint2((unsigned)a, (unsigned)(run_hi - a < 32 ? run_hi - a : 32)));
+        n_direct += run_hi - run_lo;
+        run_lo = run_hi = 0;
+    };
+    for (uint32_t b = 0; b < nb; ++b) {
+        const uint32_t c = cnt[b];
+        if (c == 0) continue;
+        if (c >= thr) {
+            if (run_hi > run_lo) flush_run();
+            const uint32_t pieces = (c + mx - 1) / mx;
+            uint32_t per = (c + pieces - 1) / pieces;
+            per = (per + 31u) & ~31u;
+            for (uint32_t a = 0; a < c; a += per)
+                items.push_back(TileItem{(uint32_t)(off + a), c - a < per ? c - a : per, b, 0u});
+            n_tile += c;
+        } else {
+            if (run_hi == run_lo) run_lo = off;
+            run_hi = off + c;
+        }
+        off += c;
+    }
+    if (run_hi > run_lo) flush_run();
+    if (items.empty()) return TOFMLEM_OK;
+    if (ctx->items_cap < items.size()) {
+        cudaFree(ctx->d_items);
+        ctx->d_items = nullptr;
+        ctx->items_cap = 0;
+        CU(cudaMalloc(&ctx->d_items, items.size() * sizeof(TileItem)));
+        ctx->items_cap = items.size();
+    }
+    if (ctx->chunks_cap < chunks.size()) {
+        cudaFree(ctx->d_chunks);
+        ctx->d_chunks = nullptr;
+        ctx->chunks_cap = 0;
+        CU(cudaMalloc(&ctx->d_chunks, chunks.size() * sizeof(uint2)));
+        ctx->chunks_cap = chunks.size();
+    }
+    CU(cudaMemcpyAsync(ctx->d_items, items.data(), items.size() * sizeof(TileItem), cudaMemcpyHostToDevice, s));
+    if (!chunks.empty())
+        CU(cudaMemcpyAsync(ctx->d_chunks, chunks.data(), chunks.size() * sizeof(uint2), cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
+    ctx->plan.valid = true;
+    ctx->plan.x1 = ev->x1;
+    ctx->plan.n = n;
+    ctx->plan.tile_log2 = ctx->tile_log2;
+    ctx->plan.n_items = (uint32_t)items.size();
+    ctx->plan.n_chunks = (uint32_t)chunks.size();
+    ctx->plan.tile_events = n_tile;
+    ctx->plan.direct_events = n_direct;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_plan_info(const tofmlem_ctx *ctx, tofmlem_plan *h_out) {
+    if (!ctx || !h_out) return TOFMLEM_EINVAL;
+    h_out->active = ctx->plan.valid ? 1 : 0;
+    h_out->sorted = ctx->plan.sorted;
+    h_out->n_tile_items = ctx->plan.n_items;
+    h_out->n_direct_chunks = ctx->plan.n_chunks;
+    h_out->n_tile_events = ctx->plan.tile_events;
+    h_out->n_direct_events = ctx->plan.direct_events;
     return TOFMLEM_OK;
 }
 
@@ -1037,6 +1209,8 @@ int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out) {
     h_out->n_skipped = ctx->last_n >= h.n_valid ? ctx->last_n - h.n_valid : 0;
     h_out->visits = h.visits;
     h_out->reductions = h.reds;
+    h_out->tile_events = h.tile_events;
+    h_out->tile_oob = h.tile_oob;
     h_out->sum_image_sens = h.sum_image_sens;
     return TOFMLEM_OK;
 }

@@ -87,6 +87,30 @@ __device__ __forceinline__ int predicted_visits(const GridF32 &g, const SubBin &
     return visits;
 }
 
+// Locality key of one event per F1: dirclass * (Tx Ty Tz) + tile of the TOF centre; 0xFFFFFFFF for an invalid event.
+// d receives the float32 direction p2 - p1.
+__device__ __forceinline__ uint32_t event_key(const GridF32 &g, int tile_log2, uint32_t Tx, uint32_t Ty, uint32_t Tz,
+                                              const EventPtrs &ev, uint64_t e, float d[3]) {
+    float c[3];
+    if (!tof_centre(ev, e, c, d)) return 0xFFFFFFFFu;
+    const int ix = centre_voxel(c[0], g.ox, g.vx, g.nx);
+    const int iy = centre_voxel(c[1], g.oy, g.vy, g.ny);
+    const int iz = centre_voxel(c[2], g.oz, g.vz, g.nz);
+    const uint32_t tile =
+        (((uint32_t)(iz >> tile_log2)) * Ty + (uint32_t)(iy >> tile_log2)) * Tx + (uint32_t)(ix >> tile_log2);
+    int a = 0;
+    float best = fabsf(d[0]);
+    if (fabsf(d[1]) > best) { a = 1; best = fabsf(d[1]); }
+    if (fabsf(d[2]) > best) { a = 2; }
+    const float da = a == 0 ? d[0] : (a == 1 ? d[1] : d[2]);
+    const float db0 = a == 0 ? d[1] : (a == 1 ? d[2] : d[0]);
+    const float dc0 = a == 0 ? d[2] : (a == 1 ? d[0] : d[1]);
+    const bool neg = da < 0.0f;
+    const float db = neg ? -db0 : db0, dc = neg ? -dc0 : dc0;
+    const uint32_t dirclass = 4u * (uint32_t)a + 2u * (db < 0.0f ? 1u : 0u) + (dc < 0.0f ? 1u : 0u);
+    return dirclass * (Tx * Ty * Tz) + tile;
+}
+
 // key (F1) of every event; with `sub` also the sub-bin (events of one locality bin ordered by predicted visit count,
 // so that the 32 events of a warp run loops of nearly equal length) and the histogram of the fine key
 // key * sb.S + sub (invalid events: the last fine bin).
@@ -99,30 +123,12 @@ __global__ void __launch_bounds__(kBlock) bin_keys_kernel(GridF32 g, int tile_lo
     const int t = 1 << tile_log2;
     const uint32_t Tx = (uint32_t)((g.nx + t - 1) >> tile_log2), Ty = (uint32_t)((g.ny + t - 1) >> tile_log2),
                    Tz = (uint32_t)((g.nz + t - 1) >> tile_log2);
-    float c[3], d[3];
-    uint32_t k = 0xFFFFFFFFu;
+    float d[3];
+    const uint32_t k = event_key(g, tile_log2, Tx, Ty, Tz, ev, e, d);
     uint32_t sbin = 0;
-    if (tof_centre(ev, e, c, d)) {
-        const int ix = centre_voxel(c[0], g.ox, g.vx, g.nx);
-        const int iy = centre_voxel(c[1], g.oy, g.vy, g.ny);
-        const int iz = centre_voxel(c[2], g.oz, g.vz, g.nz);
-        const uint32_t tile =
-            (((uint32_t)(iz >> tile_log2)) * Ty + (uint32_t)(iy >> tile_log2)) * Tx + (uint32_t)(ix >> tile_log2);
-        int a = 0;
-        float best = fabsf(d[0]);
-        if (fabsf(d[1]) > best) { a = 1; best = fabsf(d[1]); }
-        if (fabsf(d[2]) > best) { a = 2; }
-        const float da = a == 0 ? d[0] : (a == 1 ? d[1] : d[2]);
-        const float db0 = a == 0 ? d[1] : (a == 1 ? d[2] : d[0]);
-        const float dc0 = a == 0 ? d[2] : (a == 1 ? d[0] : d[1]);
-        const bool neg = da < 0.0f;
-        const float db = neg ? -db0 : db0, dc = neg ? -dc0 : dc0;
-        const uint32_t dirclass = 4u * (uint32_t)a + 2u * (db < 0.0f ? 1u : 0u) + (dc < 0.0f ? 1u : 0u);
-        k = dirclass * (Tx * Ty * Tz) + tile;
-        if (sub) {
-            const int vis = predicted_visits(g, sb, ev, e, d);
-            sbin = vis <= 0 ? 0u : min(sb.S - 1u, 1u + (uint32_t)vis / sb.quantum);
-        }
+    if (k != 0xFFFFFFFFu && sub) {
+        const int vis = predicted_visits(g, sb, ev, e, d);
+        sbin = vis <= 0 ? 0u : min(sb.S - 1u, 1u + (uint32_t)vis / sb.quantum);
     }
     key[e] = k;
     if (sub) sub[e] = (uint8_t)sbin;
@@ -349,6 +355,33 @@ __global__ void __launch_bounds__(kBlock) scatter_keep_kernel(EventPtrs ev, uint
 }
 
 static inline unsigned grid_for(uint64_t n) { return (unsigned)((n + kBlock - 1) / kBlock); }
+
+// Plan of the tile-mode EM pass (tile.cu): histogram of the keys of an event list that is expected to be sorted by
+// key already (the output of tofmlem_bin_events + tofmlem_permute_events), and a flag that says whether it is.
+__global__ void __launch_bounds__(kBlock) plan_hist_kernel(GridF32 g, int tile_log2, EventPtrs ev, uint64_t n,
+                                                           uint32_t *__restrict__ hist, uint32_t nbins,
+                                                           unsigned *__restrict__ unsorted) {
+    __shared__ uint32_t keys[kBlock + 1];
+    const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    const int t = 1 << tile_log2;
+    const uint32_t Tx = (uint32_t)((g.nx + t - 1) >> tile_log2), Ty = (uint32_t)((g.ny + t - 1) >> tile_log2),
+                   Tz = (uint32_t)((g.nz + t - 1) >> tile_log2);
+    float d[3];
+    uint32_t k = 0xFFFFFFFFu;
+    if (e < n) k = event_key(g, tile_log2, Tx, Ty, Tz, ev, e, d);
+    keys[threadIdx.x + 1] = k;
+    if (threadIdx.x == 0) keys[0] = e > 0 && e < n ? event_key(g, tile_log2, Tx, Ty, Tz, ev, e - 1, d) : 0u;
+    __syncthreads();
+    if (e >= n) return;
+    if (k < keys[threadIdx.x]) *unsorted = 1u;
+    if (k < nbins) atomicAdd(hist + k, 1u);
+}
+
+void launch_plan_hist(const GridF32 &g, int tile_log2, const EventPtrs &ev, uint64_t n, uint32_t *hist, uint32_t nbins,
+                      unsigned *unsorted, cudaStream_t s) {
+    if (n == 0) return;
+    plan_hist_kernel<<<(unsigned)((n + kBlock - 1) / kBlock), kBlock, 0, s>>>(g, tile_log2, ev, n, hist, nbins, unsorted);
+}
 
 void launch_bin_keys(const GridF32 &g, int tile_log2, const SubBin &sb, const EventPtrs &ev, uint64_t n, uint32_t *key,
                      uint8_t *sub, uint32_t *hist, uint32_t nbins, cudaStream_t s) {

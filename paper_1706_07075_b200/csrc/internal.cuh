@@ -34,8 +34,11 @@ struct DeviceStats {
     unsigned long long n_valid;
     unsigned long long visits;
     unsigned long long reds;  // reduction instructions (requests to the L2 atomic units) of the scatter walk
+    unsigned long long tile_events;  // valid events whose window was accumulated in a shared-memory tile (tile.cu)
+    unsigned long long tile_oob;     // TOFMLEM_OPT_TILE_CHECK: tile accesses found out of range (must stay 0)
     double sum_image_sens;
 };
+constexpr int kStatsCounters = 5;  // leading unsigned long long members, reset before every pass
 
 // float32 grid for the bit-exact key / region arithmetic (specification F1)
 struct GridF32 {
@@ -55,6 +58,40 @@ constexpr int kMaxQueues = 2048;
 void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *evw,
                           const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,
                           cudaStream_t s);
+
+// chunks (optional): the pass runs over a list of (first event, count <= 32) pieces instead of 0..n-1 (the events the
+// tile-mode pass leaves over); then n_chunks pieces are processed and `n` only bounds the event indices.
+void launch_em_correction_chunks(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const uint2 *chunks,
+                                 uint32_t n_chunks, const float *evw, const float *image, float *corr, bool vec_ok,
+                                 DeviceStats *stats, unsigned *queues, cudaStream_t s);
+
+// ---- tile.cu: fused EM pass with the image and the correction image of one locality bin held in shared memory
+constexpr int kTileMaxPlanes = 96;
+// Footprint of a locality bin (cube of T voxels, direction class with dominant axis a): the union of the +-T sigma
+// windows of all events whose TOF centre lies in the cube and whose direction is in the class is a double cone.  It is
+// stored plane by plane along a: plane p (p = i_a - cube origin + RA) holds a W[0] x W[1] rectangle of the two lateral
+// axes (fast axis f = the lower-numbered one, slow axis s) whose low corner, in cell coordinates mirrored so that the
+// class's rays run towards +f and +s, is (lo[0][p], lo[1][p]).
+struct TileGeom {
+    int T;                 // cube edge in voxels
+    int ok;                // tile mode is available for this context (all three dominant axes fit)
+    int RA[3], PA[3];      // planes below the cube / planes in all, per dominant axis
+    int W[3][2];           // rectangle width along f and s
+    int PS[3];             // words per plane (odd, >= W[0] * W[1])
+    int words;             // words of the largest tile: max PA * PS
+    signed char lo[3][2][kTileMaxPlanes];
+};
+struct TileItem {
+    uint32_t start, count, key, pad;  // events [start, start + count) of the sorted list, all with this key
+};
+// false (g.ok = 0) when a tile pair does not fit in `smem_budget` bytes of shared memory
+void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, TileGeom &g);
+size_t tile_smem_bytes(const TileGeom &g);
+// d_geom: the same structure in device memory
+void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const EventPtrs &ev,
+                    const float *evw, const float *image, float *corr, DeviceStats *stats, const TileItem *items,
+                    uint32_t n_items, unsigned *counter /* one word, zeroed by the call */, int n_sm, bool check,
+                    cudaStream_t s);
 
 // ---- image_ops.cu
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);
@@ -79,6 +116,9 @@ struct SubBin {
     uint32_t S, quantum;
     float half_window;  // trunc_sigmas * sigma (mm); 0 for non-TOF
 };
+void launch_plan_hist(const GridF32 &g, int tile_log2, const EventPtrs &ev, uint64_t n, uint32_t *hist /* zeroed */,
+                      uint32_t nbins, unsigned *unsorted /* zeroed; set to 1 when a key is below its predecessor's */,
+                      cudaStream_t s);
 void launch_bin_keys(const GridF32 &g, int tile_log2, const SubBin &sb, const EventPtrs &ev, uint64_t n, uint32_t *key,
                      uint8_t *sub /* n, or NULL */, uint32_t *hist /* nbins*S+1, zeroed by caller */, uint32_t nbins,
                      cudaStream_t s);

@@ -22,243 +22,12 @@
 #include <math.h>
 
 #include "internal.cuh"
+#include "walk.cuh"
 
 namespace tofmlem {
 
-struct Ray {
-    float t_end, tc;
-    float t0x, t0y, t0z;
-    float tdx, tdy, tdz;
-    int idx;            // flat index of the first voxel
-    int dxi, dyi, dzi;  // flat-index increments of a step along each axis, 0 when parallel
-    // brick layout of the correction image (2x2x1 voxels per 16-byte group, see ProjParams::brick):
-    int bidx;        // brick-layout index of the first voxel
-    int bdx0, bdxs;  // x step: increment for the first step, and the sum of the two alternating increments
-    int bdy0, bdys;  // y step: likewise
-};
-
-__device__ __forceinline__ float ex2_approx(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-__device__ __forceinline__ bool finite_f(float x) { return fabsf(x) <= 3.402823466e+38f; }  // false for NaN/Inf
-
-__device__ __forceinline__ void red_v4(float *p, float a, float b, float c, float d) {
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
-}
-
-__device__ __forceinline__ void red_v4_if(bool p, float *ptr, float a, float b, float c, float d) {
-    asm volatile(
-        "{\n .reg .pred q;\n setp.ne.s32 q, %5, 0;\n @q red.global.add.v4.f32 [%0], {%1, %2, %3, %4};\n}" ::"l"(ptr),
-        "f"(a), "f"(b), "f"(c), "f"(d), "r"((int)p)
-        : "memory");
-}
-
-constexpr float kBigT = 1.0e30f;
-
-// Per-axis set-up; returns the parameter at which the ray leaves the grid through this axis.
-__device__ __forceinline__ float axis_setup(double p1, double u, double s_lo, double o, double v, double iv, int n,
-                                            int stride, int &i, int &di, float &t0, float &td) {
-    const double q = (p1 + u * s_lo - o) * iv;
-    const double fl = floor(q);
-    int ii = (int)fl;
-    if (u < 0.0 && fl == q) ii -= 1;  // sitting exactly on a plane and moving down: the voxel below
-    ii = max(0, min(n - 1, ii));
-    i = ii;
-    if (u == 0.0) {
-        di = 0;
-        t0 = __int_as_float(0x7f800000);
-        td = 0.0f;
-        return t0;
-    }
-    const double iu = 1.0 / u;
-    const int k = u > 0.0 ? ii + 1 : ii;
-    const double sc = (o + (double)k * v - p1) * iu - s_lo;
-    di = u > 0.0 ? stride : -stride;
-    t0 = (float)fmax(sc, 0.0);
-    td = fminf((float)(v * fabs(iu)), kBigT);
-    const int nsteps = u > 0.0 ? n - 1 - ii : ii;
-    return nsteps == 0 ? t0 : fmaf((float)nsteps, td, t0);
-}
-
-// Slab clip of one axis; false when the ray is parallel to the axis and outside the slab.
-__device__ __forceinline__ bool axis_clip(double p1, double u, double lo, double hi, double &s_lo, double &s_hi) {
-    if (u == 0.0) return !(p1 < lo || p1 >= hi);
-    const double iu = 1.0 / u;
-    const double a = (lo - p1) * iu, b = (hi - p1) * iu;
-    s_lo = fmax(s_lo, fmin(a, b));
-    s_hi = fmin(s_hi, fmax(a, b));
-    return true;
-}
-
-// Ray set-up in fp64 (comment (1) at the top); false when the event is skipped or its window misses the grid.
-template <bool TOF>
-__device__ __forceinline__ bool ray_setup(const ProjParams &P, float fx1, float fy1, float fz1, float fx2, float fy2,
-                                          float fz2, float fdt, Ray &r) {
-    if (!(finite_f(fx1) && finite_f(fy1) && finite_f(fz1) && finite_f(fx2) && finite_f(fy2) && finite_f(fz2)))
-        return false;
-    if (TOF && !finite_f(fdt)) return false;
-    constexpr int A = 0, B = 1, C = 2;
-    const int nA = P.n[A], nB = P.n[B], nC = P.n[C];
-    const double oA = P.o[A], oB = P.o[B], oC = P.o[C];
-    const double hA = P.h[A], hB = P.h[B], hC = P.h[C];
-    const double vA = P.v[A], vB = P.v[B], vC = P.v[C];
-    const double ivA = P.iv[A], ivB = P.iv[B], ivC = P.iv[C];
-    const double x1 = fx1, y1 = fy1, z1 = fz1;
-    const double dx = (double)fx2 - x1, dy = (double)fy2 - y1, dz = (double)fz2 - z1;
-    const double L2 = dx * dx + dy * dy + dz * dz;
-    if (!(L2 > 0.0)) return false;
-    const double L = sqrt(L2);
-    const double iL = 1.0 / L;
-    const double ux = dx * iL, uy = dy * iL, uz = dz * iL;
-    double s_lo = 0.0, s_hi = L;
-    if (!axis_clip(x1, ux, oA, hA, s_lo, s_hi)) return false;
-    if (!axis_clip(y1, uy, oB, hB, s_lo, s_hi)) return false;
-    if (!axis_clip(z1, uz, oC, hC, s_lo, s_hi)) return false;
-    double s_c = 0.0;
-    if (TOF) {
-        s_c = 0.5 * L + (0.5 * kCmmPerPs) * (double)fdt;
-        s_lo = fmax(s_lo, s_c - P.half_window);
-        s_hi = fmin(s_hi, s_c + P.half_window);
-    }
-    if (!(s_hi > s_lo)) return false;
-    r.tc = (float)(s_c - s_lo);
-    int ia, ib, ic;
-    const float ea = axis_setup(x1, ux, s_lo, oA, vA, ivA, nA, 1, ia, r.dxi, r.t0x, r.tdx);
-    const float eb = axis_setup(y1, uy, s_lo, oB, vB, ivB, nB, nA, ib, r.dyi, r.t0y, r.tdy);
-    const float ec = axis_setup(z1, uz, s_lo, oC, vC, ivC, nC, nA * nB, ic, r.dzi, r.t0z, r.tdz);
-    r.t_end = fminf(fminf((float)(s_hi - s_lo), ea), fminf(eb, ec));
-    r.idx = (ic * nB + ib) * nA + ia;
-    if (P.brick) {
-        // index = (brick number) * 4 + (iy & 1) * 2 + (ix & 1): a step in x alternates between +-1 (inside the brick)
-        // and +-3 (into the neighbouring brick), a step in y between +-2 and +-(2 nx - 2); z steps are unchanged
-        r.bidx = ((ic * (nB >> 1) + (ib >> 1)) * (nA >> 1) + (ia >> 1)) * 4 + ((ib & 1) << 1) + (ia & 1);
-        const int xa = r.dxi > 0 ? 1 : (r.dxi < 0 ? -3 : 0), xb = r.dxi > 0 ? 3 : (r.dxi < 0 ? -1 : 0);
-        r.bdx0 = (ia & 1) ? xb : xa;
-        r.bdxs = xa + xb;
-        const int yo = 2 * nA - 2;
-        const int ya = r.dyi > 0 ? 2 : (r.dyi < 0 ? -yo : 0), yb = r.dyi > 0 ? yo : (r.dyi < 0 ? -2 : 0);
-        r.bdy0 = (ib & 1) ? yb : ya;
-        r.bdys = ya + yb;
-    }
-    return true;
-}
-
-// Branch-free incremental walk.  step() returns the un-normalised weight of the current clipped chord and its
-// flat voxel index, and advances; `done` is set on the last chord.
-template <bool TOF, bool BRICK = false>
-struct Walker {
-    float tx, ty, tz, kx, ky, kz, t;
-    int idx, dxc, dyc;
-    __device__ __forceinline__ explicit Walker(const Ray &r)
-        : tx(r.t0x), ty(r.t0y), tz(r.t0z), kx(0.f), ky(0.f), kz(0.f), t(0.f), idx(BRICK ? r.bidx : r.idx),
-          dxc(BRICK ? r.bdx0 : r.dxi), dyc(BRICK ? r.bdy0 : r.dyi) {}
-    __device__ __forceinline__ float step(const ProjParams &P, const Ray &r, int &at, bool &done) {
-        const float tn = fminf(fminf(tx, ty), fminf(tz, r.t_end));
-        const float l = tn - t;
-        float w = l;
-        if (TOF) {
-            const float tm = fmaf(0.5f, t + tn, -r.tc);
-            w = l * ex2_approx(P.gauss_a * tm * tm);
-        }
-        at = idx;
-        done = tn >= r.t_end;
-        if (tx <= tn) {
-            kx += 1.0f;
-            idx += dxc;
-            if (BRICK) dxc = r.bdxs - dxc;
-        }
-        if (ty <= tn) {
-            ky += 1.0f;
-            idx += dyc;
-            if (BRICK) dyc = r.bdys - dyc;
-        }
-        if (tz <= tn) { kz += 1.0f; idx += r.dzi; }
-        tx = fmaf(kx, r.tdx, r.t0x);
-        ty = fmaf(ky, r.tdy, r.t0y);
-        tz = fmaf(kz, r.tdz, r.t0z);
-        t = tn;
-        return w;
-    }
-};
-
-// sum_j w_j image[j] over the window (un-normalised).  Software pipeline of depth kGatherDepth on the gathers: the
-// value loaded in one step is consumed kGatherDepth steps later, which hides the L1/L2 latency behind whole steps of
-// arithmetic.  Depth 3 was measured (48 registers): 24.01 vs 24.09 ms, no gain -- the pass is not gather-latency-bound.
-constexpr int kGatherDepth = 2;
-
-template <bool TOF>
-__device__ __forceinline__ float ray_gather(const ProjParams &P, const Ray &r, const float *__restrict__ image,
-                                            int &visits) {
-    Walker<TOF> wk(r);
-    float acc = 0.0f;
-    float w[kGatherDepth], v[kGatherDepth];
-#pragma unroll
-    for (int i = 0; i < kGatherDepth; ++i) w[i] = v[i] = 0.0f;
-    int at, n = 0;
-    bool done = false;
-    while (!done) {
-#pragma unroll
-        for (int i = 0; i < kGatherDepth; ++i) {
-            if (!done) {
-                acc = fmaf(w[i], v[i], acc);  // the pair this slot has held for kGatherDepth steps
-                w[i] = wk.step(P, r, at, done);
-                v[i] = __ldg(image + at);
-                ++n;
-            }
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < kGatherDepth; ++i) acc = fmaf(w[i], v[i], acc);
-    visits = n;
-    return acc;
-}
-
-// out[j] += w_j * scale over the window: float32 reductions at L2, fire and forget.
-// VEC: one 16-byte vector reduction per aligned group of 4 voxels (needs a 16-byte aligned `out` whose
-// allocation covers whole groups); otherwise one scalar reduction per voxel.
-// BRICK (with VEC): `out` is in the brick layout, whose 16-byte groups are 2x2x1 voxels: a line that meets a group meets
-// 1.50 of its voxels on average against 1.34 for 4x1x1 groups (Cauchy: 4 * 6 / surface), i.e. 11 % fewer reductions.
-template <bool TOF, bool VEC, bool BRICK = false>
-__device__ __forceinline__ int ray_scatter(const ProjParams &P, const Ray &r, float *__restrict__ out, float scale) {
-    Walker<TOF, BRICK> wk(r);
-    int at, reds = 1;
-    bool done;
-    if (VEC) {
-        // The flush is a predicated instruction, not a branch: some lane of a warp flushes in nearly every step
-        // (ncu r01b: 97 % of the warp iterations), so a branch only adds its re-convergence overhead.
-        int grp = (BRICK ? r.bidx : r.idx) >> 2;
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-#pragma unroll 2
-        do {
-            const float val = wk.step(P, r, at, done) * scale;
-            const int g = at >> 2;
-            const bool fl = g != grp;
-            red_v4_if(fl, out + 4 * (size_t)grp, a0, a1, a2, a3);
-            reds += fl;
-            grp = g;
-            const int sl = at & 3;  // each voxel is met once per ray: plain writes, no accumulation
-            a0 = sl == 0 ? val : (fl ? 0.f : a0);
-            a1 = sl == 1 ? val : (fl ? 0.f : a1);
-            a2 = sl == 2 ? val : (fl ? 0.f : a2);
-            a3 = sl == 3 ? val : (fl ? 0.f : a3);
-        } while (!done);
-        red_v4(out + 4 * (size_t)grp, a0, a1, a2, a3);
-    } else {
-        reds = 0;
-        do {
-            const float w = wk.step(P, r, at, done);
-            atomicAdd(out + at, w * scale);  // zero-length chords (corner crossings) add +0: harmless, rare
-            ++reds;
-        } while (!done);
-    }
-    return reds;
-}
-
-
 constexpr int kBlock = 256;
+constexpr int kMaxDevices = 64;
 
 template <bool TOF>
 __device__ __forceinline__ bool load_and_setup(const ProjParams &P, const EventPtrs &ev, uint64_t e, Ray &r) {
@@ -346,9 +115,10 @@ __global__ void __launch_bounds__(kBlock) em_correction_kernel(ProjParams P, Eve
 }
 
 // Persistent form of the fused pass (the default): the locality-binned event list is cut into `nseg` contiguous
-// segments, two per SM; every warp takes 32-event chunks from the queue of the SM it runs on (%smid), so the warps
-// resident on an SM work on neighbouring events and share that SM's L1 for their image gathers (the 8 co-resident
-// CTAs of the grid-order form come from 8 unrelated places and thrash it), while different SMs reduce into different
+// segments, `segs_per_sm` (1, 3 or 4, see launch_em) per SM; every warp takes 32-event chunks from the queue of the SM it
+// runs on (%smid), so the warps resident on an SM (5 CTAs of 256 threads) work on neighbouring events and share that
+// SM's L1 for their image gathers (the co-resident CTAs of the grid-order form come from unrelated places and thrash
+// it), while different SMs reduce into different
 // parts of the volume.  A warp whose segment is exhausted moves on to other segments (work stealing; the invalid
 // events sorted to the end of the list make the last segments empty).  Measured at cfg-3: 30.2 -> 25.2 ms.
 template <bool TOF, bool VEC, bool BRICK>
@@ -357,7 +127,8 @@ __global__ void __launch_bounds__(kBlock, 5) em_persistent_kernel(ProjParams P, 
                                                                const float *__restrict__ image,
                                                                float *__restrict__ corr, DeviceStats *stats,
                                                                unsigned *queues, unsigned nseg, unsigned per_seg,
-                                                               unsigned segs_per_sm) {
+                                                               unsigned segs_per_sm,
+                                                               const uint2 *__restrict__ chunks, unsigned n_chunks) {
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
@@ -375,8 +146,16 @@ __global__ void __launch_bounds__(kBlock, 5) em_persistent_kernel(ProjParams P, 
         }
         int visits, reds;
         bool valid;
-        em_event<TOF, VEC, BRICK>(P, ev, ((uint64_t)seg * per_seg + c) * 32u + lane, n, evw, image, corr, visits, valid,
-                                  reds);
+        const uint64_t wc = (uint64_t)seg * per_seg + c;  // index of the warp's 32-event piece
+        uint64_t e = wc * 32u + lane;
+        if (chunks) {  // the pieces come from a list (the events the tile-mode pass leaves over)
+            e = n;
+            if (wc < n_chunks) {
+                const uint2 ch = __ldg(chunks + wc);
+                if (lane < ch.y) e = (uint64_t)ch.x + lane;
+            }
+        }
+        em_event<TOF, VEC, BRICK>(P, ev, e, n, evw, image, corr, visits, valid, reds);
         nv += valid;
         vis += visits;
         nr += reds;
@@ -489,14 +268,11 @@ __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P
 template <bool TOF, bool BRICK>
 static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
                              float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
-    static int n_sm = 0;
     const size_t smem = sizeof(unsigned long long) << kCacheLog2;
-    if (!n_sm) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        cudaFuncSetAttribute(em_cached_kernel<TOF, BRICK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    }
+    int dev = 0, n_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaFuncSetAttribute(em_cached_kernel<TOF, BRICK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     unsigned nseg = (unsigned)n_sm;
     if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
     if (nseg % 61u == 0) nseg -= 1;
@@ -541,15 +317,20 @@ void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint
 
 template <bool TOF, bool VEC, bool BRICK>
 static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
-                      float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
-    if (p.variant != 1 && queues) {
-        static int n_sm = 0, per_sm = 0;  // per instantiation; one device per process
-        if (!n_sm) {
-            int dev = 0;
-            cudaGetDevice(&dev);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
-            cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+                      float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s, const uint2 *chunks = nullptr,
+                      uint32_t n_chunks = 0) {
+    if ((p.variant != 1 || chunks) && queues) {
+        // SM count and resident CTAs per SM of THIS instantiation on the CURRENT device (cached per device; a race on
+        // the first use only writes the same values twice)
+        static int sm_of[kMaxDevices] = {0}, per_of[kMaxDevices] = {0};
+        int dev = 0;
+        cudaGetDevice(&dev);
+        const int slot = dev < kMaxDevices ? dev : kMaxDevices - 1;
+        if (!sm_of[slot] || dev >= kMaxDevices) {
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_of[slot], em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
+            cudaDeviceGetAttribute(&sm_of[slot], cudaDevAttrMultiProcessorCount, dev);
         }
+        const int n_sm = sm_of[slot], per_sm = per_of[slot];
         // Short windows: the warps of an SM spread over several list segments (measured at 146 M events: 300 ps, 1 / 2 /
         // 3 / 4 / 8 segments per SM -> 21.47 / 21.04 / 20.75 / 22.25 / 23.54 ms; 100 ps, 1 / 2 / 3 / 4 -> 11.35 / 9.57 /
         // 9.44 / 9.32 ms).  Long walks (600 ps: 43.3 -> 45.1 ms, non-TOF: 203 -> 218 ms with 2) keep one.
@@ -558,11 +339,11 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         unsigned nseg = (unsigned)n_sm * kSegsPerSm;
         if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / kSegsPerSm * kSegsPerSm;
         if (nseg % 61u == 0) nseg -= kSegsPerSm;  // the stealing stride 61 must not divide the number of segments
-        const uint64_t wchunks = (n + 31) / 32;
+        const uint64_t wchunks = chunks ? (uint64_t)n_chunks : (n + 31) / 32;
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
         cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
         em_persistent_kernel<TOF, VEC, BRICK><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(
-            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, kSegsPerSm);
+            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, kSegsPerSm, chunks, n_chunks);
     } else {
         em_correction_kernel<TOF, VEC, BRICK><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
     }
@@ -571,8 +352,14 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
 void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *evw,
                           const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,
                           cudaStream_t s) {
-    if (n == 0) return;
-    if (p.variant == 2 && queues && vec_ok) {
+    launch_em_correction_chunks(p, tof, ev, n, nullptr, 0, evw, image, corr, vec_ok, stats, queues, s);
+}
+
+void launch_em_correction_chunks(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const uint2 *chunks,
+                                 uint32_t n_chunks, const float *evw, const float *image, float *corr, bool vec_ok,
+                                 DeviceStats *stats, unsigned *queues, cudaStream_t s) {
+    if (n == 0 || (chunks && n_chunks == 0)) return;
+    if (p.variant == 2 && queues && vec_ok && !chunks) {
         if (tof) {
             if (p.brick)
                 launch_em_cached<true, true>(p, ev, n, evw, image, corr, stats, queues, s);
@@ -588,21 +375,21 @@ void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, ui
     }
     if (p.brick && vec_ok) {  // the brick layout exists only together with the 16-byte reductions
         if (tof)
-            launch_em<true, true, true>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<true, true, true>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
         else
-            launch_em<false, true, true>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<false, true, true>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
         return;
     }
     if (tof) {
         if (vec_ok)
-            launch_em<true, true, false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<true, true, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
         else
-            launch_em<true, false, false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<true, false, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
     } else {
         if (vec_ok)
-            launch_em<false, true, false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<false, true, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
         else
-            launch_em<false, false, false>(p, ev, n, evw, image, corr, stats, queues, s);
+            launch_em<false, false, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
     }
 }
 

@@ -25,6 +25,9 @@ OPT_MEDIAN = 10
 OPT_CACHE_SHARE = 11
 OPT_CORR_BRICKS = 12
 OPT_DETERMINISTIC = 13
+OPT_TILE_MIN_EVENTS = 14
+OPT_TILE_CHECK = 15
+OPT_TILE_MAX_EVENTS = 16
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
@@ -36,6 +39,7 @@ SYMBOLS = (
     "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
     "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
     "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events", "tofmlem_reserve", "tofmlem_trim",
+    "tofmlem_plan_events", "tofmlem_plan_info",
 )
 
 
@@ -59,7 +63,13 @@ class Events(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_valid", C.c_uint64), ("n_skipped", C.c_uint64), ("visits", C.c_uint64),
-                ("sum_image_sens", C.c_double), ("reductions", C.c_uint64)]
+                ("sum_image_sens", C.c_double), ("reductions", C.c_uint64), ("tile_events", C.c_uint64),
+                ("tile_oob", C.c_uint64)]
+
+
+class Plan(C.Structure):
+    _fields_ = [("active", C.c_int32), ("sorted", C.c_int32), ("n_tile_items", C.c_uint32),
+                ("n_direct_chunks", C.c_uint32), ("n_tile_events", C.c_uint64), ("n_direct_events", C.c_uint64)]
 
 
 class TofMlemError(RuntimeError):
@@ -177,6 +187,15 @@ class Context:
         self._check(self._L.tofmlem_em_correction(self._h, C.byref(e), C.c_uint64(n),
                                                   C.c_void_p(_ptr(image, torch.float32, "cuda", self.nvox)),
                                                   C.c_void_p(_ptr(corr, torch.float32, "cuda", self.nvox))))
+
+    def plan_events(self, ev, n: int) -> "Plan":
+        self._check(self._L.tofmlem_plan_events(self._h, C.byref(_events(ev, n)), C.c_uint64(n)))
+        return self.plan_info()
+
+    def plan_info(self) -> "Plan":
+        p = Plan()
+        self._check(self._L.tofmlem_plan_info(self._h, C.byref(p)))
+        return p
 
     def reset_stats(self):
         self._check(self._L.tofmlem_reset_stats(self._h))

@@ -42,7 +42,10 @@ def fwd_rel_err(gpu, ref):
     return np.abs(gpu - ref) / den
 
 
-def check_image(gpu, ref, l2=IMG_L2, mx=IMG_MAX):
+def check_image(gpu, ref, l2=IMG_L2, mx=IMG_MAX, zero_tol=0.0):
+    """zero_tol: largest value (relative to the image maximum) the CUDA path may hold in a voxel where the oracle holds
+    exactly 0.  0 for dense data; sparse data on a large grid has voxels whose ONLY contribution is the sliver chord at
+    a clipped window end, which exists in fp32 and not in fp64 or vice versa (SURVEY.md 8(c) "sliver < 1e-3 mm")."""
     gpu = np.asarray(gpu, np.float64).reshape(-1)
     ref = np.asarray(ref, np.float64).reshape(-1)
     rel_l2 = np.linalg.norm(gpu - ref) / np.linalg.norm(ref)
@@ -50,7 +53,8 @@ def check_image(gpu, ref, l2=IMG_L2, mx=IMG_MAX):
     max_rel = np.max(np.abs(gpu[big] - ref[big]) / ref[big])
     assert rel_l2 <= l2, f"rel-L2 {rel_l2:.3e}"
     assert max_rel <= mx, f"max rel {max_rel:.3e}"
-    assert np.all(gpu[ref == 0] == 0)
+    z = gpu[ref == 0]
+    assert z.size == 0 or z.max() <= zero_tol * ref.max(), (z.max(), ref.max(), int((z != 0).sum()))
     return rel_l2, max_rel
 
 
@@ -487,6 +491,20 @@ def test_full_size_bench_configuration(pkg):
     assert float(d) <= 1e-5, float(d)
     big = corr_a > 0.01 * corr_a.max()
     assert float(((corr_a - corr_b).abs()[big] / corr_a[big]).max()) <= 1e-3
+    # tile mode (tofmlem_plan_events: what bench.py times): the same correction image again, most events through the
+    # shared-memory tiles, far fewer reductions at L2
+    plan = ctx.plan_events(sev, n)
+    assert plan.active and plan.n_tile_events > 0.6 * n
+    corr_c = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.reset_stats()
+    ctx.em_correction(sev, n, img, corr_c)
+    st_c = ctx.get_stats()
+    assert st_c.n_valid == n_pos and st_c.visits == st_a.visits and st_c.tile_oob == 0
+    assert st_c.tile_events > 0.6 * n_pos and st_c.reductions < 0.6 * st_b.reductions
+    d = (corr_a.double() - corr_c.double()).norm() / corr_a.double().norm()
+    assert float(d) <= 1e-5, float(d)
+    assert float(((corr_a - corr_c).abs()[big] / corr_a[big]).max()) <= 1e-3
+    del corr_c
     # P7 at full size: after the update sum(sens * x) = n_valid (sens = any positive image; mask = all voxels)
     sens = torch.full((g.nvox,), 0.25, dtype=torch.float32, device="cuda")
     ctx.update(img, corr_b, sens)

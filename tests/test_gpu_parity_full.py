@@ -58,15 +58,22 @@ def test_full_grid_five_iterations_subsample(pkg, full_sens):
     ev = synth.make_events(cfg, n, start=7_000_000, device="cuda")
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
     sev, _ = binned(ctx, ev, n)
-    if hasattr(ctx, "plan_events"):
-        ctx.plan_events(sev, n)
+    # tile mode on every bin with >= 8 events (2 M events on 384 k bins are sparse; the default threshold is 1024),
+    # every tile access bounds-tested
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 8)
+    ctx.set_option(pkg.OPT_TILE_CHECK, 1)
+    plan = ctx.plan_events(sev, n)
+    assert plan.active and plan.sorted and plan.n_tile_events + plan.n_direct_events == n
+    assert plan.n_tile_events > 0.3 * n
     sens_np = full_sens.cpu().numpy()
     mask = oracle.mask_f32(sens_np)
     x = torch.from_numpy(mask.astype(np.float32)).cuda()
     ctx.iterate(sev, n, x, full_sens, iters)
     st = ctx.get_stats()
+    assert st.tile_oob == 0 and st.tile_events > 0.25 * st.n_valid, (st.tile_oob, st.tile_events, st.n_valid)
+    print(f"tile items {plan.n_tile_items}, tile events {plan.n_tile_events}, through tiles {st.tile_events} of {st.n_valid}")
     ref, ost = oracle.mlem(og, oracle.sigma_mm(cfg.tof_fwhm_ps), to_np(ev), mask.astype(np.float64), sens_np, iters)
-    l2, mx = check_image(x.cpu().numpy(), ref)
+    l2, mx = check_image(x.cpu().numpy(), ref, zero_tol=1e-6)
     print(f"cfg-3 grid, 2 M events, 5 iterations: rel-L2 {l2:.2e}, max rel {mx:.2e}")
     assert st.n_valid == ost.n_valid
     assert abs(st.sum_image_sens - st.n_valid) / st.n_valid < 1e-4  # P7
@@ -86,8 +93,6 @@ def test_full_grid_fused_pass_every_context(pkg, full_sens, fwhm):
         ev["dt"].zero_()
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
     sev, _ = binned(ctx, ev, n)
-    if hasattr(ctx, "plan_events"):
-        ctx.plan_events(sev, n)
     sens_np = full_sens.cpu().numpy()
     mask = oracle.mask_f32(sens_np)
     sig = oracle.sigma_mm(fwhm) if fwhm > 0 else 0.0
@@ -104,7 +109,7 @@ def test_full_grid_fused_pass_every_context(pkg, full_sens, fwhm):
         st = ctx.get_stats()
         c_ref, nv_ref, vis_ref = oracle.em_correction(og, sig, ev_np, xr)
         xr = oracle.update(xr, c_ref, sens_np, mask)
-        l2, mx = check_image(x.cpu().numpy(), xr)
+        l2, mx = check_image(x.cpu().numpy(), xr, zero_tol=1e-6)
         assert st.n_valid == nv_ref, (fwhm, it, st.n_valid, nv_ref)
         assert abs(int(st.visits) - int(vis_ref)) <= 1e-4 * vis_ref
         print(f"fwhm {fwhm:g} pass {it}: rel-L2 {l2:.2e}, max rel {mx:.2e}, visits/event {st.visits / max(1, st.n_valid):.1f}")
@@ -174,3 +179,114 @@ def test_deterministic_option_is_declared_and_refused(pkg):
     with pytest.raises(pkg.TofMlemError) as e:
         ctx.set_option(pkg.OPT_DETERMINISTIC, 2)
     assert e.value.code == -1
+
+
+# ------------------------------------------------------------------ tile mode (tofmlem_plan_events, tile.cu)
+def _tile_case(pkg, cfg, n, m, min_events, iters=2, expect_active=True, seed_img=None):
+    g, og = grids(pkg, cfg)
+    ev = synth.make_events(cfg, n, device="cuda")
+    lors = synth.make_sens_lors(cfg, m, device="cuda")
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    sens = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.sensitivity(lors, m, sens)
+    sev, _ = binned(ctx, ev, n)
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, min_events)
+    ctx.set_option(pkg.OPT_TILE_CHECK, 1)
+    plan = ctx.plan_events(sev, n)
+    assert bool(plan.active) == expect_active, (plan.active, plan.sorted, plan.n_tile_items)
+    sens_np = sens.cpu().numpy()
+    mask = oracle.mask_f32(sens_np)
+    x = torch.from_numpy(mask.astype(np.float32)).cuda()
+    ctx.iterate(sev, n, x, sens, iters)
+    st = ctx.get_stats()
+    sig = oracle.sigma_mm(cfg.tof_fwhm_ps)
+    ref, ost = oracle.mlem(og, sig, to_np(ev), mask.astype(np.float64), sens_np, iters)
+    check_image(x.cpu().numpy(), ref, zero_tol=1e-6)
+    assert st.n_valid == ost.n_valid
+    assert abs(int(st.visits) - int(ost.visits)) <= 1e-4 * ost.visits
+    assert st.tile_oob == 0
+    assert abs(st.sum_image_sens - st.n_valid) / st.n_valid < 1e-4
+    return ctx, plan, st, sev, x, sens
+
+
+def test_tile_mode_parity_tiny(pkg):
+    """cfg-1 in tile mode (bins of >= 64 events through shared-memory tiles, bounds-tested) vs oracle.mlem; the planned
+    and the unplanned pass of the same context give the same correction (up to the float32 summation order)."""
+    cfg = synth.TINY
+    ctx, plan, st, sev, x, sens = _tile_case(pkg, cfg, cfg.n_events, 400_000, 64)
+    assert st.tile_events > 0.8 * st.n_valid, (st.tile_events, st.n_valid)
+    n = cfg.n_events
+    img = synth.random_image((ctx.nvox,), 19, device="cuda")
+    a = torch.zeros(ctx.nvox, dtype=torch.float32, device="cuda")
+    b = torch.zeros_like(a)
+    ctx.reset_stats()
+    ctx.em_correction(sev, n, img, a)  # planned
+    st_a = ctx.get_stats()
+    other = {k: v.clone() for k, v in sev.items()}  # another list (same events): no plan for it
+    ctx.reset_stats()
+    ctx.em_correction(other, n, img, b)
+    st_b = ctx.get_stats()
+    assert st_a.tile_events > 0 and st_b.tile_events == 0
+    assert st_a.n_valid == st_b.n_valid and st_a.visits == st_b.visits
+    assert st_a.reductions < 0.5 * st_b.reductions  # what the tiles are for: far fewer reductions at L2
+    d = (a.double() - b.double()).norm() / b.double().norm()
+    assert float(d) < 1e-6, float(d)
+    # a list changed in place after the plan still gives correct results: every event is checked against its tile
+    rev = {k: v.flip(0).contiguous() for k, v in sev.items()}
+    for k in sev:
+        sev[k].copy_(rev[k])
+    c = torch.zeros_like(a)
+    ctx.reset_stats()
+    ctx.em_correction(sev, n, img, c)
+    st_c = ctx.get_stats()
+    assert st_c.n_valid == st_b.n_valid and st_c.tile_oob == 0
+    assert float((c.double() - b.double()).norm() / b.double().norm()) < 1e-6
+    # an unsorted list leaves the plan inactive
+    plan2 = ctx.plan_events(rev, n)
+    assert not plan2.sorted and not plan2.active
+
+
+def test_tile_mode_anisotropic_voxels_and_weights(pkg):
+    """Tile envelopes with three different voxel sizes (the lateral slopes v_a / v_b differ per class), a grid that is not
+    a multiple of the 8-voxel cube, events with per-event weights."""
+    cfg = synth.Config("aniso", 30, 26, 22, 4.0, 150.0, 110.0, synth.Phantom(
+        parts=(synth.Shape("ellipsoid", (0.0, 0.0, 0.0), (45.0, 40.0, 40.0), 1.0),),
+        inner=(synth.Shape("ellipsoid", (12.0, -8.0, 5.0), (9.0, 9.0, 9.0), 4.0),)), 150_000, 0.15, 300.0, 2, 300_000, 23)
+    n, m = cfg.n_events, cfg.sens_lors
+    vox = (4.0, 4.6, 5.0)
+    g = pkg.make_grid(cfg.nx, cfg.ny, cfg.nz, vox)
+    og = oracle.make_grid(cfg.nx, cfg.ny, cfg.nz, vox)
+    ev = synth.make_events(cfg, n, device="cuda")
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    sev, perm = binned(ctx, ev, n)
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 32)
+    ctx.set_option(pkg.OPT_TILE_CHECK, 1)
+    plan = ctx.plan_events(sev, n)
+    assert plan.active
+    w = (0.5 + torch.rand(n, generator=torch.Generator().manual_seed(3))).cuda()
+    sw = torch.empty_like(w)
+    ctx.gather_f32(w, perm, n, sw)
+    img = synth.random_image((g.nvox,), 29, device="cuda")
+    corr = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.set_option(pkg.OPT_CORR_BRICKS, 0)  # read the correction image directly
+    ctx.reset_stats()
+    ctx.em_correction_weighted(sev, n, sw, img, corr)
+    st = ctx.get_stats()
+    ref, nv, vis = oracle.em_correction(og, oracle.sigma_mm(300.0), to_np(ev), img.cpu().numpy().astype(np.float64),
+                                        weights=w.cpu().numpy())
+    assert st.n_valid == nv and st.tile_oob == 0 and st.tile_events > 0.5 * nv
+    check_image(corr.cpu().numpy(), ref, l2=1e-5, mx=1e-3, zero_tol=1e-6)
+
+
+def test_tile_mode_inactive_when_tiles_do_not_fit(pkg):
+    """cfg-2 (2 mm voxels: the +-3 sigma window spans 57 voxels, a tile pair would need > 227 KB): the plan stays inactive
+    and the pass is the direct one."""
+    cfg = synth.MID
+    g, og = grids(pkg, cfg)
+    n = 100_000
+    ev = synth.make_events(cfg, n, device="cuda")
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    sev, _ = binned(ctx, ev, n)
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 8)
+    plan = ctx.plan_events(sev, n)
+    assert not plan.active
