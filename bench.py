@@ -24,6 +24,9 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "events/s per TOF-MLEM iteration (fwd+backproj)"
+# DRAM bytes of one launch of the dominant kernel at cfg-3 (ncu --set full; refresh with the capture)
+TRAFFIC_BYTES = 8.177348e9
+TRAFFIC_SOURCE = "profiles/r04_em_persistent_ncu_full_metrics.txt (6.894 GB read + 1.283 GB written per launch)"
 UNIT = "events/s"
 
 
@@ -83,42 +86,64 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
-def run_reference(args):
-    """--impl reference: the fp64 oracle, as it stands, on the host cores (rank 0 only)."""
-    if int(os.environ.get("RANK", "0")) != 0:
-        return
+def make_config(cfg, n, m, world, binned=True):
+    """The `config` object of the JSON line: the same for the b200 arm and the reference (oracle) arm."""
+    return {
+        "workload": f"{cfg.name}: {cfg.nx}x{cfg.ny}x{cfg.nz} voxels of {cfg.voxel_mm} mm, scanner R={cfg.radius_mm:g} L={cfg.axial_mm:g} mm, "
+                    f"{n} events/GPU, {cfg.scatter_fraction:.0%} scatter-like, TOF {cfg.tof_fwhm_ps:g} ps FWHM",
+        "events_per_gpu": n, "l2": "inputs larger than L2 (events 28 B x n >> 126 MB); no flush",
+        "binned": binned, "sens_lors": m,
+        "parallelism": "event shards + one fp32 all-reduce of the correction image per iteration" if world > 1 else "single GPU",
+    }
+
+
+def oracle_arm(cfg, n_sample, steps, warmup):
+    """The oracle, as it stands, on the host cores: one EM pass + update per step over a bounded sample of the workload.
+    The sample is the first `n_sample` events of the seeded set in generation order -- the events are independent draws,
+    so a prefix is an unbiased sample of the workload's LOR mix -- on the full grid, image = 1, sensitivity = 1 (the
+    oracle's cost does not depend on the image values).  Used by --impl reference and by the b200 arm's `cpu_baseline`,
+    so that both report the same thing."""
     import numpy as np
 
     import oracle
     import synth
 
-    cfg = synth.CONFIGS[args.workload]
     og = oracle.make_grid(cfg.nx, cfg.ny, cfg.nz, cfg.voxel_mm)
     sig = oracle.sigma_mm(cfg.tof_fwhm_ps)
-    n = args.ref_events
+    n = min(n_sample, cfg.n_events)
     ev = {k: v.numpy() for k, v in synth.make_events_chunked(cfg, n, chunk=500_000).items()}
     x = np.ones(og.nvox)
     sens = np.ones(og.nvox, np.float32)
     mask = np.ones(og.nvox, np.uint8)
     times = []
-    for step in range(args.warmup + args.steps):
+    for step in range(warmup + steps):
         t0 = time.perf_counter()
         corr, n_valid, visits = oracle.em_correction(og, sig, ev, x)
         x = oracle.update(x, corr, sens, mask)
         x *= og.nvox / max(x.sum(), 1e-300)  # keep the image scale stable without a real sensitivity image
-        if step >= args.warmup:
+        if step >= warmup:
             times.append(time.perf_counter() - t0)
     ms = 1e3 * sum(times) / len(times)
-    value = n / (ms * 1e-3)
-    cores = oracle.num_threads()
+    return {"value": n / (ms * 1e-3), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"first {n} events of the seeded {cfg.name} set in generation order (independent draws: an unbiased "
+                      f"sample), one EM pass + update per step on the full grid, {steps} timed steps of {ms / 1e3:.2f} s"}, ms
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import synth
+
+    cfg = synth.CONFIGS[args.workload]
+    cpu, ms = oracle_arm(cfg, args.ref_events, args.steps, args.warmup)
+    value = cpu["value"]
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{cfg.name}: {cfg.nx}x{cfg.ny}x{cfg.nz} x {cfg.voxel_mm} mm, TOF {cfg.tof_fwhm_ps:g} ps",
-                   "events_per_step": n},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": f"{n}-event prefix of the seeded {cfg.name} set, one EM pass + update per step, full grid"},
+        "config": make_config(cfg, args.events or cfg.n_events, args.sens_lors or cfg.sens_lors, max(1, args.gpus)),
+        "cpu_baseline": cpu,
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -400,13 +425,15 @@ def main():
     ap.add_argument("--ref-events", type=int, default=8_000_000,
                     help="events per step of --impl reference (the oracle's per-call cost of ~0.75 s -- one private fp64 "
                          "correction image per thread -- is amortised from a few million events on)")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target duration of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-bin", action="store_true", help="skip locality binning (for comparison)")
     ap.add_argument("--subbins", type=int, default=0, help="TOFMLEM_OPT_SUBBINS override (0 = library default)")
     ap.add_argument("--em-variant", type=int, default=-1, help="TOFMLEM_OPT_EM_VARIANT override (-1 = library default)")
     ap.add_argument("--cache-share", type=int, default=-1, help="TOFMLEM_OPT_CACHE_SHARE override")
+    ap.add_argument("--tile", type=int, default=0, help="1: tofmlem_plan_events on the binned list (tile-mode fused pass)")
+    ap.add_argument("--tile-min", type=int, default=0, help="TOFMLEM_OPT_TILE_MIN_EVENTS override")
+    ap.add_argument("--tile-max", type=int, default=0, help="TOFMLEM_OPT_TILE_MAX_EVENTS override")
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next", "pipeline"],
                     help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
                          "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
@@ -478,6 +505,13 @@ def main():
         del key, perm, ev
         ev = sev
     torch.cuda.empty_cache()
+    plan = None
+    if args.tile and not args.no_bin:
+        if args.tile_min:
+            ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, args.tile_min)
+        if args.tile_max:
+            ctx.set_option(pkg.OPT_TILE_MAX_EVENTS, args.tile_max)
+        plan = ctx.plan_events(ev, n)
 
     image = torch.ones(nvox, dtype=torch.float32, device=dev)
     corr = torch.zeros(nvox, dtype=torch.float32, device=dev)
@@ -521,6 +555,7 @@ def main():
     st = ctx.get_stats()
     kern_ms = statistics.mean(a.elapsed_time(b) for a, b in zip(k_start, k_stop))
     p7 = float((image.double() * sens.double()).sum().item())
+    n_valid_all = sharding.sum_over_ranks(int(st.n_valid), dev)  # the image was updated with the all-reduced correction
 
     # ---- roofline of the dominant kernel (em_correction): see DESIGN.md "Measurement"
     hbm_peak, peak_src = load_peaks()
@@ -540,12 +575,20 @@ def main():
     t_red = reds / red_peak
     t_ld = visits / ld_rand
     achieved = reds / (kern_ms * 1e-3)
+    # the same launch against SURVEY.md 8(d)'s visit-based formula, T_roof = max(HBM, visits / R_gather, visits / R_red)
+    # with the conflict-free RANDOM rates (may exceed 1: 16-byte reductions carry 1.5 visits each and most gathers hit
+    # L1), and against the COALESCED L2 rates of the same probes (what the method would need with full sectors)
+    t_roof_visits = max(t_hbm, visits / ld_rand, visits / red_rand)
+    t_roof_row = max(t_hbm, visits / ld_row, visits / red_row)
+    full_default = args.workload == "full" and not args.events and not args.no_bin
     roofline = {
         "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_peak / 1e9, "unit": "G reductions/s",
         "frac": achieved / red_peak,
-        # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3 from the committed ncu --set full capture
-        # (profiles/r04_em_persistent_ncu_full_metrics.txt: 6.894 GB read + 1.283 GB written); default full workload only
-        "traffic": 8.177348e9 if (args.workload == "full" and not args.events) else None,
+        "frac_visits": t_roof_visits / (kern_ms * 1e-3), "frac_l2_coalesced": t_roof_row / (kern_ms * 1e-3),
+        # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3: a CONSTANT copied from the committed
+        # ncu --set full capture named in traffic_source (not measured in this run); default full workload only
+        "traffic": TRAFFIC_BYTES if full_default else None,
+        "traffic_source": TRAFFIC_SOURCE if full_default else None,
         "kernel": "em_persistent_kernel<TOF, v4, BRICK>", "kernel_ms": kern_ms, "visits_per_launch": visits,
         "reductions_per_launch": reds, "visits_per_reduction": visits / max(1, reds),
         "visits_Gps": visits / (kern_ms * 1e-3) / 1e9,
@@ -578,50 +621,28 @@ def main():
                "call": "tofmlem_iterate_host(iters=1), pinned host buffers, binned event order"}
         del h_ev, h_img, h_sens
 
-    # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only)
+    # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only): exactly what
+    # `--impl reference` times (same events, same order, same image), so the two arms describe one configuration
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        import numpy as np
-
-        import oracle
-
-        og = oracle.make_grid(cfg.nx, cfg.ny, cfg.nz, cfg.voxel_mm)
-        x = image.cpu().numpy().astype(np.float64)
-        sens_np, ones = sens.cpu().numpy(), np.ones(nvox, np.uint8)
-        # events are binned (spatially ordered): a strided sample keeps the workload's mix of LORs
-        ns, dt = min(n, 500_000), 0.0
-        for attempt in range(3):
-            stride = max(1, n // ns)
-            sub = {k: v[::stride][:ns].cpu().numpy() for k, v in ev.items()}
-            tt = time.perf_counter()
-            c_ref, nv_ref, vis_ref = oracle.em_correction(og, oracle.sigma_mm(cfg.tof_fwhm_ps), sub, x)
-            oracle.update(x.copy(), c_ref, sens_np, ones)
-            dt = time.perf_counter() - tt
-            ns2 = min(n, int(ns * args.cpu_seconds / max(dt, 1e-3)))
-            if attempt == 2 or ns2 <= 1.5 * ns:
-                break
-            ns = ns2
-        cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{ns} events (stride {stride} through the binned set), one EM pass + update on the full grid, {dt:.1f} s"}
+        cpu, _ = oracle_arm(cfg, args.ref_events, 3, 1)
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {
-                "workload": f"{cfg.name}: {cfg.nx}x{cfg.ny}x{cfg.nz} voxels of {cfg.voxel_mm} mm, scanner R={cfg.radius_mm:g} L={cfg.axial_mm:g} mm, "
-                            f"{n} events/GPU, {cfg.scatter_fraction:.0%} scatter-like, TOF {cfg.tof_fwhm_ps:g} ps FWHM",
-                "events_per_gpu": n, "l2": "inputs larger than L2 (events 28 B x n >> 126 MB); no flush",
-                "binned": not args.no_bin, "sens_lors": m,
-                "parallelism": "event shards + one fp32 all-reduce of the correction image per iteration" if world > 1 else "single GPU",
-            },
+            "config": make_config(cfg, n, m, world, binned=not args.no_bin),
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "setup": {"sensitivity_ms": sens_ms, "bin_sort_gather_ms": bin_ms,
                       "recon_wall_s": (bin_ms + cfg.iters * ms_per_step) * 1e-3,
                       "recon_wall_note": f"binning + {cfg.iters} iterations, events resident in HBM"},
             "stats": {"n_valid": int(st.n_valid), "visits": visits, "visits_per_valid_event": visits / max(1, int(st.n_valid)),
-                      "sum_image_sens": p7, "p7_rel_err": abs(p7 - st.n_valid) / max(1, int(st.n_valid))},
+                      "sum_image_sens": p7, "p7_rel_err": abs(p7 - n_valid_all) / max(1, n_valid_all),
+                      "tile_events": int(st.tile_events),
+                      "plan": None if plan is None else {"active": int(plan.active), "items": int(plan.n_tile_items),
+                                                         "tile_events": int(plan.n_tile_events),
+                                                         "direct_events": int(plan.n_direct_events)}},
             "paper_context": "PAPER.md:17,:299 -- 3.5 min for the slowest of nine regions (20 iterations, Tesla C2075 + 16 CPU threads); context, not the target",
         }
         print(json.dumps(line))

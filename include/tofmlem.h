@@ -73,11 +73,12 @@ typedef struct {
 
 /* What tofmlem_plan_events decided (tofmlem_plan_info). */
 typedef struct {
-    int32_t active;           /* 1: the fused pass of the planned list runs in tile mode */
-    int32_t sorted;           /* 1: the list was sorted by locality key */
-    uint32_t n_tile_items;    /* pieces of locality bins that are accumulated in shared-memory tiles */
-    uint32_t n_direct_chunks; /* 32-event pieces left to the direct pass */
-    uint64_t n_tile_events, n_direct_events;
+    int32_t active;           /* 1: the context holds ray records for the planned list */
+    int32_t sorted;           /* 1: the list was found sorted by locality key (0 also when tiles do not fit: not looked at) */
+    uint32_t n_tile_items;    /* pieces of locality bins that are accumulated in shared-memory tiles (0: none) */
+    uint32_t n_direct_chunks; /* 32-event pieces of the direct pass on records (without the tile items' stragglers) */
+    uint64_t n_tile_events;   /* events that run on a tile */
+    uint64_t n_direct_events; /* n - n_tile_events */
 } tofmlem_plan;
 
 /* Option keys for tofmlem_set_option. */
@@ -112,7 +113,8 @@ enum {
                                        accumulated in a shared-memory tile (default 1024; performance only) */
     TOFMLEM_OPT_TILE_MAX_EVENTS = 16, /* ... in pieces of at most this many events per CTA (default 8192) */
     TOFMLEM_OPT_TILE_CHECK = 15,    /* 1: bounds-test every access to the shared-memory tiles and count violations in
-                                       tofmlem_stats.tile_oob (a debugging aid; default 0) */
+                                       tofmlem_stats.tile_oob (a debugging aid; default 0).  The plan has already
+                                       dry-run every tile event against its tile, so the count must stay 0 */
     TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
                                        generated an identically reconstructed image").  0 (default) is accepted; 1
                                        returns TOFMLEM_EUNSUPPORTED: the correction image is summed with float32
@@ -164,16 +166,21 @@ int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, 
 int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr);
 int tofmlem_reset_stats(tofmlem_ctx *ctx);
 
-/* Tile mode of the fused pass (north_star bullet 4: "shared-memory tile accumulation rather than naive global atomics";
- * the paper's "direct technique for voxel filling").  ev must be a list sorted by locality key (the
- * output of tofmlem_bin_events + tofmlem_permute_events) on a TOF context with the Siddon projector.  The call looks at
- * the keys once and remembers, for THIS list (its x1 pointer and n), which bins are populous enough to be walked with
- * the image and the correction image of the bin's +-T sigma neighbourhood held in shared memory; later
- * tofmlem_em_correction[_weighted] / tofmlem_iterate[_weighted] calls with the same list run those bins in tile mode
- * and the remaining events through the direct pass.  Results are the same up to the order of the float32 sums.  The
- * plan is an optimisation only: every event is checked against its tile inside the kernel, so a list that was changed
- * in place after the call still gives correct results.  A list that is not sorted, a non-TOF context or a window whose
- * tiles do not fit in shared memory leave the plan inactive (no error).  Replaces any earlier plan.  SYNCHRONISES. */
+/* Planned event list: ray records + shared-memory tiles for the fused pass (north_star bullets 3 and 4: a fused pass that
+ * "recomputes or caches the weights", "shared-memory tile accumulation rather than naive global atomics"; the paper's
+ * "direct technique for voxel filling").  For a TOF context with the Siddon projector the call
+ * computes, once, a 48-byte ray record per event (the fp64 ray set-up, quantised so that the float32 voxel walk adds
+ * exactly) and keeps it in the context; tofmlem_em_correction[_weighted], tofmlem_iterate[_weighted] and
+ * tofmlem_forward calls with THIS list (same x1 pointer and n; the records are a snapshot: changing the arrays in place
+ * needs a new plan) then run on the records.  If ev is sorted by locality key (the output of tofmlem_bin_events +
+ * tofmlem_permute_events) and the +-T sigma neighbourhood of a locality bin fits in shared memory, bins with at least
+ * TOFMLEM_OPT_TILE_MIN_EVENTS events are walked with the image and the correction image of that neighbourhood held in
+ * shared memory ("tile items"); every event of such a bin is dry-run against the tile at plan time and the few whose
+ * window leaves it join the other events in the direct pass.  Results equal the unplanned pass up to float32 rounding
+ * (forward values within 1e-4 of the oracle like the unplanned ones).  Changing sigma-related options, the tile size,
+ * the projector or the layout of the correction image makes later calls ignore the plan (they take the unplanned path);
+ * tofmlem_trim drops it.  A non-TOF context or the K-sample projector leave the plan inactive (no error).  Replaces any
+ * earlier plan.  SYNCHRONISES; keeps 48 B per event of device memory. */
 int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n);
 int tofmlem_plan_info(const tofmlem_ctx *ctx, tofmlem_plan *h_out);
 

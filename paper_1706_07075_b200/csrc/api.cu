@@ -69,13 +69,22 @@ struct tofmlem_ctx {
     uint2 *d_chunks = nullptr;
     size_t chunks_cap = 0;
     unsigned *d_plan_flags = nullptr;  // [0] tile work counter, [1] "keys not sorted" flag
+    RecPtrs d_rec{nullptr, nullptr, nullptr};  // ray records of the planned list (prepared.cuh), 48 B per event
+    size_t rec_cap = 0;
+    uint32_t *d_strag = nullptr;       // events of tile items that do not fit their tile
+    size_t strag_cap = 0;
+    float *d_ev_scale = nullptr;       // w_e / fwd_e of the tile events between the two phases of tile.cu (rec_cap floats)
+    size_t smem_per_sm = 0;
+    void *d_plan_counters = nullptr;
     struct {
         bool valid = false;
         const float *x1 = nullptr;  // the plan describes THIS event list (first member array) ...
         uint64_t n = 0;             // ... of this length, binned with
-        int tile_log2 = 0;          // ... this cube size
-        uint32_t n_items = 0, n_chunks = 0;
-        uint64_t tile_events = 0, direct_events = 0;
+        int tile_log2 = 0;          // ... this cube size, for a context with
+        double sigma = 0.0, trunc = 0.0;  // ... this TOF kernel
+        int brick = 0;              // ... and this layout of the correction image
+        uint32_t n_items = 0, n_chunks = 0, n_strag = 0, max_item_events = 0;
+        uint64_t tile_events = 0, direct_events = 0, valid_events = 0, visits = 0;
         int sorted = 0;
     } plan;
     std::string err;
@@ -210,6 +219,19 @@ int ensure_bin_scratch(tofmlem_ctx *ctx, size_t nfine, uint64_t n_sub) {
     return TOFMLEM_OK;
 }
 
+void free_records(tofmlem_ctx *ctx) {
+    cudaFree(ctx->d_rec.a);
+    cudaFree(ctx->d_rec.b);
+    cudaFree(ctx->d_rec.c);
+    cudaFree(ctx->d_strag);
+    cudaFree(ctx->d_ev_scale);
+    ctx->d_rec = RecPtrs{nullptr, nullptr, nullptr};
+    ctx->d_strag = nullptr;
+    ctx->d_ev_scale = nullptr;
+    ctx->rec_cap = ctx->strag_cap = 0;
+    ctx->plan.valid = false;
+}
+
 // 32-byte event records of tofmlem_permute_events (grows only).  false: not enough memory (the caller falls back).
 bool ensure_pack(tofmlem_ctx *ctx, uint64_t n) {
     if (ctx->pack_cap >= n) return true;
@@ -279,6 +301,12 @@ int ensure_lut(tofmlem_ctx *ctx) {
     return TOFMLEM_OK;
 }
 
+// Does the context hold ray records for exactly this list and this TOF kernel?
+bool plan_matches(const tofmlem_ctx *c, const float *x1, uint64_t n) {
+    return c->plan.valid && c->plan.x1 == x1 && c->plan.n == n && c->plan.tile_log2 == c->tile_log2 && c->tof &&
+           c->projector == 0 && c->plan.sigma == c->sigma && c->plan.trunc == c->trunc_sigmas;
+}
+
 // One fused EM pass with the context's projector (0 = Siddon x Gaussian, 1 = K-sample kernel).
 int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint64_t n, const float *evw,
             const float *d_image, float *d_corr, bool vec, cudaStream_t s) {
@@ -289,28 +317,26 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         int rc = ensure_lut(ctx);
         if (rc) return rc;
         launch_sampled_em(p, ctx->d_lut, ctx->samples_k, ev, n, evw, d_image, d_corr, ctx->d_stats, ctx->d_queues, s);
-    } else if (ctx->plan.valid && ctx->plan.x1 == ev.x1 && ctx->plan.n == n && ctx->plan.tile_log2 == ctx->tile_log2 &&
-               ctx->tof && vec && ctx->em_variant == 0 && ctx->plan.n_items > 0) {
-        // Tile mode (tile.cu): the list is the one tofmlem_plan_events looked at.  The geometry of the tiles follows the
-        // CURRENT window (trunc_sigmas may have changed since the plan, which only depends on the keys).
-        TileGeom g;
-        build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);
-        if (!g.ok) {
-            launch_em_correction(p, ctx->tof, ev, n, evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, s);
+    } else if (plan_matches(ctx, ev.x1, n) && ctx->plan.brick == p.brick && ctx->em_variant == 0) {
+        // Planned list (tofmlem_plan_events): the pass runs on the ray records -- the items on shared-memory tiles
+        // (tile.cu), the other events and the stragglers of the items through the direct pass on records (prepared.cu).
+        const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 1;
+        if (ctx->plan.n_items) {
+            TileGeom g;
+            build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);  // the same as at plan time (sigma, trunc match)
+            launch_em_tile(p, g, ctx->d_geom, ctx->tile_log2, ctx->d_rec, evw, d_image, d_corr, ctx->d_stats,
+                           ctx->d_items, ctx->plan.n_items, ctx->d_plan_flags, n_sm, ctx->smem_per_sm,
+                           ctx->tile_check != 0, ctx->sigma, ctx->plan.max_item_events, ctx->d_ev_scale, s);
             CHECK_LAUNCH(1);
-            return TOFMLEM_OK;
         }
-        if (!ctx->d_geom) CU(cudaMalloc(&ctx->d_geom, sizeof(TileGeom)));
-        if (memcmp(&g, &ctx->h_geom_sent, sizeof g) != 0) {
-            ctx->h_geom_sent = g;
-            CU(cudaMemcpyAsync(ctx->d_geom, &ctx->h_geom_sent, sizeof g, cudaMemcpyHostToDevice, s));
-        }
-        launch_em_tile(p, g, ctx->d_geom, ctx->tile_log2, ev, evw, d_image, d_corr, ctx->d_stats, ctx->d_items,
-                       ctx->plan.n_items, ctx->d_plan_flags, ctx->n_sm > 0 ? ctx->n_sm : 1, ctx->tile_check != 0, s);
-        CHECK_LAUNCH(1);
         if (ctx->plan.n_chunks) {
-            launch_em_correction_chunks(p, true, ev, n, ctx->d_chunks, ctx->plan.n_chunks, evw, d_image, d_corr, vec,
-                                        ctx->d_stats, ctx->d_queues, s);
+            launch_em_planned(p, ev, ctx->d_rec, ctx->d_chunks, nullptr, ctx->plan.n_chunks, 0, evw, d_image, d_corr, vec,
+                              ctx->d_stats, ctx->d_queues, n_sm, s);
+            CHECK_LAUNCH(1);
+        }
+        if (ctx->plan.n_strag) {
+            launch_em_planned(p, ev, ctx->d_rec, nullptr, ctx->d_strag, (ctx->plan.n_strag + 31u) / 32u, ctx->plan.n_strag,
+                              evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, n_sm, s);
             CHECK_LAUNCH(1);
         }
         return TOFMLEM_OK;
@@ -386,6 +412,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
         if (cudaGetDevice(&dev) == cudaSuccess) {
             if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) ctx->n_sm = v;
             if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess) ctx->smem_optin = (size_t)v;
+            if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev) == cudaSuccess) ctx->smem_per_sm = (size_t)v;
         }
         cudaGetLastError();
     }
@@ -394,6 +421,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_queues, kMaxQueues * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_rcounts, 2 * (kMaxRegions + 1) * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_flags, 2 * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_counters, plan_counter_bytes());
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_stats, 0, sizeof(DeviceStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_max, 0, sizeof(float), ctx->stream);
     if (e != cudaSuccess) {
@@ -403,6 +431,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
         cudaFree(ctx->d_queues);
         cudaFree(ctx->d_rcounts);
         cudaFree(ctx->d_plan_flags);
+        cudaFree(ctx->d_plan_counters);
         delete ctx;
         return rc;
     }
@@ -442,6 +471,8 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_geom);
     cudaFree(ctx->d_items);
     cudaFree(ctx->d_chunks);
+    cudaFree(ctx->d_plan_counters);
+    free_records(ctx);
     delete ctx;
     return TOFMLEM_OK;
 }
@@ -553,6 +584,7 @@ int tofmlem_trim(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_hev);
     cudaFree(ctx->d_himg);
     cudaFree(ctx->d_hsens);
+    free_records(ctx);  // the plan goes with its records
     ctx->d_pack = nullptr;
     ctx->d_sub = nullptr;
     ctx->d_rg_region = nullptr;
@@ -587,6 +619,8 @@ int tofmlem_forward(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, cons
         if (rc) return rc;
         launch_sampled_forward(make_params(ctx, true), ctx->d_lut, ctx->samples_k, ev_ptrs(ev), n, d_image, d_fwd,
                                ctx->stream);
+    } else if (plan_matches(ctx, ev->x1, n)) {  // planned list: the walk of the fused pass, on the ray records
+        launch_planned_forward(make_params(ctx, true), ctx->sigma, ev_ptrs(ev), ctx->d_rec, n, d_image, d_fwd, ctx->stream);
     } else {
         launch_forward(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_fwd, ctx->stream);
     }
@@ -795,63 +829,91 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
 int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) {
     if (!ctx) return TOFMLEM_EINVAL;
     ctx->plan.valid = false;
-    ctx->plan.n_items = ctx->plan.n_chunks = 0;
-    ctx->plan.tile_events = ctx->plan.direct_events = 0;
+    ctx->plan.n_items = ctx->plan.n_chunks = ctx->plan.n_strag = 0;
+    ctx->plan.tile_events = ctx->plan.direct_events = ctx->plan.valid_events = ctx->plan.visits = 0;
     ctx->plan.sorted = 0;
     if (n == 0) return TOFMLEM_OK;
     if (!ev_ok(ev, ctx->tof) || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "plan_events: bad argument");
-    if (!ctx->tof || ctx->projector != 0) return TOFMLEM_OK;  // tile mode exists for the TOF Siddon pass only
-    {
-        TileGeom g;
-        build_tile_geom(make_params(ctx, true), ctx->tile_log2, ctx->smem_optin, g);
-        if (!g.ok) return TOFMLEM_OK;  // the tiles of this window do not fit in shared memory: direct pass
-    }
-    const uint32_t nb = num_bins(ctx);
-    int rc = ensure_bin_scratch(ctx, (size_t)nb + 1, 0);
-    if (rc) return rc;
+    if (!ctx->tof || ctx->projector != 0) return TOFMLEM_OK;  // records exist for the TOF Siddon pass only
+    ProjParams p = make_params(ctx, true);
+    // the layout the context's own correction image will have (ensure_corr aligns it): decides which group count the
+    // direct records carry; a pass into another layout ignores the plan
+    p.brick = ctx->corr_bricks && (ctx->grid.nx & 1) == 0 && (ctx->grid.ny & 1) == 0 && (ctx->nvox & 3) == 0 ? 1 : 0;
+    TileGeom g;
+    build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);
     cudaStream_t s = ctx->stream;
-    CU(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)nb + 1) * sizeof(uint32_t), s));
-    CU(cudaMemsetAsync(ctx->d_plan_flags, 0, 2 * sizeof(unsigned), s));
-    launch_plan_hist(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, ctx->d_hist, nb, ctx->d_plan_flags + 1, s);
-    CHECK_LAUNCH(1);
-    std::vector<uint32_t> cnt(nb);
-    unsigned flags[2] = {0, 0};
-    CU(cudaMemcpyAsync(cnt.data(), ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-    CU(cudaMemcpyAsync(flags, ctx->d_plan_flags, sizeof flags, cudaMemcpyDeviceToHost, s));
-    CU(cudaStreamSynchronize(s));
-    ctx->plan.sorted = flags[1] ? 0 : 1;
-    if (flags[1]) return TOFMLEM_OK;  // not sorted by key: the bins are not contiguous, direct pass
-    // bins with at least tile_min_events events become tile work (pieces of at most tile_max_events, whole warps);
-    // maximal runs of the other bins are cut into 32-event pieces for the direct pass
+    // ---- which bins become tile items?  Needs a list sorted by key (tofmlem_permute_events) and tiles that fit.
     std::vector<TileItem> items;
     std::vector<uint2> chunks;
-    const uint32_t thr = (uint32_t)ctx->tile_min_events, mx = (uint32_t)ctx->tile_max_events;
-    uint64_t off = 0, run_lo = 0, run_hi = 0, n_tile = 0, n_direct = 0;
-    auto flush_run = [&]() {
-        for (uint64_t a = run_lo; a < run_hi; a += 32)
-            chunks.push_back(make_uint2((unsigned)a, (unsigned)(run_hi - a < 32 ? run_hi - a : 32)));
-        n_direct += run_hi - run_lo;
-        run_lo = run_hi = 0;
+    uint64_t in_items = 0;
+    auto add_run = [&](uint64_t lo, uint64_t hi) {
+        for (uint64_t a = lo; a < hi; a += 32)
+            chunks.push_back(make_uint2((unsigned)a, (unsigned)(hi - a < 32 ? hi - a : 32)));
     };
-    for (uint32_t b = 0; b < nb; ++b) {
-        const uint32_t c = cnt[b];
-        if (c == 0) continue;
-        if (c >= thr) {
-            if (run_hi > run_lo) flush_run();
-            const uint32_t pieces = (c + mx - 1) / mx;
-            uint32_t per = (c + pieces - 1) / pieces;
-            per = (per + 31u) & ~31u;
-            for (uint32_t a = 0; a < c; a += per)
-                items.push_back(TileItem{(uint32_t)(off + a), c - a < per ? c - a : per, b, 0u});
-            n_tile += c;
-        } else {
-            if (run_hi == run_lo) run_lo = off;
-            run_hi = off + c;
+    bool sorted = false;
+    if (g.ok) {
+        const uint32_t nb = num_bins(ctx);
+        int rc = ensure_bin_scratch(ctx, (size_t)nb + 1, 0);
+        if (rc) return rc;
+        CU(cudaMemsetAsync(ctx->d_hist, 0, ((size_t)nb + 1) * sizeof(uint32_t), s));
+        CU(cudaMemsetAsync(ctx->d_plan_flags, 0, 2 * sizeof(unsigned), s));
+        launch_plan_hist(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, ctx->d_hist, nb, ctx->d_plan_flags + 1, s);
+        CHECK_LAUNCH(1);
+        std::vector<uint32_t> cnt(nb);
+        unsigned flags[2] = {0, 0};
+        CU(cudaMemcpyAsync(cnt.data(), ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(flags, ctx->d_plan_flags, sizeof flags, cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+        sorted = flags[1] == 0;
+        if (sorted) {
+            // bins with at least tile_min_events events become tile work (pieces of at most tile_max_events, whole
+            // warps); maximal runs of the other bins are cut into 32-event pieces for the direct pass
+            const uint32_t thr = (uint32_t)ctx->tile_min_events, mx = (uint32_t)ctx->tile_max_events;
+            uint64_t off = 0, run_lo = 0, run_hi = 0;
+            for (uint32_t b = 0; b < nb; ++b) {
+                const uint32_t c = cnt[b];
+                if (c == 0) continue;
+                if (c >= thr) {
+                    if (run_hi > run_lo) add_run(run_lo, run_hi);
+                    run_lo = run_hi = 0;
+                    const uint32_t pieces = (c + mx - 1) / mx;
+                    uint32_t per = (c + pieces - 1) / pieces;
+                    per = (per + 31u) & ~31u;
+                    for (uint32_t a = 0; a < c; a += per)
+                        items.push_back(TileItem{(uint32_t)(off + a), c - a < per ? c - a : per, b, 0u});
+                    in_items += c;
+                } else {
+                    if (run_hi == run_lo) run_lo = off;
+                    run_hi = off + c;
+                }
+                off += c;
+            }
+            if (run_hi > run_lo) add_run(run_lo, run_hi);
+            if (off < n) add_run(off, n);  // events with an invalid key (sorted to the end): their records are invalid
         }
-        off += c;
     }
-    if (run_hi > run_lo) flush_run();
-    if (items.empty()) return TOFMLEM_OK;
+    ctx->plan.sorted = sorted ? 1 : 0;
+    if (items.empty()) {  // no tiles (window too wide, unsorted list, sparse bins): the whole list in order
+        chunks.clear();
+        add_run(0, n);
+        in_items = 0;
+    }
+    // ---- scratch (grows only)
+    if (ctx->rec_cap < n) {
+        free_records(ctx);
+        CU(cudaMalloc(&ctx->d_rec.a, n * sizeof(float4)));
+        CU(cudaMalloc(&ctx->d_rec.b, n * sizeof(float4)));
+        CU(cudaMalloc(&ctx->d_rec.c, n * sizeof(uint4)));
+        CU(cudaMalloc(&ctx->d_ev_scale, n * sizeof(float)));
+        ctx->rec_cap = n;
+    }
+    if (ctx->strag_cap < in_items) {
+        cudaFree(ctx->d_strag);
+        ctx->d_strag = nullptr;
+        ctx->strag_cap = 0;
+        CU(cudaMalloc(&ctx->d_strag, in_items * sizeof(uint32_t)));
+        ctx->strag_cap = in_items;
+    }
     if (ctx->items_cap < items.size()) {
         cudaFree(ctx->d_items);
         ctx->d_items = nullptr;
@@ -866,18 +928,42 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMalloc(&ctx->d_chunks, chunks.size() * sizeof(uint2)));
         ctx->chunks_cap = chunks.size();
     }
-    CU(cudaMemcpyAsync(ctx->d_items, items.data(), items.size() * sizeof(TileItem), cudaMemcpyHostToDevice, s));
+    if (!items.empty()) {
+        if (!ctx->d_geom) CU(cudaMalloc(&ctx->d_geom, sizeof(TileGeom)));
+        if (memcmp(&g, &ctx->h_geom_sent, sizeof g) != 0) {
+            ctx->h_geom_sent = g;
+            CU(cudaMemcpyAsync(ctx->d_geom, &ctx->h_geom_sent, sizeof g, cudaMemcpyHostToDevice, s));
+        }
+        CU(cudaMemcpyAsync(ctx->d_items, items.data(), items.size() * sizeof(TileItem), cudaMemcpyHostToDevice, s));
+    }
     if (!chunks.empty())
         CU(cudaMemcpyAsync(ctx->d_chunks, chunks.data(), chunks.size() * sizeof(uint2), cudaMemcpyHostToDevice, s));
+    // ---- the records: fp64 set-up, quantisation, dry run against the tile (prepared.cu)
+    launch_prepare_rays(p, ctx->sigma, items.empty() ? nullptr : ctx->d_geom, ctx->tile_log2, ev_ptrs(ev), n, ctx->d_items,
+                        (uint32_t)items.size(), ctx->d_rec, ctx->d_strag, ctx->d_plan_counters, s);
+    CHECK_LAUNCH(1);
+    std::vector<unsigned char> hc(plan_counter_bytes());
+    CU(cudaMemcpyAsync(hc.data(), ctx->d_plan_counters, hc.size(), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
+    uint64_t cnt4[4];
+    read_plan_counters(hc.data(), cnt4);
     ctx->plan.valid = true;
     ctx->plan.x1 = ev->x1;
     ctx->plan.n = n;
     ctx->plan.tile_log2 = ctx->tile_log2;
+    ctx->plan.sigma = ctx->sigma;
+    ctx->plan.trunc = ctx->trunc_sigmas;
+    ctx->plan.brick = p.brick;
     ctx->plan.n_items = (uint32_t)items.size();
+    ctx->plan.max_item_events = 0;
+    for (const TileItem &it : items)
+        if (it.count > ctx->plan.max_item_events) ctx->plan.max_item_events = it.count;
     ctx->plan.n_chunks = (uint32_t)chunks.size();
-    ctx->plan.tile_events = n_tile;
-    ctx->plan.direct_events = n_direct;
+    ctx->plan.n_strag = (uint32_t)cnt4[2];
+    ctx->plan.valid_events = cnt4[0];
+    ctx->plan.tile_events = cnt4[1];
+    ctx->plan.direct_events = n - cnt4[1];
+    ctx->plan.visits = cnt4[3];
     return TOFMLEM_OK;
 }
 

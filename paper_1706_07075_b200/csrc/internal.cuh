@@ -5,6 +5,7 @@
 
 #include <string>
 
+#include "prepared.cuh"
 #include "tofmlem.h"
 
 namespace tofmlem {
@@ -87,11 +88,31 @@ struct TileItem {
 // false (g.ok = 0) when a tile pair does not fit in `smem_budget` bytes of shared memory
 void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, TileGeom &g);
 size_t tile_smem_bytes(const TileGeom &g);
-// d_geom: the same structure in device memory
-void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const EventPtrs &ev,
+// d_geom: the same structure in device memory; rec: the ray records of the planned list (prepared.cuh)
+void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const RecPtrs &rec,
                     const float *evw, const float *image, float *corr, DeviceStats *stats, const TileItem *items,
-                    uint32_t n_items, unsigned *counter /* one word, zeroed by the call */, int n_sm, bool check,
+                    uint32_t n_items, unsigned *counter /* one word, zeroed by the call */, int n_sm,
+                    size_t smem_per_sm, bool check, double sigma, uint32_t max_item_events /* no item holds more */,
+                    float *ev_scale /* one float per event of the list: scratch between the two phases */,
                     cudaStream_t s);
+
+// ---- prepared.cu: ray records of a planned list and the passes that run on them
+// Writes one record per event (p.brick says which group count the direct records carry), appends the events of tile
+// items that do not fit their tile to `stragglers` (room for every event of a tile item) and fills the counters
+// (plan_counter_bytes() bytes of device memory; read_plan_counters: valid events, tile events, stragglers, visits).
+size_t plan_counter_bytes();
+void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom /* NULL: no tiles */, int tile_log2,
+                         const EventPtrs &ev, uint64_t n, const TileItem *items, uint32_t n_items, const RecPtrs &rec,
+                         uint32_t *stragglers, void *d_counters, cudaStream_t s);
+void read_plan_counters(const void *h_counters, uint64_t out[4]);
+// ev: the raw events of the planned list (the kRecTiny records are walked from them)
+void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &ev, const RecPtrs &rec, uint64_t n,
+                            const float *image, float *fwd, cudaStream_t s);
+// chunks: n_pieces (first event, count <= 32) pairs; or index: n_index event numbers, 32 per piece
+void launch_em_planned(const ProjParams &p, const EventPtrs &ev, const RecPtrs &rec, const uint2 *chunks,
+                       const uint32_t *index,
+                       uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
+                       bool vec_ok, DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s);
 
 // ---- image_ops.cu
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);

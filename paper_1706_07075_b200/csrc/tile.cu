@@ -6,10 +6,15 @@
 // at which an SM can hand requests to the crossbar (ncu r04: 3.6e9 reductions, 0.88 of the measured request rate), and
 // its image gathers keep the L1 data pipe 76 % busy with ~27 sectors per warp-wide load.  Events are sorted by
 // locality key (direction class x cube of T^3 voxels holding the TOF centre), so the +-3 sigma windows of the events
-// of one bin cover a small double cone around the cube (7.8 k voxels at 300 ps / 3.75 mm; its bounding box would be
-// 35 k).  One CTA per SM takes a bin, copies the image values of that cone into shared memory, walks all events of
-// the bin with both the gathers (LDS) and the accumulation (shared-memory atomics) on the tile, and adds the tile to
-// the global correction image once.  Bins with few events stay on the direct pass (the plan, api.cu, decides).
+// of one bin cover a small double cone around the cube (18.5 k voxels at 300 ps / 3.75 mm in the plane-by-plane layout
+// below; its bounding box would be 43 k).  A CTA takes a bin ("item") and works in two phases on ONE tile buffer:
+//   A. the tile holds the IMAGE values of the cone: every event of the item is walked forward (LDS gathers), its
+//      w_e / fwd_e goes to a per-event scratch array and its exponent into a histogram;
+//   B. the tile is cleared and becomes the CORRECTION tile: every event is walked again and adds its chord weights
+//      with shared-memory integer atomics (fixed point, see the kernel); the tile is then added to the global
+//      correction image once.
+// One buffer instead of an image/correction pair means three CTAs (items) per SM at cfg-3, which overlap each other's
+// barriers, tile loads and flushes.  Bins with few events stay on the direct pass (the plan, api.cu, decides).
 //
 // Tile layout: plane by plane along the class's dominant axis a; plane p holds a W[0] x W[1] rectangle of the lateral
 // axes (f fast, s slow) whose low corner follows the cone (TileGeom::lo, closed-form envelopes + 1 voxel of slack on
@@ -17,22 +22,22 @@
 // +-(plane stride - shift of the rectangle), read from a per-plane table in shared memory.  The weights are computed
 // by exactly the arithmetic of the direct walk (walk.cuh), so both passes give the same forward values.
 //
-// Safety: an event uses the tile only if its TOF centre lies in the bin's cube and its direction in the bin's class,
-// checked in fp64 inside the kernel (the envelopes are derived from exactly these two facts), and its first voxel lies
-// inside the tile; every other event of the bin (the float32 key put it there by a rounding, or its centre was
-// clamped to the grid edge) takes the direct walk.  TOFMLEM_OPT_TILE_CHECK adds a bounds test to every tile access.
+// The pass runs on the ray records of a planned list (prepared.cuh): the per-event fp64 set-up is done once by
+// tofmlem_plan_events, which also DRY-RUNS the walk of every event of a tile item against the item's tile and marks
+// the event for the tile only if every voxel of its window lies inside; the few others (the float32 key put them in
+// the bin by a rounding, or their centre was clamped to the grid edge) go to the direct pass as stragglers.  The walk
+// here therefore needs no bounds test.  The record's exact-add arithmetic makes the dry run and this walk visit the
+// same voxels bit for bit.
 #include <math.h>
 #include <string.h>
 
 #include "internal.cuh"
-#include "walk.cuh"
+#include "prepared.cuh"
 
 namespace tofmlem {
 
-constexpr int kTileThreads = 1024;
-
 size_t tile_smem_bytes(const TileGeom &g) {
-    return ((size_t)2 * g.words + 3 * kTileMaxPlanes + 8) * sizeof(float);
+    return ((size_t)g.words + 4 * (kTileMaxPlanes + 1) + 8 + 256) * sizeof(float);
 }
 
 void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, TileGeom &g) {
@@ -79,40 +84,13 @@ __device__ __forceinline__ int sel3(int a, int v0, int v1, int v2) { return a ==
 __device__ __forceinline__ float sel3(int a, float v0, float v1, float v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
 __device__ __forceinline__ double sel3(int a, double v0, double v1, double v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
 
+
 // Geometry of the bin a CTA is working on (uniform over the CTA).
 struct Residency {
     int a;             // dominant axis; f = (a == 0 ? 1 : 0), s = (a == 2 ? 1 : 2)
     int ca, cf, cs;    // cube origin (voxels) along a, f, s
     int sgf, sgs;      // +1 / -1: the class's rays run towards +f (+s) or -f (-s) while moving towards +a
     int RA, PA, Wf, Ws, PS, T;
-};
-
-// The walk of walk.cuh's Walker on the tile: same crossing arithmetic (so the same weights), tile-local index.
-struct TileWalker {
-    float ta, tf, ts, ka, kf, ks, t;
-    int li, pq;
-    __device__ __forceinline__ float step(float gauss_a, float t_end, float tc, float t0a, float t0f, float t0s,
-                                          float tda, float tdf, float tds, const int *__restrict__ ainc, int dir_a,
-                                          int inc_f, int inc_s, int &at, bool &done) {
-        const float tn = fminf(fminf(ta, tf), fminf(ts, t_end));
-        const float l = tn - t;
-        const float tm = fmaf(0.5f, t + tn, -tc);
-        const float w = l * ex2_approx(gauss_a * tm * tm);
-        at = li;
-        done = tn >= t_end;
-        if (ta <= tn) {
-            ka += 1.0f;
-            li += dir_a * ainc[pq];
-            pq += dir_a;
-        }
-        if (tf <= tn) { kf += 1.0f; li += inc_f; }
-        if (ts <= tn) { ks += 1.0f; li += inc_s; }
-        ta = fmaf(ka, tda, t0a);
-        tf = fmaf(kf, tdf, t0f);
-        ts = fmaf(ks, tds, t0s);
-        t = tn;
-        return w;
-    }
 };
 
 // flat index of voxel (x, y, z) in the correction image
@@ -122,75 +100,149 @@ __device__ __forceinline__ int corr_index(int x, int y, int z, int nx, int ny) {
     return (z * ny + y) * nx + x;
 }
 
-// Visits every word of the bin's tile once, lanes running along x (global memory rows): op(tile index, x, y, z) for
-// the words whose voxel lies in the grid, op_out(tile index) for the others.
-template <typename In, typename Out>
+// Visits every word of the bin's tile once: op(tile index, x, y, z) for the words whose voxel lies in the grid,
+// op_out(tile index) for the others.  A warp takes whole planes (everything that depends on the plane only is
+// warp-uniform), its lanes sweep the plane's W[0] x W[1] rectangle in tile order, which is x-fastest in global memory
+// for the classes whose dominant axis is y or z.  (ncu on the first form, rows of 21 words per 32 lanes and two integer
+// divisions per row: the tile load and flush were 32 % of the kernel's instructions.)
+template <int NT, typename In, typename Out>
 __device__ __forceinline__ void for_each_tile_voxel(const Residency &R, const int *__restrict__ lof,
                                                     const int *__restrict__ los, int nx, int ny, int nz, In op,
                                                     Out op_out) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int a = R.a;
     const int na = sel3(a, nx, ny, nz), nf = a == 0 ? ny : nx, ns = a == 2 ? ny : nz;
-    if (a != 0) {  // f = x: a row of a plane's rectangle is a run of x
-        for (int row = warp; row < R.PA * R.Ws; row += kTileThreads / 32) {
-            const int p = row / R.Ws, ls = row - p * R.Ws;
-            const int ia = R.ca + p - R.RA;
-            const int n_s = ls + los[p];
-            const int is = R.sgs > 0 ? R.cs + n_s : R.cs + R.T - 1 - n_s;
-            const bool row_in = ia >= 0 && ia < na && is >= 0 && is < ns;
-            const int lo_f = lof[p];
-            for (int lf = lane; lf < R.Wf; lf += 32) {
-                const int n_f = lf + lo_f;
-                const int i_f = R.sgf > 0 ? R.cf + n_f : R.cf + R.T - 1 - n_f;
-                const int ti = p * R.PS + ls * R.Wf + lf;
-                if (row_in && i_f >= 0 && i_f < nf) {
-                    if (a == 1) op(ti, i_f, ia, is); else op(ti, i_f, is, ia);
-                } else {
-                    op_out(ti);
-                }
-            }
-        }
-    } else {  // a = x: the planes are consecutive in x
-        for (int col = warp; col < R.Wf * R.Ws; col += kTileThreads / 32) {
-            const int ls = col / R.Wf, lf = col - ls * R.Wf;
-            for (int p = lane; p < R.PA; p += 32) {
-                const int ia = R.ca + p - R.RA;
-                const int n_f = lf + lof[p], n_s = ls + los[p];
-                const int i_f = R.sgf > 0 ? R.cf + n_f : R.cf + R.T - 1 - n_f;
-                const int is = R.sgs > 0 ? R.cs + n_s : R.cs + R.T - 1 - n_s;
-                const int ti = p * R.PS + col;
-                if (ia >= 0 && ia < na && i_f >= 0 && i_f < nf && is >= 0 && is < ns) op(ti, ia, i_f, is);
-                else op_out(ti);
+    const int rect = R.Wf * R.Ws;
+    const unsigned magic = 65536u / (unsigned)R.Wf + 1u;  // i / Wf = (i * magic) >> 16 for i < 2^16 / Wf (rect <= 2^11)
+    const int bf = R.sgf > 0 ? R.cf : R.cf + R.T - 1, bs = R.sgs > 0 ? R.cs : R.cs + R.T - 1;
+    for (int p = warp; p < R.PA; p += NT / 32) {
+        const int ia = R.ca + p - R.RA;
+        const bool plane_in = ia >= 0 && ia < na;
+        const int of = bf + R.sgf * lof[p], os = bs + R.sgs * los[p];  // voxel of the rectangle's corner (0, 0)
+        const int base = p * R.PS;
+        for (int i = lane; i < rect; i += 32) {
+            const int ls = (int)(((unsigned)i * magic) >> 16), lf = i - ls * R.Wf;
+            const int i_f = of + R.sgf * lf, is = os + R.sgs * ls;
+            if (plane_in && (unsigned)i_f < (unsigned)nf && (unsigned)is < (unsigned)ns) {
+                if (a == 0) op(base + i, ia, i_f, is);
+                else if (a == 1) op(base + i, i_f, ia, is);
+                else op(base + i, i_f, is, ia);
+            } else {
+                op_out(base + i);
             }
         }
     }
 }
 
-template <bool BRICK, bool CHECK>
-__global__ void __launch_bounds__(kTileThreads, 1)
-em_tile_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, EventPtrs ev,
+// Shared-memory accesses by 32-bit byte address (the walk keeps its tile index as the address itself: no index
+// arithmetic per step).
+__device__ __forceinline__ float lds_f32(unsigned addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void red_shared_u32(unsigned addr, unsigned v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");  // ATOMS.ADD, no loop, no return
+}
+
+// if (ta <= tn) { ta += da; li += na; pq += dpq; na = *pq; }: the step along the tile's plane axis.  pq is the ADDRESS of
+// the current plane's entry in the increment table; the increment of the NEXT plane change is fetched right away (na),
+// so the table look-up is off the critical path.
+__device__ __forceinline__ void advance_plane(float &ta, unsigned &li, int &na, unsigned &pq, float tn, float da,
+                                              int dpq) {
+    asm volatile(
+        "{\n .reg .pred p;\n setp.le.f32 p, %0, %4;\n @p add.f32 %0, %0, %5;\n @p add.s32 %1, %1, %2;\n"
+        " @p add.s32 %3, %3, %6;\n @p ld.shared.s32 %2, [%3];\n}"
+        : "+f"(ta), "+r"(li), "+r"(na), "+r"(pq)
+        : "f"(tn), "f"(da), "r"(dpq));
+}
+
+__device__ __forceinline__ void advance_addr(float &tx, unsigned &li, float tn, float dx, int inc) {
+    asm("{\n .reg .pred p;\n setp.le.f32 p, %0, %2;\n @p add.f32 %0, %0, %3;\n @p add.s32 %1, %1, %4;\n}"
+        : "+f"(tx), "+r"(li)
+        : "f"(tn), "f"(dx), "r"(inc));
+}
+
+// Fixed-point accumulation of the correction tile (see the kernel).
+constexpr int kMedianBits = 4;
+struct FixedPoint {
+    float lmax;  // longest chord a voxel can hold, t units (kappa x voxel diagonal)
+    float qmax;  // an event's contributions stay below this many quanta: 2^31 / tile_max_events
+    float qmin;  // ... and its longest possible chord is worth at least this many
+    int qexp;    // floor(log2(qmax / lmax))
+};
+
+// The rare event of a tile item whose w_e / fwd_e does not suit the item's fixed-point scale: float32 reductions into the
+// global correction image, one per voxel.  The record is in the tile's (a, f, s) axis order with the grid directions in
+// c.w (prepared.cuh); the brick layout index is formed from the flat one per voxel.
+template <bool BRICK>
+__device__ __noinline__ void scatter_global(float4 ra, float4 rb, uint4 rc, int nx, int ny, float *__restrict__ corr,
+                                            float scale) {
+    const int a = (int)((rc.y >> kRecAxisShift) & 3u), f = a == 0 ? 1 : 0, s = a == 2 ? 1 : 2;
+    const int st[3] = {1, nx, nx * ny};
+    const int i0 = (rc.w & 1u) ? -st[a] : st[a], i1 = (rc.w & 2u) ? -st[f] : st[f], i2 = (rc.w & 4u) ? -st[s] : st[s];
+    float t = ra.x, t0 = ra.z, t1 = ra.w, t2 = rb.x;
+    int at = (int)rc.x;
+    auto put = [&](float w) {
+        int j = at;
+        if (BRICK) {
+            const int z = at / (nx * ny), rem = at - z * nx * ny, y = rem / nx, x = rem - y * nx;
+            j = ((z * (ny >> 1) + (y >> 1)) * (nx >> 1) + (x >> 1)) * 4 + ((y & 1) << 1) + (x & 1);
+        }
+        atomicAdd(corr + j, w * scale);
+    };
+    while (true) {
+        const float tn = min3f(t0, t1, t2);
+        if (!(tn < ra.y)) break;
+        put(chord_weight(t, tn));
+        advance_axis(t0, at, tn, rb.y, i0);
+        advance_axis(t1, at, tn, rb.z, i1);
+        advance_axis(t2, at, tn, rb.w, i2);
+        t = tn;
+    }
+    put(chord_weight(t, ra.y));
+}
+
+// CHECK (TOFMLEM_OPT_TILE_CHECK, a debugging aid): every tile access is bounds-tested and violations are counted in
+// tofmlem_stats.tile_oob (must stay 0: the plan's dry run has already walked every event against its tile).
+//
+// Fixed point: shared memory has a native 32-bit integer add (ATOMS.ADD) but no float add -- atomicAdd(float) is a
+// compare-and-swap loop whose retries split the warp for the rest of the walk (ncu on the float form: the scatter loop
+// ran with 14 of 32 lanes, twice the instructions).  Scale of an item: S, a power of two, puts the MEDIAN of its
+// events' w_e / fwd_e (histogram of float exponents, phase A) kMedianBits below fx.qmax = 2^31 / (largest item) quanta
+// for the longest possible chord; no contribution exceeds qmax, so no voxel can overflow whatever the item holds.  An
+// event whose largest possible contribution would exceed qmax (w_e / fwd_e more than ~16 x the median: a window that
+// barely touches activity) or stay below fx.qmin = 1024 quanta (rounding error of a contribution <= 2^-11 of the
+// event's longest chord) adds float32 values to the global correction image instead.  Rounding is to nearest.
+template <int NT, int NCTA, bool BRICK, bool CHECK>
+__global__ void __launch_bounds__(NT, NCTA)
+em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile_log2, RecPtrs rec,
                const float *__restrict__ evw, const float *__restrict__ image, float *__restrict__ corr,
-               DeviceStats *stats, const TileItem *__restrict__ items, unsigned n_items, unsigned *counter) {
+               DeviceStats *stats, const TileItem *__restrict__ items, unsigned n_items, unsigned *counter,
+               FixedPoint fx, float *__restrict__ ev_scale) {
     extern __shared__ __align__(16) float smem[];
     const int words = Gp->words;
-    float *img = smem;
-    float *acc = smem + words;
-    int *ainc = reinterpret_cast<int *>(smem + 2 * words);
-    int *lof = ainc + kTileMaxPlanes;
-    int *los = lof + kTileMaxPlanes;
-    unsigned *ctl = reinterpret_cast<unsigned *>(los + kTileMaxPlanes);  // [0] item, [1] next chunk of the item
+    float *tile = smem;
+    // plane tables: up[p] = byte increment of a step from plane p to p + 1, dn[p] = from p to p - 1; lof / los
+    int *up = reinterpret_cast<int *>(smem + words);
+    int *dn = up + (kTileMaxPlanes + 1);
+    int *lof = dn + (kTileMaxPlanes + 1);
+    int *los = lof + (kTileMaxPlanes + 1);
+    unsigned *ctl = reinterpret_cast<unsigned *>(los + (kTileMaxPlanes + 1));  // [0] item, [1] / [2] next chunk of A / B
+    unsigned *hist = ctl + 8;  // 256 bins: float exponent of w_e / fwd_e
     const unsigned tid = threadIdx.x, lane = tid & 31u;
-    for (int i = tid; i < words; i += kTileThreads) acc[i] = 0.0f;
-    const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
+    const unsigned tile_addr = (unsigned)__cvta_generic_to_shared(tile);
+    const unsigned up_addr = (unsigned)__cvta_generic_to_shared(up), dn_addr = (unsigned)__cvta_generic_to_shared(dn);
     const int T = Gp->T;
     const unsigned Tx = (unsigned)((nx + T - 1) >> tile_log2), Ty = (unsigned)((ny + T - 1) >> tile_log2),
                    Tz = (unsigned)((nz + T - 1) >> tile_log2);
     const unsigned T3 = Tx * Ty * Tz;
-    unsigned nv = 0, vis = 0, nr = 0, nt = 0, oob = 0;
+    unsigned nv = 0, vis = 0, nr = 0, oob = 0, nt = 0;
     while (true) {
+        __syncthreads();  // the previous item's flush has read the tile and the tables
         if (tid == 0) {
             ctl[0] = atomicAdd(counter, 1u);
-            ctl[1] = 0u;
+            ctl[1] = ctl[2] = 0u;
         }
         __syncthreads();
         const unsigned it = ctl[0];
@@ -215,24 +267,33 @@ em_tile_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, Eve
             R.PS = Gp->PS[R.a];
             R.T = T;
         }
-        if ((int)tid < R.PA) {
-            const int l0 = Gp->lo[R.a][0][tid], l1 = Gp->lo[R.a][1][tid];
-            lof[tid] = l0;
-            los[tid] = l1;
-            if ((int)tid + 1 < R.PA)
-                ainc[tid] = R.PS - ((int)Gp->lo[R.a][0][tid + 1] - l0) - R.Wf * ((int)Gp->lo[R.a][1][tid + 1] - l1);
+        for (unsigned i = tid; i < 256u; i += NT) hist[i] = 0u;
+        for (int p = (int)tid; p <= kTileMaxPlanes; p += NT) {
+            int l0 = 0, l1 = 0, u = 0, d = 0;
+            if (p < R.PA) {
+                l0 = Gp->lo[R.a][0][p];
+                l1 = Gp->lo[R.a][1][p];
+                if (p + 1 < R.PA)
+                    u = 4 * (R.PS - ((int)Gp->lo[R.a][0][p + 1] - l0) - R.Wf * ((int)Gp->lo[R.a][1][p + 1] - l1));
+                if (p > 0)
+                    d = -4 * (R.PS - (l0 - (int)Gp->lo[R.a][0][p - 1]) - R.Wf * (l1 - (int)Gp->lo[R.a][1][p - 1]));
+            }
+            lof[p] = l0;
+            los[p] = l1;
+            up[p] = u;
+            dn[p] = d;
         }
         __syncthreads();
-        for_each_tile_voxel(
+        for_each_tile_voxel<NT>(
             R, lof, los, nx, ny, nz,
-            [&](int ti, int x, int y, int z) { img[ti] = __ldg(image + ((size_t)(z * ny + y) * nx + x)); },
-            [&](int ti) { img[ti] = 0.0f; });
+            [&](int ti, int x, int y, int z) { tile[ti] = __ldg(image + ((size_t)(z * ny + y) * nx + x)); },
+            [&](int ti) { tile[ti] = 0.0f; });
         __syncthreads();
 
-        // ---- the events of the bin, 32 per warp at a time
-        const int a = R.a;
         const unsigned nchunk = (item.count + 31u) >> 5;
-        const int tile_words = R.PA * R.PS;
+        const int Wf = R.Wf;
+        const unsigned tile_bytes = (unsigned)(R.PA * R.PS) * 4u;
+        // ---- phase A: forward values from the image tile, 32 events per warp at a time
         while (true) {
             unsigned c = 0;
             if (lane == 0) c = atomicAdd(&ctl[1], 1u);
@@ -241,94 +302,148 @@ em_tile_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, Eve
             const unsigned k = c * 32u + lane;
             if (k >= item.count) continue;
             const uint64_t e = (uint64_t)item.start + k;
-            const float x1 = __ldcs(ev.x1 + e), y1 = __ldcs(ev.y1 + e), z1 = __ldcs(ev.z1 + e);
-            const float x2 = __ldcs(ev.x2 + e), y2 = __ldcs(ev.y2 + e), z2 = __ldcs(ev.z2 + e);
-            const float dt = __ldcs(ev.dt + e);
-            Ray r;
-            RayExtra X;
-            if (!ray_setup<true, true>(P, x1, y1, z1, x2, y2, z2, dt, r, &X)) continue;
-            const double ua = sel3(a, X.u[0], X.u[1], X.u[2]);
-            const double uf = a == 0 ? X.u[1] : X.u[0], us = a == 2 ? X.u[1] : X.u[2];
-            const double qa = sel3(a, X.cv[0], X.cv[1], X.cv[2]) - (double)R.ca;
-            const double qf = (a == 0 ? X.cv[1] : X.cv[0]) - (double)R.cf;
-            const double qs = (a == 2 ? X.cv[1] : X.cv[2]) - (double)R.cs;
-            const double dT = (double)T;
-            bool fit = ua != 0.0 && fabs(uf) <= fabs(ua) && fabs(us) <= fabs(ua) &&
-                       (R.sgf > 0 ? uf * ua >= 0.0 : uf * ua <= 0.0) && (R.sgs > 0 ? us * ua >= 0.0 : us * ua <= 0.0) &&
-                       qa >= 0.0 && qa <= dT && qf >= 0.0 && qf <= dT && qs >= 0.0 && qs <= dT;
-            const int ia = sel3(a, X.i[0], X.i[1], X.i[2]);
-            const int i_f = a == 0 ? X.i[1] : X.i[0], is = a == 2 ? X.i[1] : X.i[2];
-            const int p0 = ia - R.ca + R.RA;
-            int li0 = 0;
-            if (fit && (unsigned)p0 < (unsigned)R.PA) {
-                const int lf0 = (R.sgf > 0 ? i_f - R.cf : T - 1 - (i_f - R.cf)) - lof[p0];
-                const int ls0 = (R.sgs > 0 ? is - R.cs : T - 1 - (is - R.cs)) - los[p0];
-                fit = (unsigned)lf0 < (unsigned)R.Wf && (unsigned)ls0 < (unsigned)R.Ws;
-                li0 = p0 * R.PS + ls0 * R.Wf + lf0;
-            } else {
-                fit = false;
-            }
-            const float w_e = evw ? __ldg(evw + e) : 1.0f;
-            if (fit) {
-                const int dir_a = ua > 0.0 ? 1 : -1;
-                const int inc_f = (uf > 0.0 ? 1 : -1) * R.sgf;
-                const int inc_s = (us > 0.0 ? 1 : -1) * R.sgs * R.Wf;
-                const float t0a = sel3(a, r.t0x, r.t0y, r.t0z), tda = sel3(a, r.tdx, r.tdy, r.tdz);
-                const float t0f = a == 0 ? r.t0y : r.t0x, tdf = a == 0 ? r.tdy : r.tdx;
-                const float t0s = a == 2 ? r.t0y : r.t0z, tds = a == 2 ? r.tdy : r.tdz;
-                const int pq0 = p0 + (dir_a < 0 ? -1 : 0);
-                // walk 1: forward value from the image tile (software pipeline of depth 2 on the LDS, as ray_gather)
-                TileWalker wk{t0a, t0f, t0s, 0.f, 0.f, 0.f, 0.f, li0, pq0};
-                float fw = 0.0f, w0 = 0.f, v0 = 0.f, w1 = 0.f, v1 = 0.f;
-                int at, n = 0;
-                bool done = false;
-                while (!done) {
-                    fw = fmaf(w0, v0, fw);
-                    w0 = wk.step(P.gauss_a, r.t_end, r.tc, t0a, t0f, t0s, tda, tdf, tds, ainc, dir_a, inc_f, inc_s, at, done);
-                    if (CHECK && (unsigned)at >= (unsigned)tile_words) { ++oob; at = 0; w0 = 0.f; }
-                    v0 = img[at];
-                    ++n;
-                    if (!done) {
-                        fw = fmaf(w1, v1, fw);
-                        w1 = wk.step(P.gauss_a, r.t_end, r.tc, t0a, t0f, t0s, tda, tdf, tds, ainc, dir_a, inc_f, inc_s, at, done);
-                        if (CHECK && (unsigned)at >= (unsigned)tile_words) { ++oob; at = 0; w1 = 0.f; }
-                        v1 = img[at];
-                        ++n;
+            const uint4 rc = __ldg(rec.c + e);
+            float scale = 0.f;
+            if ((rc.y & (kRecValid | kRecTile)) == (kRecValid | kRecTile)) {  // the others (stragglers): direct pass
+                const float4 ra = __ldg(rec.a + e), rb = __ldg(rec.b + e);
+                const float te = ra.y, da = rb.y, df = rb.z, ds = rb.w;
+                const bool down = rc.y & kRecNeg0;
+                const int dpq = down ? -4 : 4;
+                const int inc_f = (rc.y & kRecNeg1) ? -4 : 4, inc_s = (rc.y & kRecNeg2) ? -4 * Wf : 4 * Wf;
+                vis += rc.z;
+                float t = ra.x, ta = ra.z, tf = ra.w, ts = rb.x;
+                unsigned li = tile_addr + (rc.y >> kRecLiShift) * 4u;
+                unsigned pq = (down ? dn_addr : up_addr) + ((rc.y >> kRecPlaneShift) & 127u) * 4u;
+                int na = (int)__float_as_int(lds_f32(pq));
+                // the value loaded in one step is consumed in the next
+                float accv = 0.f, wp = 0.f, vp = 0.f;
+                while (true) {
+                    float t2;
+                    {
+                        const float tn = min3f(ta, tf, ts);
+                        if (!(tn < te)) break;
+                        const float w = chord_weight(t, tn);
+                        accv = fmaf(wp, vp, accv);
+                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                        vp = lds_f32(li);
+                        wp = w;
+                        advance_plane(ta, li, na, pq, tn, da, dpq);
+                        advance_addr(tf, li, tn, df, inc_f);
+                        advance_addr(ts, li, tn, ds, inc_s);
+                        t2 = tn;
+                    }
+                    t = t2;
+                    {
+                        const float tn = min3f(ta, tf, ts);
+                        if (!(tn < te)) break;
+                        const float w = chord_weight(t, tn);
+                        accv = fmaf(wp, vp, accv);
+                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                        vp = lds_f32(li);
+                        wp = w;
+                        advance_plane(ta, li, na, pq, tn, da, dpq);
+                        advance_addr(tf, li, tn, df, inc_f);
+                        advance_addr(ts, li, tn, ds, inc_s);
+                        t = tn;
                     }
                 }
-                fw = fmaf(w0, v0, fw);
-                fw = fmaf(w1, v1, fw);
-                vis += n;
+                const float w = chord_weight(t, te);
+                accv = fmaf(wp, vp, accv);
+                if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                const float fw = fmaf(w, lds_f32(li), accv);
                 if (fw > 0.0f) {  // R9
                     ++nv;
-                    ++nt;
-                    const float scale = w_e / fw;
-                    TileWalker wb{t0a, t0f, t0s, 0.f, 0.f, 0.f, 0.f, li0, pq0};
-                    do {
-                        const float w = wb.step(P.gauss_a, r.t_end, r.tc, t0a, t0f, t0s, tda, tdf, tds, ainc, dir_a, inc_f, inc_s, at, done);
-                        if (CHECK && (unsigned)at >= (unsigned)tile_words) { ++oob; continue; }
-                        atomicAdd(acc + at, w * scale);
-                    } while (!done);
+                    scale = (evw ? __ldg(evw + e) : 1.0f) / fw;
+                    atomicAdd(&hist[__float_as_uint(scale) >> 23], 1u);
                 }
-            } else {  // the direct walk of projector.cu for the few events of the bin whose window may leave the tile
-                int n;
-                const float fw = ray_gather<true>(P, r, image, n);
-                vis += n;
-                if (fw > 0.0f) {
-                    ++nv;
-                    nr += ray_scatter<true, true, BRICK>(P, r, corr, w_e / fw);
+            }
+            ev_scale[e] = scale;
+        }
+        __syncthreads();
+        // ---- the item's scale: bin B = the lowest exponent with at most half of the events above it (the median's bin);
+        // S = 2^(qexp - kMedianBits - (B + 1 - 127)).  Every warp computes it.
+        float S;
+        {
+            unsigned cnt[8], mine = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                cnt[j] = hist[lane * 8u + j];
+                mine += cnt[j];
+            }
+            unsigned incl = mine;  // suffix sum over lanes (this lane and the higher ones)
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned o = __shfl_down_sync(0xffffffffu, incl, d);
+                if (lane + d < 32u) incl += o;
+            }
+            const unsigned total = __shfl_sync(0xffffffffu, incl, 0);
+            const unsigned limit = total >> 1;
+            int B = 0;
+            unsigned run = incl - mine;  // events strictly above the bin looked at
+#pragma unroll
+            for (int j = 7; j >= 0; --j) {
+                if (run > limit && B == 0) B = (int)(lane * 8u) + j + 1;
+                run += cnt[j];
+            }
+            B = __reduce_max_sync(0xffffffffu, B);
+            if (B > 255) B = 255;
+            int field = fx.qexp - kMedianBits - B + 253;  // exponent field of S
+            field = field < 1 ? 1 : (field > 254 ? 254 : field);
+            S = __uint_as_float((unsigned)field << 23);
+        }
+        for (int i = tid; i < words; i += NT) tile[i] = 0.0f;  // all-zero bits: the integer zero
+        __syncthreads();
+        // ---- phase B: the same chords again, w_e / fwd_e * chord weight accumulated on the tile in integer quanta
+        while (true) {
+            unsigned c = 0;
+            if (lane == 0) c = atomicAdd(&ctl[2], 1u);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c >= nchunk) break;
+            const unsigned k = c * 32u + lane;
+            if (k >= item.count) continue;
+            const uint64_t e = (uint64_t)item.start + k;
+            const float scale = ev_scale[e];
+            if (!(scale > 0.0f)) continue;
+            const uint4 rc = __ldg(rec.c + e);
+            const float4 ra = __ldg(rec.a + e), rb = __ldg(rec.b + e);
+            const float scaleS = scale * S;
+            const float top = scaleS * fx.lmax;  // quanta of the longest possible chord of this event
+            if (top < fx.qmax && top >= fx.qmin) {
+                ++nt;
+                const float te = ra.y, da = rb.y, df = rb.z, ds = rb.w;
+                const bool down = rc.y & kRecNeg0;
+                const int dpq = down ? -4 : 4;
+                const int inc_f = (rc.y & kRecNeg1) ? -4 : 4, inc_s = (rc.y & kRecNeg2) ? -4 * Wf : 4 * Wf;
+                float t = ra.x, ta = ra.z, tf = ra.w, ts = rb.x;
+                unsigned li = tile_addr + (rc.y >> kRecLiShift) * 4u;
+                unsigned pq = (down ? dn_addr : up_addr) + ((rc.y >> kRecPlaneShift) & 127u) * 4u;
+                int na = (int)__float_as_int(lds_f32(pq));
+                while (true) {
+                    const float tn = min3f(ta, tf, ts);
+                    if (!(tn < te)) break;
+                    if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                    red_shared_u32(li, __float_as_uint(fmaf(chord_weight(t, tn), scaleS, 8388608.0f)) - 0x4B000000u);
+                    advance_plane(ta, li, na, pq, tn, da, dpq);
+                    advance_addr(tf, li, tn, df, inc_f);
+                    advance_addr(ts, li, tn, ds, inc_s);
+                    t = tn;
                 }
+                if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                red_shared_u32(li, __float_as_uint(fmaf(chord_weight(t, te), scaleS, 8388608.0f)) - 0x4B000000u);
+            } else {
+                nr += rc.z;
+                scatter_global<BRICK>(ra, rb, rc, nx, ny, corr, scale);
             }
         }
         __syncthreads();
-        // ---- add the tile to the correction image and clear it
-        for_each_tile_voxel(
+        // ---- add the tile to the correction image
+        const float inv_S = 1.0f / S;
+        for_each_tile_voxel<NT>(
             R, lof, los, nx, ny, nz,
             [&](int ti, int x, int y, int z) {
-                const float v = acc[ti];
-                if (v != 0.0f) {
-                    acc[ti] = 0.0f;
-                    atomicAdd(corr + corr_index<BRICK>(x, y, z, nx, ny), v);
+                const unsigned q = __float_as_uint(tile[ti]);
+                if (q != 0u) {
+                    atomicAdd(corr + corr_index<BRICK>(x, y, z, nx, ny), (float)q * inv_S);
                     ++nr;
                 }
             },
@@ -337,40 +452,81 @@ em_tile_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, Eve
     nv = __reduce_add_sync(0xffffffffu, nv);
     vis = __reduce_add_sync(0xffffffffu, vis);
     nr = __reduce_add_sync(0xffffffffu, nr);
-    nt = __reduce_add_sync(0xffffffffu, nt);
     oob = __reduce_add_sync(0xffffffffu, oob);
+    nt = __reduce_add_sync(0xffffffffu, nt);
     if (lane == 0 && stats) {
+        if (oob) atomicAdd(&stats->tile_oob, (unsigned long long)oob);
         if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
+        if (nt) atomicAdd(&stats->tile_events, (unsigned long long)nt);
         if (vis) atomicAdd(&stats->visits, (unsigned long long)vis);
         if (nr) atomicAdd(&stats->reds, (unsigned long long)nr);
-        if (nt) atomicAdd(&stats->tile_events, (unsigned long long)nt);
-        if (oob) atomicAdd(&stats->tile_oob, (unsigned long long)oob);
     }
 }
 
-template <bool BRICK, bool CHECK>
-static void launch_tile(const ProjParams &p, const TileGeom *d_geom, size_t smem, int tile_log2, const EventPtrs &ev,
-                        const float *evw, const float *image, float *corr, DeviceStats *stats, const TileItem *items,
-                        uint32_t n_items, unsigned *counter, int n_sm, cudaStream_t s) {
-    cudaFuncSetAttribute(em_tile_kernel<BRICK, CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    em_tile_kernel<BRICK, CHECK><<<n_sm, kTileThreads, smem, s>>>(p, d_geom, tile_log2, ev, evw, image, corr, stats,
-                                                                 items, n_items, counter);
+struct TileLaunch {
+    const ProjParams &p;
+    const TileGeom *d_geom;
+    size_t smem;
+    int tile_log2;
+    const RecPtrs &rec;
+    const float *evw, *image;
+    float *corr;
+    DeviceStats *stats;
+    const TileItem *items;
+    uint32_t n_items;
+    unsigned *counter;
+    int n_sm;
+    FixedPoint fx;
+    float *ev_scale;
+    cudaStream_t s;
+};
+
+template <int NT, int NCTA, bool BRICK, bool CHECK>
+static void launch_tile(const TileLaunch &L) {
+    auto k = em_tile_kernel<NT, NCTA, BRICK, CHECK>;
+    cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
+    cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    const uint32_t cap = (uint32_t)L.n_sm * NCTA;
+    k<<<L.n_items < cap ? L.n_items : cap, NT, L.smem, L.s>>>(L.p.n[0], L.p.n[1], L.p.n[2], L.d_geom, L.tile_log2, L.rec,
+                                                              L.evw, L.image, L.corr, L.stats, L.items, L.n_items,
+                                                              L.counter, L.fx, L.ev_scale);
 }
 
-void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const EventPtrs &ev,
+template <int NT, int NCTA>
+static void launch_tile_cfg(const TileLaunch &L, bool check) {
+    if (L.p.brick) {
+        if (check) launch_tile<NT, NCTA, true, true>(L); else launch_tile<NT, NCTA, true, false>(L);
+    } else {
+        if (check) launch_tile<NT, NCTA, false, true>(L); else launch_tile<NT, NCTA, false, false>(L);
+    }
+}
+
+void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const RecPtrs &rec,
                     const float *evw, const float *image, float *corr, DeviceStats *stats, const TileItem *items,
-                    uint32_t n_items, unsigned *counter, int n_sm, bool check, cudaStream_t s) {
+                    uint32_t n_items, unsigned *counter, int n_sm, size_t smem_per_sm, bool check, double sigma,
+                    uint32_t max_item_events, float *ev_scale, cudaStream_t s) {
     if (n_items == 0) return;
     cudaMemsetAsync(counter, 0, sizeof(unsigned), s);
-    const size_t smem = tile_smem_bytes(g);
-    const unsigned grid = (unsigned)(n_items < (uint32_t)n_sm ? n_items : (uint32_t)n_sm);
-    if (p.brick) {
-        if (check) launch_tile<true, true>(p, d_geom, smem, tile_log2, ev, evw, image, corr, stats, items, n_items, counter, (int)grid, s);
-        else launch_tile<true, false>(p, d_geom, smem, tile_log2, ev, evw, image, corr, stats, items, n_items, counter, (int)grid, s);
-    } else {
-        if (check) launch_tile<false, true>(p, d_geom, smem, tile_log2, ev, evw, image, corr, stats, items, n_items, counter, (int)grid, s);
-        else launch_tile<false, false>(p, d_geom, smem, tile_log2, ev, evw, image, corr, stats, items, n_items, counter, (int)grid, s);
+    FixedPoint fx;
+    {
+        const double kappa = sqrt(1.4426950408889634 / 2.0) / sigma;
+        fx.lmax = (float)(kappa * sqrt(p.v[0] * p.v[0] + p.v[1] * p.v[1] + p.v[2] * p.v[2]) * 1.0001);
+        double qmax = 2147483648.0 / (double)(max_item_events < 1 ? 1 : max_item_events);
+        if (qmax > 4194304.0) qmax = 4194304.0;  // the float -> integer conversion holds 23 bits
+        fx.qmax = (float)qmax;
+        fx.qmin = 1024.0f;
+        fx.qexp = (int)floor(log2(qmax / (double)fx.lmax));
     }
+    const size_t smem = tile_smem_bytes(g);
+    const TileLaunch L{p, d_geom, smem, tile_log2, rec, evw, image, corr, stats, items, n_items, counter, n_sm, fx,
+                       ev_scale, s};
+    // CTAs per SM by shared memory (1 KB per CTA is reserved by the system); threads so that 56 registers fit
+    const size_t per_sm = smem_per_sm ? smem_per_sm : 233472;
+    const int ncta = (int)(per_sm / (smem + 1024));
+    if (ncta >= 4) launch_tile_cfg<256, 4>(L, check);
+    else if (ncta == 3) launch_tile_cfg<384, 3>(L, check);
+    else if (ncta == 2) launch_tile_cfg<512, 2>(L, check);
+    else launch_tile_cfg<1024, 1>(L, check);
 }
 
 }  // namespace tofmlem

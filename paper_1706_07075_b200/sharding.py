@@ -48,3 +48,12 @@ def max_over_ranks_ms(ms: float, device: Optional[torch.device] = None, group: O
     t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
     dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+def sum_over_ranks(count: int, device: Optional[torch.device] = None, group: Optional[dist.ProcessGroup] = None) -> int:
+    """An integer count (e.g. the valid events of a pass) summed over ranks; the value itself for a single process."""
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
+        return int(count)
+    t = torch.tensor([count], dtype=torch.int64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return int(t.item())

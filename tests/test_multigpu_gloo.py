@@ -64,9 +64,8 @@ def _rank_main(rank: int, world: int, port: int, out_dir: str):
             x = oracle.update(x, t.numpy(), sens, mask)
             n_valid = nv
         ms = sharding.max_over_ranks_ms(10.0 + rank)
-        nv_t = torch.tensor([n_valid], dtype=torch.int64)
-        dist.all_reduce(nv_t)
-        np.savez(os.path.join(out_dir, f"rank{rank}.npz"), x=x, ms=ms, n_valid=int(nv_t.item()))
+        nv_all = sharding.sum_over_ranks(n_valid)  # what bench.py compares sum(image * sens) with (P7)
+        np.savez(os.path.join(out_dir, f"rank{rank}.npz"), x=x, ms=ms, n_valid=nv_all)
     finally:
         dist.destroy_process_group()
 
