@@ -431,7 +431,9 @@ def main():
     ap.add_argument("--subbins", type=int, default=0, help="TOFMLEM_OPT_SUBBINS override (0 = library default)")
     ap.add_argument("--em-variant", type=int, default=-1, help="TOFMLEM_OPT_EM_VARIANT override (-1 = library default)")
     ap.add_argument("--cache-share", type=int, default=-1, help="TOFMLEM_OPT_CACHE_SHARE override")
-    ap.add_argument("--tile", type=int, default=0, help="1: tofmlem_plan_events on the binned list (tile-mode fused pass)")
+    ap.add_argument("--tile", type=int, default=1,
+                    help="1 (default): tofmlem_plan_events on the binned list (ray records + shared-memory tiles); 0: the "
+                         "unplanned fused pass of round 1")
     ap.add_argument("--tile-min", type=int, default=0, help="TOFMLEM_OPT_TILE_MIN_EVENTS override")
     ap.add_argument("--tile-max", type=int, default=0, help="TOFMLEM_OPT_TILE_MAX_EVENTS override")
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next", "pipeline"],
@@ -505,13 +507,14 @@ def main():
         del key, perm, ev
         ev = sev
     torch.cuda.empty_cache()
-    plan = None
+    plan, plan_ms = None, 0.0
     if args.tile and not args.no_bin:
         if args.tile_min:
             ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, args.tile_min)
         if args.tile_max:
             ctx.set_option(pkg.OPT_TILE_MAX_EVENTS, args.tile_max)
-        plan = ctx.plan_events(ev, n)
+        plan_ms = timed(lambda: ctx.plan_events(ev, n))
+        plan = ctx.plan_info()
 
     image = torch.ones(nvox, dtype=torch.float32, device=dev)
     corr = torch.zeros(nvox, dtype=torch.float32, device=dev)
@@ -557,49 +560,79 @@ def main():
     p7 = float((image.double() * sens.double()).sum().item())
     n_valid_all = sharding.sum_over_ranks(int(st.n_valid), dev)  # the image was updated with the all-reduced correction
 
-    # ---- roofline of the dominant kernel (em_correction): see DESIGN.md "Measurement"
+    # ---- roofline of the dominant kernel: see DESIGN.md "Measurement"
     hbm_peak, peak_src = load_peaks()
     visits = int(st.visits)
+    tile_visits = int(st.tile_visits)
+    t_tile_ms, t_direct_ms, t_strag_ms = ctx.pass_timing()  # CUDA events around the kernels of the last planned pass
     probe_buf = torch.zeros(nvox, dtype=torch.float32, device=dev)
     n_ops = 1 << 30
     red_rand = n_ops / (ctx.probe(0, probe_buf, n_ops) * 1e-3)
     red_row = n_ops / (ctx.probe(1, probe_buf, n_ops) * 1e-3)
     ld_rand = n_ops / (ctx.probe(2, probe_buf, n_ops) * 1e-3)
     ld_row = n_ops / (ctx.probe(3, probe_buf, n_ops) * 1e-3)
-    red_rand_v4 = n_ops / (ctx.probe(5, probe_buf, n_ops) * 1e-3)  # the kernel's own instruction: 16-byte reductions
+    red_rand_v4 = n_ops / (ctx.probe(5, probe_buf, n_ops) * 1e-3)  # the direct kernel's own instruction
+    smem_add = n_ops / (ctx.probe(6, probe_buf, n_ops) * 1e-3)     # ATOMS.ADD on a 72 KB tile, 3 CTAs per SM
+    smem_ld = n_ops / (ctx.probe(7, probe_buf, n_ops) * 1e-3)      # LDS, same pattern
     red_peak = max(red_rand, red_rand_v4)  # the roofline uses the HIGHER of the two request rates
     del probe_buf
-    hbm_bytes = 28.0 * n  # algorithmic HBM bytes per launch: 7 float32 per event
-    reds = int(st.reductions)  # reduction instructions of one launch (each is one request to an L2 atomic unit)
+    planned = plan is not None and bool(plan.active)
+    rec_bytes = 48.0 if planned else 28.0
+    hbm_bytes = rec_bytes * n  # algorithmic HBM bytes per pass: one ray record (or 7 float32) per event
+    reds = int(st.reductions)  # reduction requests to the L2 atomic units (direct pass + tile flushes)
     t_hbm = hbm_bytes / (hbm_peak * 1e9)
-    t_red = reds / red_peak
-    t_ld = visits / ld_rand
-    achieved = reds / (kern_ms * 1e-3)
-    # the same launch against SURVEY.md 8(d)'s visit-based formula, T_roof = max(HBM, visits / R_gather, visits / R_red)
-    # with the conflict-free RANDOM rates (may exceed 1: 16-byte reductions carry 1.5 visits each and most gathers hit
-    # L1), and against the COALESCED L2 rates of the same probes (what the method would need with full sectors)
+    # the same pass against SURVEY.md 8(d)'s visit-based formula, T_roof = max(HBM, visits / R_gather, visits / R_red)
+    # with the conflict-free RANDOM L2 rates, and against the COALESCED L2 rates of the same probes (what the method
+    # would need with full sectors)
     t_roof_visits = max(t_hbm, visits / ld_rand, visits / red_rand)
     t_roof_row = max(t_hbm, visits / ld_row, visits / red_row)
     full_default = args.workload == "full" and not args.events and not args.no_bin
-    roofline = {
-        "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_peak / 1e9, "unit": "G reductions/s",
-        "frac": achieved / red_peak,
+    probes = {"red_random": red_rand / 1e9, "red_random_v4": red_rand_v4 / 1e9, "red_row": red_row / 1e9,
+              "gather_random": ld_rand / 1e9, "gather_row": ld_row / 1e9, "smem_add_random": smem_add / 1e9,
+              "smem_load_random": smem_ld / 1e9}
+    common = {
         "frac_visits": t_roof_visits / (kern_ms * 1e-3), "frac_l2_coalesced": t_roof_row / (kern_ms * 1e-3),
-        # dram__bytes_read.sum + dram__bytes_write.sum of one launch at cfg-3: a CONSTANT copied from the committed
-        # ncu --set full capture named in traffic_source (not measured in this run); default full workload only
-        "traffic": TRAFFIC_BYTES if full_default else None,
-        "traffic_source": TRAFFIC_SOURCE if full_default else None,
-        "kernel": "em_persistent_kernel<TOF, v4, BRICK>", "kernel_ms": kern_ms, "visits_per_launch": visits,
-        "reductions_per_launch": reds, "visits_per_reduction": visits / max(1, reds),
-        "visits_Gps": visits / (kern_ms * 1e-3) / 1e9,
-        "peak_source": "tofmlem_probe: random-address reductions into an L2-resident array of nvox floats, the higher of "
-                       "the 4-byte (kind 0) and the 16-byte (kind 5) request rates, measured in this run",
-        "probes_Gops": {"red_random": red_rand / 1e9, "red_random_v4": red_rand_v4 / 1e9, "red_row": red_row / 1e9, "gather_random": ld_rand / 1e9,
-                        "gather_row": ld_row / 1e9},
-        "t_roof_ms": {"hbm": t_hbm * 1e3, "red": t_red * 1e3, "gather": t_ld * 1e3},
+        "kernel_ms": kern_ms, "visits_per_launch": visits, "reductions_per_launch": reds,
+        "visits_Gps": visits / (kern_ms * 1e-3) / 1e9, "probes_Gops": probes,
         "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_GBs": hbm_bytes / (kern_ms * 1e-3) / 1e9, "peak_GBs": hbm_peak,
                 "frac": hbm_bytes / (kern_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src},
     }
+    if planned and t_tile_ms > 0.0 and t_tile_ms >= t_direct_ms:
+        # Dominant kernel: em_tile_kernel.  Every tile visit is one shared-memory load (forward walk) and one
+        # shared-memory integer add (scatter walk) through the SM's shared-memory pipe: algorithmic time = visits x
+        # (1 / R_load + 1 / R_add) with both rates measured on the tile pass's own footprint (probe kinds 6, 7).
+        peak_vis = 1.0 / (1.0 / smem_ld + 1.0 / smem_add)
+        ach = tile_visits / (t_tile_ms * 1e-3)
+        roofline = {
+            "bound": "smem_atomic", "achieved": ach / 1e9, "peak": peak_vis / 1e9, "unit": "G tile visits/s",
+            "frac": ach / peak_vis,
+            "kernel": "em_tile_kernel<384, 3, BRICK>", "dominant_kernel_ms": t_tile_ms,
+            "tile_visits_per_launch": tile_visits,
+            "traffic": TRAFFIC_BYTES if full_default else None,
+            "traffic_source": TRAFFIC_SOURCE if full_default else None,
+            "peak_source": "tofmlem_probe kinds 6 / 7: random ATOMS.ADD.U32 and LDS on a 72 KB shared-memory tile, 3 CTAs "
+                           "of 384 threads per SM, measured in this run; one tile visit = one load + one add",
+            # the second kernel of the step: the direct pass on records, bound by L2 reduction requests as in round 1
+            "direct": {"kernel": "em_planned_kernel<v4, BRICK>", "kernel_ms": t_direct_ms + t_strag_ms,
+                       "bound": "l2_atomic", "peak": red_peak / 1e9, "unit": "G reductions/s",
+                       "note": "reductions_per_launch counts the direct pass's 16-byte reductions and the tiles' flushes"},
+            # both kernels together: algorithmic time of the step over its measured time
+            "frac_step": (tile_visits / peak_vis + (visits - tile_visits) / 1.5 / red_peak) / (kern_ms * 1e-3),
+            **common,
+        }
+    else:
+        achieved = reds / (kern_ms * 1e-3)
+        roofline = {
+            "bound": "l2_atomic", "achieved": achieved / 1e9, "peak": red_peak / 1e9, "unit": "G reductions/s",
+            "frac": achieved / red_peak,
+            "traffic": None, "traffic_source": None,
+            "kernel": "em_planned_kernel<v4, BRICK>" if planned else "em_persistent_kernel<TOF, v4, BRICK>",
+            "visits_per_reduction": visits / max(1, reds),
+            "peak_source": "tofmlem_probe: random-address reductions into an L2-resident array of nvox floats, the higher of "
+                           "the 4-byte (kind 0) and the 16-byte (kind 5) request rates, measured in this run",
+            "t_roof_ms": {"hbm": t_hbm * 1e3, "red": reds / red_peak * 1e3, "gather": visits / ld_rand * 1e3},
+            **common,
+        }
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -634,9 +667,9 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": make_config(cfg, n, m, world, binned=not args.no_bin),
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "setup": {"sensitivity_ms": sens_ms, "bin_sort_gather_ms": bin_ms,
-                      "recon_wall_s": (bin_ms + cfg.iters * ms_per_step) * 1e-3,
-                      "recon_wall_note": f"binning + {cfg.iters} iterations, events resident in HBM"},
+            "setup": {"sensitivity_ms": sens_ms, "bin_sort_gather_ms": bin_ms, "plan_ms": plan_ms,
+                      "recon_wall_s": (bin_ms + plan_ms + cfg.iters * ms_per_step) * 1e-3,
+                      "recon_wall_note": f"binning + plan (ray records) + {cfg.iters} iterations, events resident in HBM"},
             "stats": {"n_valid": int(st.n_valid), "visits": visits, "visits_per_valid_event": visits / max(1, int(st.n_valid)),
                       "sum_image_sens": p7, "p7_rel_err": abs(p7 - n_valid_all) / max(1, n_valid_all),
                       "tile_events": int(st.tile_events),

@@ -69,6 +69,7 @@ typedef struct {
                               atomic units: the unit of the l2_atomic roofline */
     uint64_t tile_events;  /* of n_valid: events accumulated through a shared-memory tile (tofmlem_plan_events) */
     uint64_t tile_oob;     /* TOFMLEM_OPT_TILE_CHECK: tile accesses found out of range; must be 0 */
+    uint64_t tile_visits;  /* of visits: voxel visits of the forward walk on shared-memory tiles */
 } tofmlem_stats;
 
 /* What tofmlem_plan_events decided (tofmlem_plan_info). */
@@ -284,12 +285,17 @@ int tofmlem_scatter_reject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t 
  * operations against d_buf[0..n_elems) and returns the elapsed milliseconds in *h_ms (second of two passes, so
  * the array is L2-resident when it fits).  kind 0: RED.ADD.F32 to unrelated random elements per lane; 1: RED to
  * 32 consecutive elements of a random row per warp; 2 / 3: the same two patterns with 4-byte loads; 4 / 5: random
- * 8-byte / 16-byte vector reductions (one n_ops unit = one instruction per lane).
+ * 8-byte / 16-byte vector reductions (one n_ops unit = one instruction per lane); 6 / 7: random 32-bit integer adds /
+ * 4-byte loads on a 72 KB SHARED-MEMORY tile, three CTAs per SM (the tile pass's own access pattern; d_buf untouched).
  * d_buf is modified by kinds 0, 1, 4, 5.  SYNCHRONISES. */
 int tofmlem_probe(tofmlem_ctx *ctx, int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *h_ms);
 
 /* Copies the counters of the last pass to *h_out.  SYNCHRONISES the context's stream. */
 int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out);
+/* Device time of the kernels of the LAST planned fused pass (tofmlem_plan_events), in milliseconds, measured with CUDA
+ * events on the context's stream: h_ms[0] = tile pass (tile.cu), h_ms[1] = direct pass on records, h_ms[2] = the tile
+ * items' stragglers; 0 for a part that did not run (all 0 after an unplanned pass).  SYNCHRONISES. */
+int tofmlem_pass_timing(tofmlem_ctx *ctx, float h_ms[3]);
 /* Text of the last error of this context ("" if none).  Valid until the next call on the context. */
 const char *tofmlem_last_error(const tofmlem_ctx *ctx);
 /* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches). */

@@ -76,6 +76,8 @@ struct tofmlem_ctx {
     float *d_ev_scale = nullptr;       // w_e / fwd_e of the tile events between the two phases of tile.cu (rec_cap floats)
     size_t smem_per_sm = 0;
     void *d_plan_counters = nullptr;
+    cudaEvent_t t_ev[4] = {nullptr, nullptr, nullptr, nullptr};  // tofmlem_pass_timing: around the planned kernels
+    int t_have = 0;                                              // bit k: part k of the last planned pass ran
     struct {
         bool valid = false;
         const float *x1 = nullptr;  // the plan describes THIS event list (first member array) ...
@@ -321,6 +323,10 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         // Planned list (tofmlem_plan_events): the pass runs on the ray records -- the items on shared-memory tiles
         // (tile.cu), the other events and the stragglers of the items through the direct pass on records (prepared.cu).
         const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 1;
+        if (!ctx->t_ev[0])
+            for (auto &te : ctx->t_ev) CU(cudaEventCreate(&te));
+        ctx->t_have = (ctx->plan.n_items ? 1 : 0) | (ctx->plan.n_chunks ? 2 : 0) | (ctx->plan.n_strag ? 4 : 0);
+        CU(cudaEventRecord(ctx->t_ev[0], s));
         if (ctx->plan.n_items) {
             TileGeom g;
             build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);  // the same as at plan time (sigma, trunc match)
@@ -329,20 +335,24 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
                            ctx->tile_check != 0, ctx->sigma, ctx->plan.max_item_events, ctx->d_ev_scale, s);
             CHECK_LAUNCH(1);
         }
+        CU(cudaEventRecord(ctx->t_ev[1], s));
         if (ctx->plan.n_chunks) {
             launch_em_planned(p, ev, ctx->d_rec, ctx->d_chunks, nullptr, ctx->plan.n_chunks, 0, evw, d_image, d_corr, vec,
                               ctx->d_stats, ctx->d_queues, n_sm, s);
             CHECK_LAUNCH(1);
         }
+        CU(cudaEventRecord(ctx->t_ev[2], s));
         if (ctx->plan.n_strag) {
             launch_em_planned(p, ev, ctx->d_rec, nullptr, ctx->d_strag, (ctx->plan.n_strag + 31u) / 32u, ctx->plan.n_strag,
                               evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, n_sm, s);
             CHECK_LAUNCH(1);
         }
+        CU(cudaEventRecord(ctx->t_ev[3], s));
         return TOFMLEM_OK;
     } else {
         launch_em_correction(p, ctx->tof, ev, n, evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, s);
     }
+    ctx->t_have = 0;
     CHECK_LAUNCH(1);
     return TOFMLEM_OK;
 }
@@ -472,6 +482,8 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_items);
     cudaFree(ctx->d_chunks);
     cudaFree(ctx->d_plan_counters);
+    for (auto &te : ctx->t_ev)
+        if (te) cudaEventDestroy(te);
     free_records(ctx);
     delete ctx;
     return TOFMLEM_OK;
@@ -1297,6 +1309,7 @@ int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out) {
     h_out->reductions = h.reds;
     h_out->tile_events = h.tile_events;
     h_out->tile_oob = h.tile_oob;
+    h_out->tile_visits = h.tile_visits;
     h_out->sum_image_sens = h.sum_image_sens;
     return TOFMLEM_OK;
 }
@@ -1307,6 +1320,16 @@ int tofmlem_probe(tofmlem_ctx *ctx, int kind, float *d_buf, uint64_t n_elems, ui
     if (rc == -1) return fail(ctx, TOFMLEM_EINVAL, "probe: bad kind or size");
     if (rc != 0) return cuda_fail(ctx, cudaGetLastError(), "probe");
     ctx->launches += 2;
+    return TOFMLEM_OK;
+}
+
+int tofmlem_pass_timing(tofmlem_ctx *ctx, float h_ms[3]) {
+    if (!ctx || !h_ms) return TOFMLEM_EINVAL;
+    h_ms[0] = h_ms[1] = h_ms[2] = 0.0f;
+    if (!ctx->t_have || !ctx->t_ev[0]) return TOFMLEM_OK;
+    CU(cudaEventSynchronize(ctx->t_ev[3]));
+    for (int k = 0; k < 3; ++k)
+        if (ctx->t_have & (1 << k)) CU(cudaEventElapsedTime(&h_ms[k], ctx->t_ev[k], ctx->t_ev[k + 1]));
     return TOFMLEM_OK;
 }
 

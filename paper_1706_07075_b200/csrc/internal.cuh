@@ -37,9 +37,10 @@ struct DeviceStats {
     unsigned long long reds;  // reduction instructions (requests to the L2 atomic units) of the scatter walk
     unsigned long long tile_events;  // valid events whose window was accumulated in a shared-memory tile (tile.cu)
     unsigned long long tile_oob;     // TOFMLEM_OPT_TILE_CHECK: tile accesses found out of range (must stay 0)
+    unsigned long long tile_visits;  // voxel visits of the forward walk on tiles
     double sum_image_sens;
 };
-constexpr int kStatsCounters = 5;  // leading unsigned long long members, reset before every pass
+constexpr int kStatsCounters = 6;  // leading unsigned long long members, reset before every pass
 
 // float32 grid for the bit-exact key / region arithmetic (specification F1)
 struct GridF32 {

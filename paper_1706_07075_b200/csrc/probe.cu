@@ -41,10 +41,41 @@ __global__ void __launch_bounds__(256) probe_kernel(float *buf, uint32_t n, int 
     if ((KIND == 2 || KIND == 3) && acc == 123.456f) *sink = acc;
 }
 
+// kind 6 / 7: random 32-bit integer adds (ATOMS.ADD, what tile.cu accumulates with) / random 4-byte loads (LDS) on a
+// 72 KB shared-memory tile, three CTAs of 384 threads per SM as the tile pass runs: the denominators of its roofline.
+template <int KIND>
+__global__ void __launch_bounds__(384, 3) smem_probe_kernel(int ops, float *sink) {
+    extern __shared__ unsigned tile[];
+    constexpr unsigned kWords = 18432;
+    for (unsigned i = threadIdx.x; i < kWords; i += 384) tile[i] = i;
+    __syncthreads();
+    uint32_t h = mix32((blockIdx.x * 384u + threadIdx.x) * 2654435761u + 777u);
+    unsigned acc = 0;
+#pragma unroll 4
+    for (int i = 0; i < ops; ++i) {
+        h = mix32(h + 0x9e3779b9u);
+        const unsigned a = h % kWords;
+        if (KIND == 6) atomicAdd(&tile[a], 1u);
+        else acc += tile[a];
+    }
+    if (KIND == 7 && acc == 0x12345678u) *sink = 1.0f;
+}
+
 int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *ms, cudaStream_t s) {
     if (n_elems < 64 || n_elems > 0xFFFFFFFFull) return -1;
-    const int blocks = 148 * 16;
-    const uint64_t threads = (uint64_t)blocks * 256;
+    const bool smem = kind == 6 || kind == 7;
+    int n_sm = 148;
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    const int blocks = smem ? n_sm * 3 : n_sm * 16;
+    const uint64_t threads = (uint64_t)blocks * (smem ? 384 : 256);
+    if (smem) {
+        cudaFuncSetAttribute(smem_probe_kernel<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, 18432 * 4);
+        cudaFuncSetAttribute(smem_probe_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, 18432 * 4);
+    }
     const int ops = (int)((n_ops + threads - 1) / threads);
     float *sink = d_buf;  // never written in practice
     cudaEvent_t a, b;
@@ -59,6 +90,8 @@ int run_probe(int kind, float *d_buf, uint64_t n_elems, uint64_t n_ops, float *m
             case 3: probe_kernel<3><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
             case 4: probe_kernel<4><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
             case 5: probe_kernel<5><<<blocks, 256, 0, s>>>(d_buf, (uint32_t)n_elems, ops, sink); break;
+            case 6: smem_probe_kernel<6><<<blocks, 384, 18432 * 4, s>>>(ops, sink); break;
+            case 7: smem_probe_kernel<7><<<blocks, 384, 18432 * 4, s>>>(ops, sink); break;
             default: cudaEventDestroy(a); cudaEventDestroy(b); return -1;
         }
         cudaEventRecord(b, s);

@@ -458,7 +458,10 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
         if (oob) atomicAdd(&stats->tile_oob, (unsigned long long)oob);
         if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
         if (nt) atomicAdd(&stats->tile_events, (unsigned long long)nt);
-        if (vis) atomicAdd(&stats->visits, (unsigned long long)vis);
+        if (vis) {
+            atomicAdd(&stats->visits, (unsigned long long)vis);
+            atomicAdd(&stats->tile_visits, (unsigned long long)vis);
+        }
         if (nr) atomicAdd(&stats->reds, (unsigned long long)nr);
     }
 }

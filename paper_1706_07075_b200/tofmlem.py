@@ -39,7 +39,7 @@ SYMBOLS = (
     "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
     "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
     "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events", "tofmlem_reserve", "tofmlem_trim",
-    "tofmlem_plan_events", "tofmlem_plan_info",
+    "tofmlem_plan_events", "tofmlem_plan_info", "tofmlem_pass_timing",
 )
 
 
@@ -64,7 +64,7 @@ class Events(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_valid", C.c_uint64), ("n_skipped", C.c_uint64), ("visits", C.c_uint64),
                 ("sum_image_sens", C.c_double), ("reductions", C.c_uint64), ("tile_events", C.c_uint64),
-                ("tile_oob", C.c_uint64)]
+                ("tile_oob", C.c_uint64), ("tile_visits", C.c_uint64)]
 
 
 class Plan(C.Structure):
@@ -191,6 +191,12 @@ class Context:
     def plan_events(self, ev, n: int) -> "Plan":
         self._check(self._L.tofmlem_plan_events(self._h, C.byref(_events(ev, n)), C.c_uint64(n)))
         return self.plan_info()
+
+    def pass_timing(self):
+        """(tile, direct, stragglers) kernel milliseconds of the last planned fused pass."""
+        ms = (C.c_float * 3)()
+        self._check(self._L.tofmlem_pass_timing(self._h, ms))
+        return float(ms[0]), float(ms[1]), float(ms[2])
 
     def plan_info(self) -> "Plan":
         p = Plan()
