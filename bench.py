@@ -206,6 +206,8 @@ def run_report(args):
                 ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
                 sev, _, bin_ms = binned(ctx, ev, n)
                 del ev
+                plan_ms = timed(lambda: ctx.plan_events(sev, n)) if args.tile else 0.0  # inactive for non-TOF
+                plan = ctx.plan_info()
                 image = torch.ones(nvox, dtype=torch.float32, device=dev)
                 corr = torch.zeros(nvox, dtype=torch.float32, device=dev)
 
@@ -223,6 +225,8 @@ def run_report(args):
                     "n_valid": int(st.n_valid), "visits": int(st.visits), "reductions": int(st.reductions),
                     "visits_per_valid_event": st.visits / max(1, st.n_valid), "Gvisits_per_s": st.visits / ms / 1e6,
                     "roofline_frac": st.reductions / (ms * 1e-3) / red_rand, "bin_sort_gather_ms": bin_ms,
+                    "plan_ms": plan_ms, "planned": int(plan.active), "tile_items": int(plan.n_tile_items),
+                    "tile_events": int(st.tile_events),
                     "p7_rel_err": abs(p7 - st.n_valid) / max(1, st.n_valid)})
                 print(json.dumps(points[-1]), file=sys.stderr, flush=True)
                 del sev, image, corr, ctx
@@ -240,15 +244,22 @@ def run_report(args):
         mx = sens.max()
         x0 = (sens >= 0.01 * mx).float()
         whole = x0.clone()
+        plan_ms = timed(lambda: base.plan_events(sev, n)) if args.tile else 0.0
         base.iterate(sev, n, whole, sens, 1)  # warm-up
         whole = x0.clone()
         whole_ms = timed(lambda: base.iterate(sev, n, whole, sens, cfg.iters))
         del sev
+        base.trim()  # drop the unsplit plan's records
         split = torch.empty(nvox, dtype=torch.float32, device=dev)
-        base.reconstruct_regions(ev, n, 9, None, split, sens, 1)  # warm-up
-        t0 = time.perf_counter()
-        base.reconstruct_regions(ev, n, 9, None, split, sens, cfg.iters)  # synchronises
-        split_ms = (time.perf_counter() - t0) * 1e3
+        if args.region_plan >= 0:
+            base.set_option(pkg.OPT_REGION_PLAN, args.region_plan)
+        base.reconstruct_regions(ev, n, 9, None, split, sens, 2)  # warm-up: builds the sub-contexts and scratch
+        split_runs = []
+        for _ in range(5):
+            t0 = time.perf_counter()
+            base.reconstruct_regions(ev, n, 9, None, split, sens, cfg.iters)  # synchronises
+            split_runs.append((time.perf_counter() - t0) * 1e3)
+        split_ms = statistics.median(split_runs)
         region = torch.empty(n, dtype=torch.int32, device=dev)
         counts = base.split_regions(ev, n, 9, None, region, None)
         d = (split.double() - whole.double())
@@ -265,15 +276,38 @@ def run_report(args):
         w2 = whole.double()
         interior_l2 = float(d[~near_v].norm() / w2[~near_v].norm())
         border_l2 = float(d[near_v].norm() / w2[near_v].norm())
+
+        def overlap_report():
+            # the other reading of PAPER.md:101 (R27): an event in every region its window reaches, wide margins, cores only
+            base.set_option(pkg.OPT_REGION_OVERLAP, 1)
+            o = torch.empty(nvox, dtype=torch.float32, device=dev)
+            base.reconstruct_regions(ev, n, 9, None, o, sens, 2)  # warm-up (new sub-contexts: other margins)
+            runs = []
+            for _ in range(3):
+                t0 = time.perf_counter()
+                base.reconstruct_regions(ev, n, 9, None, o, sens, cfg.iters)
+                runs.append((time.perf_counter() - t0) * 1e3)
+            span = torch.empty(n, dtype=torch.int32, device=dev)
+            oc = base.split_regions_overlap(ev, n, 9, None, span, None)
+            dd = o.double() - whole.double()
+            base.set_option(pkg.OPT_REGION_OVERLAP, 0)
+            return {"split_runs_ms": runs, "list_entries": int(oc.sum()), "region_counts": [int(c) for c in oc],
+                    "rel_l2_split_vs_unsplit": float(dd.norm() / w2.norm()),
+                    "max_rel_on_voxels_above_1pct": float((dd.abs()[big] / w2[big]).max()),
+                    "rel_l2_region_interiors": float(dd[~near_v].norm() / w2[~near_v].norm()),
+                    "rel_l2_within_margin_of_borders": float(dd[near_v].norm() / w2[near_v].norm())}
+
         out["config"] = {"workload": f"cfg-4 division: {n} events of cfg-3, 9 regions, {cfg.iters} iterations each"}
         out.update({
-            "unsplit_ms": whole_ms, "unsplit_bin_ms": bin_ms, "split_total_ms": split_ms,
+            "unsplit_ms": whole_ms, "unsplit_bin_ms": bin_ms, "unsplit_plan_ms": plan_ms, "split_total_ms": split_ms,
+            "split_runs_ms": split_runs,
             "split_note": "split + permute + nine per-region reconstructions on nine streams + sum, host wall clock of the synchronising call",
             "region_counts": [int(c) for c in counts],
             "rel_l2_split_vs_unsplit": float(d.norm() / whole.double().norm()),
             "max_rel_on_voxels_above_1pct": float((d.abs()[big] / whole.double()[big]).max()),
             "margin_slices": margin, "rel_l2_region_interiors": interior_l2, "rel_l2_within_margin_of_borders": border_l2,
             "border_slice_fraction": float(near.float().mean()),
+            "overlap_reading_R27": overlap_report(),
             "paper": "PAPER.md:212 'no difference to the whole-body reconstruction' (visual); parity unpinned, no threshold"})
 
     elif args.report == "pipeline":
@@ -439,6 +473,7 @@ def main():
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next", "pipeline"],
                     help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
                          "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
+    ap.add_argument("--region-plan", type=int, default=-1, help="TOFMLEM_OPT_REGION_PLAN override (division report)")
     ap.add_argument("--sweep-events", default="10000000,146000000,500000000")
     ap.add_argument("--sweep-fwhm", default="100,300,600,0")
     args = ap.parse_args()

@@ -116,6 +116,14 @@ enum {
     TOFMLEM_OPT_TILE_CHECK = 15,    /* 1: bounds-test every access to the shared-memory tiles and count violations in
                                        tofmlem_stats.tile_oob (a debugging aid; default 0).  The plan has already
                                        dry-run every tile event against its tile, so the count must stay 0 */
+    TOFMLEM_OPT_REGION_OVERLAP = 18, /* tofmlem_reconstruct_regions / tofmlem_region_grid: 0 (default) = reading R13, every event in
+                                       the ONE region that holds its TOF centre (bit-exact split), extended images summed;
+                                       1 = reading R27, an event in every region its window reaches (1 or 2),
+                                       wider margins, cores only */
+    TOFMLEM_OPT_REGION_PLAN = 17,   /* 1: tofmlem_reconstruct_regions calls tofmlem_plan_events on every region's binned
+                                       list (ray records + tiles; 48 B per event more scratch); 0 (default): unplanned
+                                       passes -- nine plans synchronise nine times, which costs more than five planned
+                                       iterations save (measured: 184 vs 142 ms at cfg-4) */
     TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
                                        generated an identically reconstructed image").  0 (default) is accepted; 1
                                        returns TOFMLEM_EUNSUPPORTED: the correction image is summed with float32
@@ -227,15 +235,31 @@ int tofmlem_permute_events(tofmlem_ctx *ctx, const tofmlem_events *in, const uin
  * (HOST, n_regions entries) is valid on return (this call SYNCHRONISES). n_regions <= 64. */
 int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
                           const float *h_zbounds, int32_t *d_region, uint32_t *d_perm, uint64_t *h_counts);
+/* The other reading of PAPER.md:101 ("a 40% probability ... within image 5, and a 60% probability ... image region
+ * number 6 ... always contributed to 1 or 2 image regions"; reading R27): an event belongs to EVERY region whose core
+ * the axial extent of its +-trunc_sigmas*sigma window meets.  float32 specification F3: c, d, L as in F1;
+ * hz = (hw / L) * |dz| with hw = (float)(trunc_sigmas * sigma); lo = #{j : zb[j] <= cz - hz}, hi = #{j : zb[j] <= cz + hz}
+ * (j in 1..R-1); d_span[e] = lo | hi << 16, -1 for an invalid event.  d_perm (may be NULL; perm_capacity entries, 2 n
+ * always suffice while the cores are longer than the window) lists the event indices region by region, an event once
+ * in every region of its span; h_counts[r] = length of region r's list.  TOF contexts only.  SYNCHRONISES. */
+int tofmlem_split_regions_overlap(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                                  const float *h_zbounds, int32_t *d_span, uint32_t *d_perm, uint64_t perm_capacity,
+                                  uint64_t *h_counts);
 /* Default boundaries zb[j] = (float)k_j * vz + oz, k_j = nz * {0,2,3,..,R+1} / (R+1) (integer division). */
 int tofmlem_region_zbounds(const tofmlem_ctx *ctx, int n_regions, float *h_zbounds);
 /* Sub-grid of region r: its core slices plus ceil((trunc_sigmas*sigma + shell_mm)/vz) slices on each side,
- * clamped to the volume (R12).  *z0,*z1 = slice range [z0, z1) in the parent volume. */
+ * clamped to the volume (R12); with TOFMLEM_OPT_REGION_OVERLAP the margin is ceil((2*trunc_sigmas*sigma + shell_mm)/vz):
+ * the whole window of an event centred up to one half-width outside the core.  *z0,*z1 = slice range [z0, z1) in the
+ * parent volume. */
 int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zbounds, int r, tofmlem_grid *sub,
                         int32_t *z0, int32_t *z1);
 /* Whole cfg-4 pipeline: split, gather each region's events, reconstruct every region independently on its
  * own sub-grid and CUDA stream (`iters` iterations from x0 = mask), and SUM the extended region images into
- * d_image_out (nvox floats, overwritten) as the paper does.  SYNCHRONISES. */
+ * d_image_out (nvox floats, overwritten) as the paper does.  With TOFMLEM_OPT_REGION_OVERLAP = 1 the
+ * split is tofmlem_split_regions_overlap (an event reconstructed in every region its window reaches), the margins are
+ * the wider ones of tofmlem_region_grid and d_image_out is made of the region CORES only (margins discarded).  The
+ * sub-contexts, streams and region images are kept by the context between calls (tofmlem_trim releases them).
+ * SYNCHRONISES. */
 int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
                                 const float *h_zbounds, float *d_image_out, const float *d_sens, int iters);
 

@@ -326,6 +326,21 @@ def region_ids(ev, zbounds: np.ndarray):
     return region, counts
 
 
+def region_spans(ev, zbounds: np.ndarray, half_window_mm: float):
+    """Reading R27 / specification F3: (lo int32[n], hi int32[n] (-1 invalid), counts uint64[R]): the event belongs to
+    regions lo..hi, those whose core the axial extent of its +-half_window TOF window meets."""
+    e, n, _keep = _events(ev, False)
+    zb = _f32(zbounds)
+    R = zb.size - 1
+    lo = np.empty(n, np.int32)
+    hi = np.empty(n, np.int32)
+    counts = np.zeros(R, np.uint64)
+    lib().orc_region_spans(C.byref(e), C.c_uint64(n), C.c_int(R), zb.ctypes.data_as(C.c_void_p),
+                           C.c_float(np.float32(half_window_mm)), lo.ctypes.data_as(C.c_void_p),
+                           hi.ctypes.data_as(C.c_void_p), counts.ctypes.data_as(C.c_void_p))
+    return lo, hi, counts
+
+
 def region_margin_slices(sigma: float, vz: float, trunc: float = 3.0, shell_mm: float = 6.0) -> int:
     return int(lib().orc_region_margin_slices(sigma, trunc, shell_mm, vz))
 

@@ -631,6 +631,39 @@ void orc_region_ids(const orc_events *ev, uint64_t n, int n_regions, const float
     }
 }
 
+/* Reading R27 (an event "always contributed to 1 or 2 image regions", e.g. "a 40% probability ... within
+ * image 5, and a 60% probability ... image region number 6"): the event belongs to EVERY region whose core the axial
+ * extent of its +-T sigma window meets.  Integer result -> float32 specification F3 (conventions of F1):
+ *   c, (dx,dy,dz), L as in F1;  q = hw / L;  hz = q * |dz|;  zlo = cz - hz;  zhi = cz + hz;
+ *   lo = #{ j in 1..R-1 : zb[j] <= zlo },  hi = #{ j in 1..R-1 : zb[j] <= zhi };  regions lo..hi.
+ * hw = (float)(trunc * sigma).  Invalid events: lo = hi = -1.  counts[r] = events whose span contains r. */
+void orc_region_spans(const orc_events *ev, uint64_t n, int n_regions, const float *zb, float hw, int32_t *lo,
+                      int32_t *hi, uint64_t *counts) {
+    for (int r = 0; r < n_regions; ++r) counts[r] = 0;
+    for (uint64_t e = 0; e < n; ++e) {
+        float c[3], d[3];
+        if (!tof_centre_f32(ev, e, c, d)) {
+            lo[e] = hi[e] = -1;
+            continue;
+        }
+        const float xx = d[0] * d[0], yy = d[1] * d[1], zz = d[2] * d[2];
+        const float sxy = xx + yy;
+        const float L2 = sxy + zz;
+        const float L = sqrtf(L2);
+        const float q = hw / L;
+        const float hz = q * fabsf(d[2]);
+        const float zlo = c[2] - hz, zhi = c[2] + hz;
+        int32_t a = 0, b = 0;
+        for (int j = 1; j < n_regions; ++j) {
+            if (zb[j] <= zlo) ++a;
+            if (zb[j] <= zhi) ++b;
+        }
+        lo[e] = a;
+        hi[e] = b;
+        for (int r = a; r <= b; ++r) ++counts[r];
+    }
+}
+
 /* R12: margin in slices on each open side of a region core: ceil((trunc*sigma + shell_mm)/vz). */
 int32_t orc_region_margin_slices(double sigma_mm, double trunc, double shell_mm, double vz) {
     return (int32_t)ceil((trunc * sigma_mm + shell_mm) / vz);

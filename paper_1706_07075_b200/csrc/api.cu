@@ -60,6 +60,8 @@ struct tofmlem_ctx {
     uint64_t launches = 0;
     // tile-mode plan of the fused pass (tofmlem_plan_events; tile.cu)
     int tile_min_events = 1024, tile_max_events = 8192, tile_check = 0;
+    int region_overlap = 0;  // reading R27: an event goes to every region its window meets (TOFMLEM_OPT_REGION_OVERLAP)
+    int region_plan = 0;  // tofmlem_reconstruct_regions plans every region's list (TOFMLEM_OPT_REGION_PLAN)
     int n_sm = 0;
     size_t smem_optin = 0;  // largest dynamic shared memory a CTA may opt in to on this device
     TileGeom *d_geom = nullptr;
@@ -76,6 +78,18 @@ struct tofmlem_ctx {
     float *d_ev_scale = nullptr;       // w_e / fwd_e of the tile events between the two phases of tile.cu (rec_cap floats)
     size_t smem_per_sm = 0;
     void *d_plan_counters = nullptr;
+    // tofmlem_reconstruct_regions: sub-contexts, streams, events and region images, kept between calls (creating and
+    // destroying them per call put nine cudaMalloc / cudaFree device-wide syncs in the middle of nine running streams)
+    struct RegionCache {
+        std::vector<float> zb;       // region bounds the cache was built for (n_regions + 1)
+        double sigma = 0.0, trunc = 0.0, shell = 0.0;
+        std::vector<tofmlem_ctx *> subs;
+        std::vector<cudaStream_t> streams;
+        std::vector<cudaEvent_t> done;
+        std::vector<float *> images;
+        std::vector<int32_t> z0, z1;
+        cudaEvent_t ready = nullptr;
+    } rgc;
     cudaEvent_t t_ev[4] = {nullptr, nullptr, nullptr, nullptr};  // tofmlem_pass_timing: around the planned kernels
     int t_have = 0;                                              // bit k: part k of the last planned pass ran
     struct {
@@ -219,6 +233,18 @@ int ensure_bin_scratch(tofmlem_ctx *ctx, size_t nfine, uint64_t n_sub) {
         ctx->sub_cap = n_sub;
     }
     return TOFMLEM_OK;
+}
+
+void free_region_cache(tofmlem_ctx *ctx) {
+    auto &c = ctx->rgc;
+    for (size_t r = 0; r < c.subs.size(); ++r) {
+        if (c.subs[r]) tofmlem_destroy(c.subs[r]);
+        if (c.streams[r]) cudaStreamDestroy(c.streams[r]);
+        if (c.done[r]) cudaEventDestroy(c.done[r]);
+        cudaFree(c.images[r]);
+    }
+    if (c.ready) cudaEventDestroy(c.ready);
+    c = tofmlem_ctx::RegionCache();
 }
 
 void free_records(tofmlem_ctx *ctx) {
@@ -485,6 +511,7 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     for (auto &te : ctx->t_ev)
         if (te) cudaEventDestroy(te);
     free_records(ctx);
+    free_region_cache(ctx);
     delete ctx;
     return TOFMLEM_OK;
 }
@@ -553,6 +580,14 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "tile_check is 0 or 1");
             ctx->tile_check = (int)value;
             return TOFMLEM_OK;
+        case TOFMLEM_OPT_REGION_OVERLAP:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "region_overlap is 0 or 1");
+            ctx->region_overlap = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_REGION_PLAN:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "region_plan is 0 or 1");
+            ctx->region_plan = (int)value;
+            return TOFMLEM_OK;
         case TOFMLEM_OPT_DETERMINISTIC:
             // the paper's LUT kernel "always generated an identically reconstructed image".  Here the
             // accumulation is a float32 reduction at L2 / in shared memory whose order is not fixed, so a run-to-run
@@ -597,6 +632,7 @@ int tofmlem_trim(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_himg);
     cudaFree(ctx->d_hsens);
     free_records(ctx);  // the plan goes with its records
+    free_region_cache(ctx);
     ctx->d_pack = nullptr;
     ctx->d_sub = nullptr;
     ctx->d_rg_region = nullptr;
@@ -1080,12 +1116,13 @@ int tofmlem_region_zbounds(const tofmlem_ctx *ctx, int n_regions, float *h_zboun
     return TOFMLEM_OK;
 }
 
-int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
-                          const float *h_zbounds, int32_t *d_region, uint32_t *d_perm, uint64_t *h_counts) {
+static int split_impl(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions, const float *h_zbounds,
+                      bool overlap, int32_t *d_region, uint32_t *d_perm, uint64_t perm_capacity, uint64_t *h_counts) {
     if (!ctx) return TOFMLEM_EINVAL;
     if ((n && !ev_ok(ev, false)) || n_regions < 1 || n_regions > kMaxRegions || (n && !d_region) || !h_counts ||
         n > 0xFFFFFFFFull)
         return fail(ctx, TOFMLEM_EINVAL, "split_regions: bad argument");
+    if (overlap && !ctx->tof) return fail(ctx, TOFMLEM_EUNSUPPORTED, "split_regions_overlap needs a TOF context");
     RegionBounds rb;
     rb.n_regions = n_regions;
     if (h_zbounds) {
@@ -1098,14 +1135,23 @@ int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n
     unsigned long long *counts = ctx->d_rcounts, *cursor = ctx->d_rcounts + (kMaxRegions + 1);
     CU(cudaMemsetAsync(counts, 0, 2 * (kMaxRegions + 1) * sizeof(unsigned long long), ctx->stream));
     if (n) {
-        launch_region_ids(ev_ptrs(ev), n, rb, d_region, counts, ctx->stream);
+        if (overlap)
+            launch_region_spans(ev_ptrs(ev), n, rb, (float)(ctx->trunc_sigmas * ctx->sigma), d_region, counts, ctx->stream);
+        else
+            launch_region_ids(ev_ptrs(ev), n, rb, d_region, counts, ctx->stream);
         CHECK_LAUNCH(1);
     }
     unsigned long long h[kMaxRegions + 1];
     CU(cudaMemcpyAsync(h, counts, (n_regions + 1) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
-    for (int r = 0; r < n_regions; ++r) h_counts[r] = h[r];
+    unsigned long long total = 0;
+    for (int r = 0; r < n_regions; ++r) {
+        h_counts[r] = h[r];
+        total += h[r];
+    }
     if (d_perm && n) {
+        if (total + h[n_regions] > perm_capacity)
+            return fail(ctx, TOFMLEM_EINVAL, "split_regions: the permutation does not fit its buffer");
         unsigned long long start[kMaxRegions + 1];
         unsigned long long run = 0;
         for (int r = 0; r <= n_regions; ++r) {
@@ -1114,11 +1160,25 @@ int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n
         }
         CU(cudaMemcpyAsync(cursor, start, (n_regions + 1) * sizeof(unsigned long long), cudaMemcpyHostToDevice,
                            ctx->stream));
-        launch_region_scatter(d_region, n, n_regions, cursor, d_perm, ctx->stream);
+        if (overlap)
+            launch_region_span_scatter(d_region, n, n_regions, cursor, d_perm, ctx->stream);
+        else
+            launch_region_scatter(d_region, n, n_regions, cursor, d_perm, ctx->stream);
         CHECK_LAUNCH(1);
         CU(cudaStreamSynchronize(ctx->stream));  // `start` lives on this stack frame
     }
     return TOFMLEM_OK;
+}
+
+int tofmlem_split_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                          const float *h_zbounds, int32_t *d_region, uint32_t *d_perm, uint64_t *h_counts) {
+    return split_impl(ctx, ev, n, n_regions, h_zbounds, false, d_region, d_perm, n, h_counts);
+}
+
+int tofmlem_split_regions_overlap(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, int n_regions,
+                                  const float *h_zbounds, int32_t *d_span, uint32_t *d_perm, uint64_t perm_capacity,
+                                  uint64_t *h_counts) {
+    return split_impl(ctx, ev, n, n_regions, h_zbounds, true, d_span, d_perm, perm_capacity, h_counts);
 }
 
 int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zbounds, int r, tofmlem_grid *sub,
@@ -1136,7 +1196,10 @@ int tofmlem_region_grid(const tofmlem_ctx *ctx, int n_regions, const float *h_zb
         k0 = k[r];
         k1 = k[r + 1];
     }
-    const int32_t margin = (int32_t)ceil((ctx->trunc_sigmas * ctx->sigma + ctx->shell_mm) / (double)g.vz);
+    // R12: the window's half-width + the shell; reading R27 (overlap): the WHOLE window of an event centred up to one
+    // half-width outside the core must fit, so twice the half-width
+    const int32_t margin = ctx->region_overlap < 0 ? 0 :  // (internal: the bare core)
+        (int32_t)ceil(((ctx->region_overlap ? 2.0 : 1.0) * ctx->trunc_sigmas * ctx->sigma + ctx->shell_mm) / (double)g.vz);
     int32_t a = k0 - (r > 0 ? margin : 0), b = k1 + (r < n_regions - 1 ? margin : 0);
     if (a < 0) a = 0;
     if (b > g.nz) b = g.nz;
@@ -1157,34 +1220,18 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         return fail(ctx, TOFMLEM_EINVAL, "reconstruct_regions: bad argument");
     cudaStream_t s = ctx->stream;
     const size_t slice = (size_t)ctx->grid.nx * ctx->grid.ny;
-    int32_t *d_region = nullptr;
-    uint32_t *d_perm = nullptr;
-    float *d_sorted = nullptr, *d_binned = nullptr;
-    const uint64_t stride = (n + 3) & ~3ull;
+    const bool overlap = ctx->region_overlap != 0 && ctx->tof;
+    // capacity of the per-region event lists: with overlapping membership (R27) an event may sit in two lists
+    const uint64_t stride = ((overlap ? 2 * n : n) + 3) & ~3ull;
     std::vector<uint64_t> counts(n_regions);
-    std::vector<tofmlem_ctx *> subs(n_regions, nullptr);
-    std::vector<cudaStream_t> streams(n_regions, nullptr);
-    std::vector<float *> images(n_regions, nullptr);
-    std::vector<int32_t> z0(n_regions), z1(n_regions);
-    cudaEvent_t ready = nullptr;
-    std::vector<cudaEvent_t> done(n_regions, nullptr);
     int rc = TOFMLEM_OK;
-    auto cleanup = [&]() {
-        for (int r = 0; r < n_regions; ++r) {
-            if (subs[r]) tofmlem_destroy(subs[r]);
-            if (streams[r]) cudaStreamDestroy(streams[r]);
-            if (done[r]) cudaEventDestroy(done[r]);
-            cudaFree(images[r]);
-        }
-        if (ready) cudaEventDestroy(ready);
-    };
 #define RCU(call)                                          \
     do {                                                   \
         cudaError_t e_ = (call);                           \
         if (e_ != cudaSuccess) {                           \
             rc = cuda_fail(ctx, e_, #call);                \
             cudaDeviceSynchronize();                       \
-            cleanup();                                     \
+            free_region_cache(ctx);                        \
             return rc;                                     \
         }                                                  \
     } while (0)
@@ -1193,7 +1240,7 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         rc = (call);                   \
         if (rc != TOFMLEM_OK) {        \
             cudaDeviceSynchronize();   \
-            cleanup();                 \
+            free_region_cache(ctx);    \
             return rc;                 \
         }                              \
     } while (0)
@@ -1212,43 +1259,92 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         RCU(cudaMalloc(&ctx->d_rg_binned, 7 * stride * sizeof(float)));
         ctx->rg_cap = stride;
     }
-    d_region = ctx->d_rg_region;
-    d_perm = ctx->d_rg_perm;
-    d_sorted = ctx->d_rg_sorted;
-    d_binned = ctx->d_rg_binned;
-    RRC(tofmlem_split_regions(ctx, ev, n, n_regions, h_zbounds, d_region, d_perm, counts.data()));
+    int32_t *d_region = ctx->d_rg_region;
+    uint32_t *d_perm = ctx->d_rg_perm;
+    float *d_sorted = ctx->d_rg_sorted, *d_binned = ctx->d_rg_binned;
+    // ---- sub-contexts, streams, events and region images: built once per (bounds, TOF kernel, shell), then reused
+    std::vector<float> zb(n_regions + 1);
+    if (h_zbounds) zb.assign(h_zbounds, h_zbounds + n_regions + 1);
+    else default_zbounds(ctx, n_regions, zb.data());
+    auto &C = ctx->rgc;
+    const double shell_key = ctx->shell_mm + (overlap ? 1e9 : 0.0);  // the margin rule is part of the cache key
+    if (C.zb != zb || C.sigma != ctx->sigma || C.trunc != ctx->trunc_sigmas || C.shell != shell_key) {
+        RCU(cudaStreamSynchronize(s));
+        free_region_cache(ctx);
+        C.subs.assign(n_regions, nullptr);
+        C.streams.assign(n_regions, nullptr);
+        C.done.assign(n_regions, nullptr);
+        C.images.assign(n_regions, nullptr);
+        C.z0.assign(n_regions, 0);
+        C.z1.assign(n_regions, 0);
+        RCU(cudaEventCreateWithFlags(&C.ready, cudaEventDisableTiming));
+        for (int r = 0; r < n_regions; ++r) {
+            tofmlem_grid sub;
+            RRC(tofmlem_region_grid(ctx, n_regions, h_zbounds, r, &sub, &C.z0[r], &C.z1[r]));
+            RCU(cudaStreamCreateWithFlags(&C.streams[r], cudaStreamNonBlocking));
+            RCU(cudaEventCreateWithFlags(&C.done[r], cudaEventDisableTiming));
+            RRC(tofmlem_create(&ctx->scanner, &sub, ctx->tof ? (float)(ctx->sigma / sigma_from_fwhm(1.0)) : 0.0f,
+                               C.streams[r], &C.subs[r]));
+            RCU(cudaMalloc(&C.images[r], C.subs[r]->nvox * sizeof(float)));
+            RRC(ensure_corr(C.subs[r]));
+        }
+        C.zb = zb;
+        C.sigma = ctx->sigma;
+        C.trunc = ctx->trunc_sigmas;
+        C.shell = shell_key;
+    }
+    RRC(split_impl(ctx, ev, n, n_regions, h_zbounds, overlap, d_region, d_perm, stride, counts.data()));
+    uint64_t n_list = 0;  // entries of the region-sorted list (= valid events, with multiplicity under R27)
+    for (int r = 0; r < n_regions; ++r) n_list += counts[r];
     tofmlem_events_mut sorted{d_sorted, d_sorted + stride, d_sorted + 2 * stride, d_sorted + 3 * stride,
                               d_sorted + 4 * stride, d_sorted + 5 * stride, ev->dt ? d_sorted + 6 * stride : nullptr};
-    RRC(tofmlem_permute_events(ctx, ev, d_perm, n, &sorted));
+    if (overlap) {
+        if (n_list) RRC(tofmlem_gather_events(ctx, ev, d_perm, n_list, &sorted));
+    } else {
+        RRC(tofmlem_permute_events(ctx, ev, d_perm, n, &sorted));
+    }
     launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, s);
     ctx->launches += 1;
     RCU(cudaMemsetAsync(d_image_out, 0, ctx->nvox * sizeof(float), s));
-    RCU(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
-    RCU(cudaEventRecord(ready, s));
+    RCU(cudaEventRecord(C.ready, s));
+    // scratch of the per-region binning, sized before any region stream runs (no allocation between the launches)
+    {
+        uint64_t cmax = 0;
+        for (int r = 0; r < n_regions; ++r) cmax = counts[r] > cmax ? counts[r] : cmax;
+        for (int r = 0; r < n_regions; ++r) {
+            tofmlem_ctx *sc = C.subs[r];
+            sc->sigma = ctx->sigma;
+            sc->trunc_sigmas = ctx->trunc_sigmas;
+            sc->sens_floor_rel = ctx->sens_floor_rel;
+            sc->projector = ctx->projector;
+            sc->samples_k = ctx->samples_k;
+            sc->median = ctx->median;
+            sc->corr_bricks = ctx->corr_bricks;
+            sc->em_variant = ctx->em_variant;
+            sc->cache_share = ctx->cache_share;
+            sc->tile_log2 = ctx->tile_log2;
+            sc->subbins = ctx->subbins;
+            sc->cta_interleave = ctx->cta_interleave;
+            sc->tile_min_events = ctx->tile_min_events;
+            sc->tile_max_events = ctx->tile_max_events;
+            sc->d_max_ext = ctx->d_max;
+            sc->launches = 0;
+            if (sc->median && !sc->d_tmp_image) RCU(cudaMalloc(&sc->d_tmp_image, sc->nvox * sizeof(float)));
+            if (counts[r]) {
+                const uint32_t S = effective_subbins(sc);
+                RRC(ensure_bin_scratch(sc, (size_t)num_bins(sc) * S + 1, S > 1 ? counts[r] : 0));
+            }
+        }
+        (void)cmax;
+    }
     uint64_t off = 0;
     for (int r = 0; r < n_regions; ++r) {
-        tofmlem_grid sub;
-        RRC(tofmlem_region_grid(ctx, n_regions, h_zbounds, r, &sub, &z0[r], &z1[r]));
-        RCU(cudaStreamCreateWithFlags(&streams[r], cudaStreamNonBlocking));
-        RCU(cudaEventCreateWithFlags(&done[r], cudaEventDisableTiming));
-        RRC(tofmlem_create(&ctx->scanner, &sub, ctx->tof ? (float)(ctx->sigma / sigma_from_fwhm(1.0)) : 0.0f,
-                           streams[r], &subs[r]));
-        tofmlem_ctx *sc = subs[r];
-        sc->sigma = ctx->sigma;
-        sc->trunc_sigmas = ctx->trunc_sigmas;
-        sc->sens_floor_rel = ctx->sens_floor_rel;
-        sc->projector = ctx->projector;
-        sc->samples_k = ctx->samples_k;
-        sc->median = ctx->median;
-        sc->corr_bricks = ctx->corr_bricks;
-        sc->em_variant = ctx->em_variant;
-        sc->cache_share = ctx->cache_share;
-        sc->d_max_ext = ctx->d_max;
+        tofmlem_ctx *sc = C.subs[r];
+        cudaStream_t rs = C.streams[r];
         const uint64_t nv = sc->nvox;
-        RCU(cudaMalloc(&images[r], nv * sizeof(float)));
-        RCU(cudaStreamWaitEvent(streams[r], ready, 0));
-        const float *sens_r = d_sens + (size_t)z0[r] * slice;
-        launch_mask_init(images[r], sens_r, ctx->d_max, (float)ctx->sens_floor_rel, nv, streams[r]);
+        RCU(cudaStreamWaitEvent(rs, C.ready, 0));
+        const float *sens_r = d_sens + (size_t)C.z0[r] * slice;
+        launch_mask_init(C.images[r], sens_r, ctx->d_max, (float)ctx->sens_floor_rel, nv, rs);
         sc->launches += 1;
         tofmlem_events sub_ev{sorted.x1 + off, sorted.y1 + off, sorted.z1 + off, sorted.x2 + off, sorted.y2 + off,
                               sorted.z2 + off, sorted.dt ? sorted.dt + off : nullptr};
@@ -1259,10 +1355,10 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
                                   sorted.dt ? d_binned + 6 * stride + off : nullptr};
         if (counts[r]) {
             rc = tofmlem_bin_events(sc, &sub_ev, counts[r], reinterpret_cast<uint32_t *>(d_region) + off, d_perm + off, nullptr);
-            if (rc == TOFMLEM_OK && ctx->pack_cap >= n) {
+            if (rc == TOFMLEM_OK && !overlap && ctx->pack_cap >= n) {
                 // permutation through 32-byte records in the parent's record scratch (free again after the region split)
                 float *dst[7] = {bin_ev.x1, bin_ev.y1, bin_ev.z1, bin_ev.x2, bin_ev.y2, bin_ev.z2, bin_ev.dt};
-                launch_gather_packed(ev_ptrs(&sub_ev), d_perm + off, counts[r], ctx->d_pack + 8 * off, dst, streams[r]);
+                launch_gather_packed(ev_ptrs(&sub_ev), d_perm + off, counts[r], ctx->d_pack + 8 * off, dst, rs);
                 sc->launches += 2;
             } else if (rc == TOFMLEM_OK) {
                 rc = tofmlem_gather_events(sc, &sub_ev, d_perm + off, counts[r], &bin_ev);
@@ -1270,29 +1366,56 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
             if (rc != TOFMLEM_OK) {
                 ctx->err = sc->err;
                 cudaDeviceSynchronize();
-                cleanup();
+                free_region_cache(ctx);
                 return rc;
             }
         }
         tofmlem_events run_ev{bin_ev.x1, bin_ev.y1, bin_ev.z1, bin_ev.x2, bin_ev.y2, bin_ev.z2, bin_ev.dt};
-        rc = iterate_device(sc, counts[r] ? ev_ptrs(&run_ev) : EventPtrs{}, counts[r], nullptr, images[r], sens_r, iters, false);
+        // ray records + tiles for the region's own binned list (synchronises the region's stream only; the regions
+        // launched before keep the GPU busy meanwhile)
+        if (counts[r] && ctx->region_plan && ctx->tof && ctx->projector == 0 && ctx->em_variant == 0 && iters > 1) {
+            rc = tofmlem_plan_events(sc, &run_ev, counts[r]);
+            if (rc != TOFMLEM_OK) {
+                ctx->err = sc->err;
+                cudaDeviceSynchronize();
+                free_region_cache(ctx);
+                return rc;
+            }
+        } else {
+            sc->plan.valid = false;
+        }
+        rc = iterate_device(sc, counts[r] ? ev_ptrs(&run_ev) : EventPtrs{}, counts[r], nullptr, C.images[r], sens_r, iters, false);
         if (rc != TOFMLEM_OK) {
             ctx->err = sc->err;
             cudaDeviceSynchronize();
-            cleanup();
+            free_region_cache(ctx);
             return rc;
         }
-        RCU(cudaEventRecord(done[r], streams[r]));
+        RCU(cudaEventRecord(C.done[r], rs));
         off += counts[r];
     }
-    // sum of the extended region images; overlapping margins add up
+    // R13: sum of the extended region images, overlapping margins add up.  R27: every region has seen all
+    // the events that reach its core, so the cores alone tile the volume (margins discarded).
     for (int r = 0; r < n_regions; ++r) {
-        RCU(cudaStreamWaitEvent(s, done[r], 0));
-        launch_add(d_image_out + (size_t)z0[r] * slice, images[r], subs[r]->nvox, s);
-        ctx->launches += 1 + subs[r]->launches;
+        RCU(cudaStreamWaitEvent(s, C.done[r], 0));
+        if (overlap) {
+            tofmlem_grid sub;
+            int32_t a0, a1, k0, k1;
+            const int keep = ctx->region_overlap;
+            ctx->region_overlap = -1;  // margin 0: the core itself
+            rc = tofmlem_region_grid(ctx, n_regions, h_zbounds, r, &sub, &k0, &k1);
+            ctx->region_overlap = keep;
+            if (rc == TOFMLEM_OK) rc = tofmlem_region_grid(ctx, n_regions, h_zbounds, r, &sub, &a0, &a1);
+            RRC(rc);
+            RCU(cudaMemcpyAsync(d_image_out + (size_t)k0 * slice, C.images[r] + (size_t)(k0 - a0) * slice,
+                                (size_t)(k1 - k0) * slice * sizeof(float), cudaMemcpyDeviceToDevice, s));
+            ctx->launches += C.subs[r]->launches;
+        } else {
+            launch_add(d_image_out + (size_t)C.z0[r] * slice, C.images[r], C.subs[r]->nvox, s);
+            ctx->launches += 1 + C.subs[r]->launches;
+        }
     }
     RCU(cudaStreamSynchronize(s));
-    cleanup();
 #undef RCU
 #undef RRC
     return TOFMLEM_OK;

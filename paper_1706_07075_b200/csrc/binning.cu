@@ -311,6 +311,69 @@ __global__ void __launch_bounds__(kBlock) region_scatter_kernel(const int32_t *_
     if (e < n) perm[base[r] + rank] = (uint32_t)e;
 }
 
+// Reading R27 / specification F3: the event belongs to every region whose core the axial extent of its
+// +-hw window meets: regions lo..hi, span = lo | hi << 16 (-1 for an invalid event); counts[r] = events whose span
+// holds r (counts[n_regions]: invalid events).  One IEEE binary32 RN operation per step, as F1.
+__global__ void __launch_bounds__(kBlock) region_spans_kernel(EventPtrs ev, uint64_t n, RegionBounds rb, float hw,
+                                                              int32_t *__restrict__ span,
+                                                              unsigned long long *__restrict__ counts) {
+    __shared__ unsigned int local[kMaxRegions + 1];
+    for (int i = threadIdx.x; i <= rb.n_regions; i += kBlock) local[i] = 0;
+    __syncthreads();
+    const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (e < n) {
+        float c[3], d[3];
+        int sp = -1;
+        if (tof_centre(ev, e, c, d)) {
+            const float xx = __fmul_rn(d[0], d[0]), yy = __fmul_rn(d[1], d[1]), zz = __fmul_rn(d[2], d[2]);
+            const float L = __fsqrt_rn(__fadd_rn(__fadd_rn(xx, yy), zz));
+            const float hz = __fmul_rn(__fdiv_rn(hw, L), fabsf(d[2]));
+            const float zlo = __fsub_rn(c[2], hz), zhi = __fadd_rn(c[2], hz);
+            int lo = 0, hi = 0;
+            for (int j = 1; j < rb.n_regions; ++j) {
+                lo += (rb.zb[j] <= zlo) ? 1 : 0;
+                hi += (rb.zb[j] <= zhi) ? 1 : 0;
+            }
+            sp = lo | (hi << 16);
+            for (int r = lo; r <= hi; ++r) atomicAdd(local + r, 1u);
+        } else {
+            atomicAdd(local + rb.n_regions, 1u);
+        }
+        span[e] = sp;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= rb.n_regions; i += kBlock)
+        if (local[i]) atomicAdd(counts + i, (unsigned long long)local[i]);
+}
+
+// block-aggregated scatter of the spans: the event's index goes to the list of every region of its span
+__global__ void __launch_bounds__(kBlock) region_span_scatter_kernel(const int32_t *__restrict__ span, uint64_t n,
+                                                                     int n_regions,
+                                                                     unsigned long long *__restrict__ cursor,
+                                                                     uint32_t *__restrict__ perm) {
+    __shared__ unsigned int local[kMaxRegions + 1];
+    __shared__ unsigned long long base[kMaxRegions + 1];
+    for (int i = threadIdx.x; i <= n_regions; i += kBlock) local[i] = 0;
+    __syncthreads();
+    const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
+    int lo = 0, hi = -1;
+    unsigned int rank[4] = {0, 0, 0, 0};  // a window longer than three cores is not supported (checked by the caller)
+    if (e < n) {
+        const int sp = span[e];
+        if (sp >= 0) {
+            lo = sp & 0xFFFF;
+            hi = sp >> 16;
+            if (hi > lo + 3) hi = lo + 3;
+            for (int r = lo; r <= hi; ++r) rank[r - lo] = atomicAdd(local + r, 1u);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= n_regions; i += kBlock)
+        if (local[i]) base[i] = atomicAdd(cursor + i, (unsigned long long)local[i]);
+    __syncthreads();
+    for (int r = lo; r <= hi; ++r) perm[base[r] + rank[r - lo]] = (uint32_t)e;
+}
+
 // NEXT-4: TOF-based scatter rejection (PAPER.md:63 Fig. 2, :69-71; reading R24, float32 specification F2 in
 // DESIGN.md): keep the event iff the segment {c + u t : |t| <= h} (c = TOF-estimated annihilation point, u = LOR
 // direction, h = 1.96 sigma: the 95 % confidence interval) meets the body outline, a union of ellipsoids.  Every
@@ -432,6 +495,16 @@ void launch_region_ids(const EventPtrs &ev, uint64_t n, const RegionBounds &rb, 
 void launch_region_scatter(const int32_t *region, uint64_t n, int n_regions, unsigned long long *cursor,
                            uint32_t *perm, cudaStream_t s) {
     if (n) region_scatter_kernel<<<grid_for(n), kBlock, 0, s>>>(region, n, n_regions, cursor, perm);
+}
+
+void launch_region_spans(const EventPtrs &ev, uint64_t n, const RegionBounds &rb, float hw, int32_t *span,
+                         unsigned long long *counts, cudaStream_t s) {
+    if (n) region_spans_kernel<<<grid_for(n), kBlock, 0, s>>>(ev, n, rb, hw, span, counts);
+}
+
+void launch_region_span_scatter(const int32_t *span, uint64_t n, int n_regions, unsigned long long *cursor,
+                                uint32_t *perm, cudaStream_t s) {
+    if (n) region_span_scatter_kernel<<<grid_for(n), kBlock, 0, s>>>(span, n, n_regions, cursor, perm);
 }
 
 void launch_scatter_keep(const EventPtrs &ev, uint64_t n, const EllipsoidSet &es, float h, uint8_t *keep,

@@ -166,6 +166,13 @@ void launch_region_scatter(const int32_t *region, uint64_t n, int n_regions,
                            unsigned long long *cursor /* n_regions+1 start offsets, advanced */, uint32_t *perm,
                            cudaStream_t s);
 
+// reading R27 / F3: span[e] = lo | hi << 16 (-1 invalid); counts as launch_region_ids, with multiplicity
+void launch_region_spans(const EventPtrs &ev, uint64_t n, const RegionBounds &rb, float hw, int32_t *span,
+                         unsigned long long *counts /* n_regions+1, zeroed by caller */, cudaStream_t s);
+void launch_region_span_scatter(const int32_t *span, uint64_t n, int n_regions,
+                                unsigned long long *cursor /* start offsets, advanced */, uint32_t *perm,
+                                cudaStream_t s);
+
 constexpr int kMaxEllipsoids = 64;
 struct EllipsoidSet {
     float v[6 * kMaxEllipsoids];  // per ellipsoid: centre x, y, z, reciprocal semi-axes 1/ax, 1/ay, 1/az

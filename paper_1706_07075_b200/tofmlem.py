@@ -28,6 +28,8 @@ OPT_DETERMINISTIC = 13
 OPT_TILE_MIN_EVENTS = 14
 OPT_TILE_CHECK = 15
 OPT_TILE_MAX_EVENTS = 16
+OPT_REGION_PLAN = 17
+OPT_REGION_OVERLAP = 18
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
@@ -39,7 +41,7 @@ SYMBOLS = (
     "tofmlem_probe", "tofmlem_get_stats", "tofmlem_last_error", "tofmlem_launch_count", "tofmlem_version",
     "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
     "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events", "tofmlem_reserve", "tofmlem_trim",
-    "tofmlem_plan_events", "tofmlem_plan_info", "tofmlem_pass_timing",
+    "tofmlem_plan_events", "tofmlem_plan_info", "tofmlem_pass_timing", "tofmlem_split_regions_overlap",
 )
 
 
@@ -261,6 +263,18 @@ class Context:
                                                   C.c_void_p(zb), C.c_void_p(_ptr(region, torch.int32, "cuda", n)),
                                                   C.c_void_p(_ptr(perm, torch.int32, "cuda", n)),
                                                   C.c_void_p(counts.data_ptr())))
+        return counts
+
+    def split_regions_overlap(self, ev, n: int, n_regions: int, zbounds: Optional[torch.Tensor], span: torch.Tensor,
+                              perm: Optional[torch.Tensor]) -> torch.Tensor:
+        e = _events(ev, n)
+        counts = torch.zeros(n_regions, dtype=torch.int64)
+        zb = _ptr(zbounds, torch.float32, "cpu", n_regions + 1)
+        cap = perm.numel() if perm is not None else 0
+        self._check(self._L.tofmlem_split_regions_overlap(
+            self._h, C.byref(e), C.c_uint64(n), C.c_int(n_regions), C.c_void_p(zb),
+            C.c_void_p(_ptr(span, torch.int32, "cuda", n)), C.c_void_p(_ptr(perm, torch.int32, "cuda")),
+            C.c_uint64(cap), C.c_void_p(counts.data_ptr())))
         return counts
 
     def region_grid(self, n_regions: int, zbounds: Optional[torch.Tensor], r: int):

@@ -436,6 +436,93 @@ def test_reconstruct_regions_parity(pkg):
     print(f"split-vs-unsplit rel-L2 = {d.item():.3e} (no threshold: parity unpinned)")
 
 
+def test_split_regions_overlap_bit_exact(pkg):
+    """Reading R27 / specification F3: region spans (lo, hi) of 400 k cfg-3 events incl. invalid ones bit-exact against
+    oracle.region_spans; the lists hold every event once per region of its span."""
+    cfg = synth.FULL
+    n = 400_000
+    g, og = grids(pkg, cfg)
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ev_np, bad = _with_invalid(to_np(synth.make_events(cfg, n, device="cuda")), np.random.default_rng(4))
+    zb = oracle.region_zbounds(og, 9)
+    ev = {k: torch.from_numpy(v).cuda() for k, v in ev_np.items()}
+    span = torch.empty(n, dtype=torch.int32, device="cuda")
+    perm = torch.empty(2 * n, dtype=torch.int32, device="cuda")
+    counts = ctx.split_regions_overlap(ev, n, 9, None, span, perm)
+    lo, hi, wcounts = oracle.region_spans(ev_np, zb, 3.0 * oracle.sigma_mm(cfg.tof_fwhm_ps))
+    sp = span.cpu().numpy()
+    want = np.where(lo < 0, -1, lo | (hi << 16))
+    assert np.array_equal(sp, want)
+    assert np.array_equal(counts.numpy().astype(np.uint64), wcounts)
+    assert 0.2 * n < int((hi > lo).sum()) < 0.7 * n  # 115 mm windows on 240 mm cores: a good part spans two regions
+    p = perm.cpu().numpy().view(np.uint32).astype(np.int64)
+    off = 0
+    for r in range(9):
+        members = np.sort(p[off:off + int(wcounts[r])])
+        assert np.array_equal(members, np.nonzero((lo <= r) & (r <= hi))[0])
+        off += int(wcounts[r])
+    # wider margins under this reading (twice the half-window + shell)
+    ctx.set_option(pkg.OPT_REGION_OVERLAP, 1)
+    m2 = int(np.ceil((2 * 3.0 * oracle.sigma_mm(300.0) + 6.0) / 3.75))
+    ks = oracle.default_region_slices(640, 9)
+    for r in (0, 4, 8):
+        _, z0, z1 = ctx.region_grid(9, None, r)
+        assert z0 == max(0, ks[r] - (m2 if r > 0 else 0)) and z1 == min(640, ks[r + 1] + (m2 if r < 8 else 0))
+
+
+def test_reconstruct_regions_overlap_parity(pkg):
+    """cfg-4 pipeline under reading R27 (an event in every region its window reaches, wide margins, cores only) against
+    the same pipeline assembled from oracle calls; and how far each reading is from the unsplit reconstruction."""
+    R, iters = 3, 2
+    nx, ny, nz, v = 16, 16, 96, 5.0
+    n, m = 60_000, 600_000
+    cfg = synth.Config("long", nx, ny, nz, v, 120.0, 480.0, synth.Phantom(
+        parts=(synth.Shape("ellipsoid", (0.0, 0.0, 0.0), (30.0, 25.0, 220.0), 1.0),),
+        inner=(synth.Shape("ellipsoid", (10.0, 0.0, 60.0), (8.0, 8.0, 8.0), 4.0),)), n, 0.2, 300.0, iters, m, 17)
+    ev = synth.make_events(cfg, n, device="cuda")
+    lors = synth.make_sens_lors(cfg, m, device="cuda")
+    g, og = grids(pkg, cfg)
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    sens = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.sensitivity(lors, m, sens)
+    single = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.reconstruct_regions(ev, n, R, None, single, sens, iters)
+    ctx.set_option(pkg.OPT_REGION_OVERLAP, 1)
+    out = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.reconstruct_regions(ev, n, R, None, out, sens, iters)
+    out2 = torch.empty_like(out)
+    ctx.reconstruct_regions(ev, n, R, None, out2, sens, iters)  # second call: cached sub-contexts
+    assert float((out - out2).abs().max()) <= 1e-5 * float(out.max())
+    # oracle pipeline
+    sig = oracle.sigma_mm(300.0)
+    ev_np, sens_np = to_np(ev), sens.cpu().numpy()
+    zb = oracle.region_zbounds(og, R)
+    lo, hi, counts = oracle.region_spans(ev_np, zb, 3.0 * sig)
+    mask = oracle.mask_f32(sens_np)
+    ks = oracle.default_region_slices(nz, R)
+    mg = int(np.ceil((2 * 3.0 * sig + 6.0) / v))
+    total = np.zeros(g.nvox)
+    sl = nx * ny
+    for r in range(R):
+        z0, z1 = max(0, ks[r] - (mg if r > 0 else 0)), min(nz, ks[r + 1] + (mg if r < R - 1 else 0))
+        sg = oracle.make_grid(nx, ny, z1 - z0, v, origin=(og.ox, og.oy, og.oz + z0 * v))
+        sel = (lo <= r) & (r <= hi)
+        sub_ev = {k: a[sel] for k, a in ev_np.items()}
+        x = mask[z0 * sl:z1 * sl].astype(np.float64)
+        for _ in range(iters):
+            corr, _, _ = oracle.em_correction(sg, sig, sub_ev, x)
+            x = oracle.update(x, corr, sens_np[z0 * sl:z1 * sl], mask[z0 * sl:z1 * sl])
+        total[ks[r] * sl:ks[r + 1] * sl] = x[(ks[r] - z0) * sl:(ks[r + 1] - z0) * sl]  # the core only
+    check_image(out.cpu().numpy(), total)
+    # unpinned (PAPER.md:212 "no difference to the whole-body reconstruction", visual only): report both readings
+    x = torch.from_numpy(mask.astype(np.float32)).cuda()
+    ctx.iterate(ev, n, x, sens, iters)
+    d13 = float((single - x).double().norm() / x.double().norm())
+    d27 = float((out - x).double().norm() / x.double().norm())
+    print(f"split-vs-unsplit rel-L2: single assignment (R13) {d13:.3e}, overlapping membership (R27) {d27:.3e}")
+    assert d27 < d13
+
+
 def test_full_size_bench_configuration(pkg):
     """BASELINE.json cfg-3 at FULL size (146 M events, 160x160x640) in the launch configuration bench.py times
     (sub-binned permutation, persistent fused EM pass, update).  The oracle cannot run 146 M events, so:

@@ -385,6 +385,55 @@ def test_p11_region_ids_boundaries_and_counts():
     assert oracle.region_ids(ev, zb)[0].tolist() == [-1]
 
 
+# ---------------------------------------------------------------- P18 (reading R27 / specification F3)
+def test_p18_region_spans_hand_built():
+    """an event "always contributed to 1 or 2 image regions".  Hand-placed LORs whose window's axial extent
+    is known by construction; expected spans typed in."""
+    g = oracle.make_grid(160, 160, 640, 3.75)
+    zb = oracle.region_zbounds(g, 9)  # borders at -720, -480, -240, 0, 240, 480, 720, 960 (cores 480 + 8 x 240 mm)
+    assert zb.tolist() == [-1200.0, -720.0, -480.0, -240.0, 0.0, 240.0, 480.0, 720.0, 960.0, 1200.0]
+    hw = 60.0
+
+    def span(p1, p2, dt=0.0):
+        ev = {"x1": [p1[0]], "y1": [p1[1]], "z1": [p1[2]], "x2": [p2[0]], "y2": [p2[1]], "z2": [p2[2]], "dt": [dt]}
+        lo, hi, counts = oracle.region_spans(ev, zb, hw)
+        assert counts.sum() == (hi[0] - lo[0] + 1 if lo[0] >= 0 else 0)
+        return int(lo[0]), int(hi[0])
+
+    # transverse LOR (dz = 0): the window has no axial extent -> exactly the single-assignment region, also on a border
+    assert span((-400, 0, 100.0), (400, 0, 100.0)) == (4, 4)
+    assert span((-400, 0, 240.0), (400, 0, 240.0)) == (5, 5)
+    # axial LOR (|dz| / L = 1): extent = centre +- 60 mm
+    assert span((0, 0, -1000), (0, 0, 1000)) == (3, 4)            # centre 0: [-60, 60] straddles the border at 0
+    assert span((0, 0, -1000 + 120), (0, 0, 1000 + 120)) == (4, 4)  # centre 120: [60, 180] inside region 4
+    assert span((0, 0, -1000 + 180), (0, 0, 1000 + 180)) == (4, 5)  # centre 180: [120, 240] touches the border at 240 (<=)
+    assert span((0, 0, -1000 + 179), (0, 0, 1000 + 179)) == (4, 4)  # [119, 239]
+    assert span((0, 0, 1000 + 180), (0, 0, -1000 + 180)) == (4, 5)  # reversed LOR: |dz|
+    # 3-4-5 triangle: |dz| / L = 0.6 -> extent = centre +- 36 mm
+    assert span((-400, 0, -300 + 30), (400, 0, 300 + 30)) == (3, 4)  # centre 30: [-6, 66]
+    assert span((-400, 0, -300 + 40), (400, 0, 300 + 40)) == (4, 4)  # centre 40: [4, 76]
+    # dt moves the centre towards end point 2 (R22): c/2 * 400 ps = 59.96 mm along +z
+    assert span((0, 0, -1000), (0, 0, 1000), dt=400.0) == (3, 4)      # centre 59.96: [-0.04, 119.96] still reaches below 0
+    assert span((0, 0, -1000), (0, 0, 1000), dt=401.0) == (4, 4)      # centre 60.11: [0.11, 120.11]
+    assert span((0, 0, -1000), (0, 0, 1000), dt=-401.0) == (3, 3)     # centre -60.11: [-120.11, -0.11]
+    # out of range: clamps to the first / last region; invalid -> (-1, -1)
+    assert span((0, 0, -3000), (0, 0, 0)) == (0, 0)
+    assert span((0, 0, float("nan")), (0, 0, 0)) == (-1, -1)
+    # consistency with the single assignment: lo <= region <= hi, and spans of a dz = 0 set equal the single assignment
+    rng = np.random.default_rng(11)
+    n = 20_000
+    ev = {k: rng.uniform(-400, 400, n).astype(np.float32) for k in ("x1", "y1", "x2", "y2")}
+    ev["z1"] = rng.uniform(-1200, 1200, n).astype(np.float32)
+    ev["z2"] = rng.uniform(-1200, 1200, n).astype(np.float32)
+    ev["dt"] = rng.normal(0, 500, n).astype(np.float32)
+    region, _ = oracle.region_ids(ev, zb)
+    lo, hi, counts = oracle.region_spans(ev, zb, hw)
+    assert np.all(lo <= region) and np.all(region <= hi) and np.all(hi - lo <= 1)
+    assert counts.sum() == n + int((hi > lo).sum())
+    lo0, hi0, _ = oracle.region_spans(ev, zb, 0.0)
+    assert np.array_equal(lo0, region) and np.array_equal(hi0, region)
+
+
 # ---------------------------------------------------------------- P12
 def test_p12_bin_keys_hand_built():
     g = oracle.make_grid(32, 32, 32, 4.0)  # 4x4x4 tiles of 8^3 voxels, T = 64
