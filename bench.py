@@ -710,7 +710,8 @@ def main():
                       "tile_events": int(st.tile_events),
                       "plan": None if plan is None else {"active": int(plan.active), "items": int(plan.n_tile_items),
                                                          "tile_events": int(plan.n_tile_events),
-                                                         "direct_events": int(plan.n_direct_events)}},
+                                                         "direct_events": int(plan.n_direct_events),
+                                                         "stragglers": int(plan.n_stragglers)}},
             "paper_context": "PAPER.md:17,:299 -- 3.5 min for the slowest of nine regions (20 iterations, Tesla C2075 + 16 CPU threads); context, not the target",
         }
         print(json.dumps(line))

@@ -80,6 +80,7 @@ typedef struct {
     uint32_t n_direct_chunks; /* 32-event pieces of the direct pass on records (without the tile items' stragglers) */
     uint64_t n_tile_events;   /* events that run on a tile */
     uint64_t n_direct_events; /* n - n_tile_events */
+    uint64_t n_stragglers;    /* of n_direct_events: valid events of tile items whose window leaves the item's tile */
 } tofmlem_plan;
 
 /* Option keys for tofmlem_set_option. */

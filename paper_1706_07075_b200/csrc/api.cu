@@ -3,6 +3,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -68,6 +69,8 @@ struct tofmlem_ctx {
     TileGeom h_geom_sent;   // what d_geom currently holds (valid when d_geom != nullptr)
     TileItem *d_items = nullptr;
     size_t items_cap = 0;
+    TileRange *d_ranges = nullptr;
+    size_t ranges_cap = 0;
     uint2 *d_chunks = nullptr;
     size_t chunks_cap = 0;
     unsigned *d_plan_flags = nullptr;  // [0] tile work counter, [1] "keys not sorted" flag
@@ -160,6 +163,7 @@ ProjParams make_params(const tofmlem_ctx *c, bool tof) {
     p.variant = c->em_variant;
     p.cache_share = c->cache_share;
     p.brick = 0;
+    p.n_sm = c->n_sm;
     return p;
 }
 
@@ -172,6 +176,13 @@ bool vec_ok(const tofmlem_ctx *c, const float *out) {
 // context's options and the pointer, so tofmlem_em_correction and tofmlem_update agree without further state.
 bool bricks_on(const tofmlem_ctx *c, const float *corr) {
     return c->corr_bricks && c->projector == 0 && (c->grid.nx & 1) == 0 && (c->grid.ny & 1) == 0 && vec_ok(c, corr);
+}
+
+// The brick-order update reads image and sens as float2: both must be 8-byte aligned there (checked by the callers
+// through update_aligned; the layout decision itself depends on corr and the options only).
+bool update_aligned(const tofmlem_ctx *c, const float *image, const float *corr, const float *sens) {
+    return !bricks_on(c, corr) ||
+           (((reinterpret_cast<uintptr_t>(image) | reinterpret_cast<uintptr_t>(sens)) & 7) == 0);
 }
 
 void update_any(const tofmlem_ctx *c, float *image, float *corr, const float *sens, const float *dmax, cudaStream_t s) {
@@ -355,7 +366,7 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         CU(cudaEventRecord(ctx->t_ev[0], s));
         if (ctx->plan.n_items) {
             TileGeom g;
-            build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);  // the same as at plan time (sigma, trunc match)
+            build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, ctx->smem_per_sm, g);  // as at plan time (sigma, trunc match)
             launch_em_tile(p, g, ctx->d_geom, ctx->tile_log2, ctx->d_rec, evw, d_image, d_corr, ctx->d_stats,
                            ctx->d_items, ctx->plan.n_items, ctx->d_plan_flags, n_sm, ctx->smem_per_sm,
                            ctx->tile_check != 0, ctx->sigma, ctx->plan.max_item_events, ctx->d_ev_scale, s);
@@ -506,6 +517,7 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_plan_flags);
     cudaFree(ctx->d_geom);
     cudaFree(ctx->d_items);
+    cudaFree(ctx->d_ranges);
     cudaFree(ctx->d_chunks);
     cudaFree(ctx->d_plan_counters);
     for (auto &te : ctx->t_ev)
@@ -719,6 +731,8 @@ int tofmlem_em_correction(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n
 int tofmlem_update(tofmlem_ctx *ctx, float *d_image, float *d_corr, const float *d_sens) {
     if (!ctx) return TOFMLEM_EINVAL;
     if (!d_image || !d_corr || !d_sens) return fail(ctx, TOFMLEM_EINVAL, "update: NULL argument");
+    if (!update_aligned(ctx, d_image, d_corr, d_sens))
+        return fail(ctx, TOFMLEM_EINVAL, "update: d_image and d_sens must be 8-byte aligned with the brick layout of d_corr");
     launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, ctx->stream);
     CHECK_LAUNCH(1);
     update_any(ctx, d_image, d_corr, d_sens, ctx->d_max, ctx->stream);
@@ -731,6 +745,8 @@ int tofmlem_iterate_weighted(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_
     if (!ctx) return TOFMLEM_EINVAL;
     if ((n && !ev_ok(ev, ctx->tof)) || !d_image || !d_sens || iters < 0 || n > 0xFFFFFFFFull || d_image == d_sens)
         return fail(ctx, TOFMLEM_EINVAL, "iterate: bad argument");
+    if (((reinterpret_cast<uintptr_t>(d_image) | reinterpret_cast<uintptr_t>(d_sens)) & 7) != 0)
+        return fail(ctx, TOFMLEM_EINVAL, "iterate: d_image and d_sens must be 8-byte aligned");
     EventPtrs p = n ? ev_ptrs(ev) : EventPtrs{};
     return iterate_device(ctx, p, n, d_weight, d_image, d_sens, iters, true);
 }
@@ -888,10 +904,11 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
     // direct records carry; a pass into another layout ignores the plan
     p.brick = ctx->corr_bricks && (ctx->grid.nx & 1) == 0 && (ctx->grid.ny & 1) == 0 && (ctx->nvox & 3) == 0 ? 1 : 0;
     TileGeom g;
-    build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, g);
+    build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, ctx->smem_per_sm, g);
     cudaStream_t s = ctx->stream;
     // ---- which bins become tile items?  Needs a list sorted by key (tofmlem_permute_events) and tiles that fit.
     std::vector<TileItem> items;
+    std::vector<TileRange> ranges;
     std::vector<uint2> chunks;
     uint64_t in_items = 0;
     auto add_run = [&](uint64_t lo, uint64_t hi) {
@@ -914,34 +931,72 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaStreamSynchronize(s));
         sorted = flags[1] == 0;
         if (sorted) {
-            // bins with at least tile_min_events events become tile work (pieces of at most tile_max_events, whole
-            // warps); maximal runs of the other bins are cut into 32-event pieces for the direct pass
+            // Tile items: a bin with at least tile_min_events events (pieces of at most tile_max_events, whole warps), or
+            // a PAIR of bins that are neighbours along the class's dominant axis and hold tile_min_events .. tile_max_events
+            // events together (one tile, T planes longer: the per-item cost is shared by more events and bins too sparse
+            // on their own become tile work).  Maximal runs of the other bins are cut into 32-event pieces for the
+            // direct pass.
             const uint32_t thr = (uint32_t)ctx->tile_min_events, mx = (uint32_t)ctx->tile_max_events;
-            uint64_t off = 0, run_lo = 0, run_hi = 0;
+            const int t = 1 << ctx->tile_log2;
+            const uint32_t Tx = (uint32_t)((ctx->grid.nx + t - 1) >> ctx->tile_log2),
+                           Ty = (uint32_t)((ctx->grid.ny + t - 1) >> ctx->tile_log2),
+                           Tz = (uint32_t)((ctx->grid.nz + t - 1) >> ctx->tile_log2), T3 = Tx * Ty * Tz;
+            std::vector<uint64_t> start(nb + 1);
+            uint64_t off = 0;
+            for (uint32_t b = 0; b < nb; ++b) {
+                start[b] = off;
+                off += cnt[b];
+            }
+            start[nb] = off;
+            std::vector<uint8_t> state(nb, 0);  // 0: direct, 1: item (first cube or single), 2: second cube of a pair
             for (uint32_t b = 0; b < nb; ++b) {
                 const uint32_t c = cnt[b];
-                if (c == 0) continue;
-                if (c >= thr) {
-                    if (run_hi > run_lo) add_run(run_lo, run_hi);
-                    run_lo = run_hi = 0;
+                if (c == 0 || state[b]) continue;
+                const uint32_t D = b / T3, tl = b - D * T3, a = D >> 2;
+                const uint32_t step = a == 0 ? 1u : (a == 1 ? Tx : Tx * Ty);
+                const uint32_t ca = a == 0 ? tl % Tx : (a == 1 ? (tl / Tx) % Ty : tl / (Tx * Ty));
+                const uint32_t na = a == 0 ? Tx : (a == 1 ? Ty : Tz);
+                const uint32_t b2 = b + step;
+                const uint32_t c2 = (g.pairs && ca + 1 < na && !state[b2]) ? cnt[b2] : 0u;
+                if (c2 > 0 && c + c2 >= thr && c + c2 <= mx) {
+                    state[b] = 1;
+                    state[b2] = 2;
+                    items.push_back(TileItem{(uint32_t)start[b], c, (uint32_t)start[b2], c2, b, 1u, 0u, 0u});
+                    in_items += c + c2;
+                } else if (c >= thr) {
+                    state[b] = 1;
                     const uint32_t pieces = (c + mx - 1) / mx;
                     uint32_t per = (c + pieces - 1) / pieces;
                     per = (per + 31u) & ~31u;
-                    for (uint32_t a = 0; a < c; a += per)
-                        items.push_back(TileItem{(uint32_t)(off + a), c - a < per ? c - a : per, b, 0u});
+                    for (uint32_t k = 0; k < c; k += per)
+                        items.push_back(TileItem{(uint32_t)(start[b] + k), c - k < per ? c - k : per, 0u, 0u, b, 0u, 0u, 0u});
                     in_items += c;
-                } else {
-                    if (run_hi == run_lo) run_lo = off;
-                    run_hi = off + c;
                 }
-                off += c;
+            }
+            uint64_t run_lo = 0, run_hi = 0;
+            for (uint32_t b = 0; b < nb; ++b) {
+                if (cnt[b] == 0) continue;
+                if (state[b]) {
+                    if (run_hi > run_lo) add_run(run_lo, run_hi);
+                    run_lo = run_hi = 0;
+                } else {
+                    if (run_hi == run_lo) run_lo = start[b];
+                    run_hi = start[b] + cnt[b];
+                }
             }
             if (run_hi > run_lo) add_run(run_lo, run_hi);
             if (off < n) add_run(off, n);  // events with an invalid key (sorted to the end): their records are invalid
+            // the items' event ranges in list order: the record set-up finds the item of an event by bisection
+            for (size_t i = 0; i < items.size(); ++i) {
+                ranges.push_back(TileRange{items[i].start, items[i].count, (uint32_t)i, 0u});
+                if (items[i].count2) ranges.push_back(TileRange{items[i].start2, items[i].count2, (uint32_t)i, 0u});
+            }
+            std::sort(ranges.begin(), ranges.end(), [](const TileRange &x, const TileRange &y) { return x.start < y.start; });
         }
     }
     ctx->plan.sorted = sorted ? 1 : 0;
     if (items.empty()) {  // no tiles (window too wide, unsorted list, sparse bins): the whole list in order
+        ranges.clear();
         chunks.clear();
         add_run(0, n);
         in_items = 0;
@@ -969,6 +1024,13 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMalloc(&ctx->d_items, items.size() * sizeof(TileItem)));
         ctx->items_cap = items.size();
     }
+    if (ctx->ranges_cap < ranges.size()) {
+        cudaFree(ctx->d_ranges);
+        ctx->d_ranges = nullptr;
+        ctx->ranges_cap = 0;
+        CU(cudaMalloc(&ctx->d_ranges, ranges.size() * sizeof(TileRange)));
+        ctx->ranges_cap = ranges.size();
+    }
     if (ctx->chunks_cap < chunks.size()) {
         cudaFree(ctx->d_chunks);
         ctx->d_chunks = nullptr;
@@ -983,12 +1045,13 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
             CU(cudaMemcpyAsync(ctx->d_geom, &ctx->h_geom_sent, sizeof g, cudaMemcpyHostToDevice, s));
         }
         CU(cudaMemcpyAsync(ctx->d_items, items.data(), items.size() * sizeof(TileItem), cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(ctx->d_ranges, ranges.data(), ranges.size() * sizeof(TileRange), cudaMemcpyHostToDevice, s));
     }
     if (!chunks.empty())
         CU(cudaMemcpyAsync(ctx->d_chunks, chunks.data(), chunks.size() * sizeof(uint2), cudaMemcpyHostToDevice, s));
     // ---- the records: fp64 set-up, quantisation, dry run against the tile (prepared.cu)
     launch_prepare_rays(p, ctx->sigma, items.empty() ? nullptr : ctx->d_geom, ctx->tile_log2, ev_ptrs(ev), n, ctx->d_items,
-                        (uint32_t)items.size(), ctx->d_rec, ctx->d_strag, ctx->d_plan_counters, s);
+                        ctx->d_ranges, (uint32_t)ranges.size(), ctx->d_rec, ctx->d_strag, ctx->d_plan_counters, s);
     CHECK_LAUNCH(1);
     std::vector<unsigned char> hc(plan_counter_bytes());
     CU(cudaMemcpyAsync(hc.data(), ctx->d_plan_counters, hc.size(), cudaMemcpyDeviceToHost, s));
@@ -1005,7 +1068,7 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
     ctx->plan.n_items = (uint32_t)items.size();
     ctx->plan.max_item_events = 0;
     for (const TileItem &it : items)
-        if (it.count > ctx->plan.max_item_events) ctx->plan.max_item_events = it.count;
+        if (it.count + it.count2 > ctx->plan.max_item_events) ctx->plan.max_item_events = it.count + it.count2;
     ctx->plan.n_chunks = (uint32_t)chunks.size();
     ctx->plan.n_strag = (uint32_t)cnt4[2];
     ctx->plan.valid_events = cnt4[0];
@@ -1023,6 +1086,7 @@ int tofmlem_plan_info(const tofmlem_ctx *ctx, tofmlem_plan *h_out) {
     h_out->n_direct_chunks = ctx->plan.n_chunks;
     h_out->n_tile_events = ctx->plan.tile_events;
     h_out->n_direct_events = ctx->plan.direct_events;
+    h_out->n_stragglers = ctx->plan.n_strag;
     return TOFMLEM_OK;
 }
 

@@ -25,6 +25,7 @@ struct ProjParams {
     int variant;           // fused EM pass: 0 = persistent per-SM queues (default), 1 = grid order, 2 = smem cache
     int cache_share;       // variant 2: warps (of every 8) that reduce through the shared-memory cache
     int brick;             // fused EM pass: the correction image is in the 2x2x1 brick layout (needs even nx, ny)
+    int n_sm;              // SM count of the context's device (persistent kernels: one work queue per SM)
 };
 
 struct EventPtrs {
@@ -74,20 +75,32 @@ constexpr int kTileMaxPlanes = 96;
 // stored plane by plane along a: plane p (p = i_a - cube origin + RA) holds a W[0] x W[1] rectangle of the two lateral
 // axes (fast axis f = the lower-numbered one, slow axis s) whose low corner, in cell coordinates mirrored so that the
 // class's rays run towards +f and +s, is (lo[0][p], lo[1][p]).
+// Two variants: [0] the item is one cube, [1] the item is a PAIR of cubes that are neighbours along a (the tile is T
+// planes longer, the lateral rectangles are the same): fewer, larger items -- the per-item cost (tile load, flush,
+// barriers) is shared by twice the events, and bins too sparse on their own become tile work.
 struct TileGeom {
     int T;                 // cube edge in voxels
     int ok;                // tile mode is available for this context (all three dominant axes fit)
-    int RA[3], PA[3];      // planes below the cube / planes in all, per dominant axis
-    int W[3][2];           // rectangle width along f and s
-    int PS[3];             // words per plane (odd, >= W[0] * W[1])
-    int words;             // words of the largest tile: max PA * PS
-    signed char lo[3][2][kTileMaxPlanes];
+    int pairs;             // variant [1] may be used (it fits without lowering the number of CTAs per SM)
+    int RA[3];             // planes below the first cube, per dominant axis
+    int PA[2][3];          // planes in all
+    int W[2][3][2];        // rectangle width along f and s
+    int PS[2][3];          // words per plane (odd, >= W[0] * W[1])
+    int words;             // words of the largest tile in use: max PA * PS
+    signed char lo[2][3][2][kTileMaxPlanes];
 };
 struct TileItem {
-    uint32_t start, count, key, pad;  // events [start, start + count) of the sorted list, all with this key
+    uint32_t start, count;    // events [start, start + count) of the sorted list: the item's (first) cube, key `key`
+    uint32_t start2, count2;  // pair items: the events of the second cube (key + one step along a), else count2 = 0
+    uint32_t key, variant, pad0, pad1;
+};
+// A contiguous run of events of the sorted list that belongs to a tile item (the plan's event -> item look-up).
+struct TileRange {
+    uint32_t start, count, item, pad;
 };
 // false (g.ok = 0) when a tile pair does not fit in `smem_budget` bytes of shared memory
-void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, TileGeom &g);
+void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, size_t smem_per_sm, TileGeom &g);
+int tile_ctas_per_sm(size_t tile_bytes, size_t smem_per_sm);
 size_t tile_smem_bytes(const TileGeom &g);
 // d_geom: the same structure in device memory; rec: the ray records of the planned list (prepared.cuh)
 void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const RecPtrs &rec,
@@ -103,7 +116,8 @@ void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_ge
 // (plan_counter_bytes() bytes of device memory; read_plan_counters: valid events, tile events, stragglers, visits).
 size_t plan_counter_bytes();
 void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom /* NULL: no tiles */, int tile_log2,
-                         const EventPtrs &ev, uint64_t n, const TileItem *items, uint32_t n_items, const RecPtrs &rec,
+                         const EventPtrs &ev, uint64_t n, const TileItem *items, const TileRange *ranges,
+                         uint32_t n_ranges, const RecPtrs &rec,
                          uint32_t *stragglers, void *d_counters, cudaStream_t s);
 void read_plan_counters(const void *h_counters, uint64_t out[4]);
 // ev: the raw events of the planned list (the kRecTiny records are walked from them)

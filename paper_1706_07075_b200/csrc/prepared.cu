@@ -112,23 +112,24 @@ __device__ __forceinline__ int sel3i(int a, int v0, int v1, int v2) { return a =
 
 __global__ void __launch_bounds__(kBlock)
 prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, EventPtrs ev, uint64_t n,
-                    const TileItem *__restrict__ items, unsigned n_items, double qs, double qi, RecPtrs rec,
-                    uint32_t *__restrict__ stragglers, PlanCounters *__restrict__ counters) {
+                    const TileItem *__restrict__ items, const TileRange *__restrict__ ranges, unsigned n_ranges,
+                    double qs, double qi, RecPtrs rec, uint32_t *__restrict__ stragglers,
+                    PlanCounters *__restrict__ counters) {
     const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
     const unsigned lane = threadIdx.x & 31u;
     bool valid = false, tile = false, straggler = false;
     unsigned visits = 0;
     if (e < n) {
-        // the tile item that holds this event, if any (items are sorted by their first event)
+        // the tile item that holds this event, if any (the items' event ranges, sorted by their first event)
         int item = -1;
-        if (n_items) {
-            unsigned lo = 0, hi = n_items;  // largest i with items[i].start <= e
+        if (n_ranges) {
+            unsigned lo = 0, hi = n_ranges;  // largest i with ranges[i].start <= e
             while (hi - lo > 1) {
                 const unsigned mid = (lo + hi) >> 1;
-                if ((uint64_t)__ldg(&items[mid].start) <= e) lo = mid; else hi = mid;
+                if ((uint64_t)__ldg(&ranges[mid].start) <= e) lo = mid; else hi = mid;
             }
-            const uint64_t st = __ldg(&items[lo].start);
-            if (st <= e && e < st + __ldg(&items[lo].count)) item = (int)lo;
+            const uint64_t st = __ldg(&ranges[lo].start);
+            if (st <= e && e < st + __ldg(&ranges[lo].count)) item = (int)__ldg(&ranges[lo].item);
         }
         Geo g;
         QRay r;
@@ -144,7 +145,8 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
             if (item >= 0 && tiny) straggler = true;
             if (item >= 0 && !tiny) {
                 // ---- does the window stay inside the bin's tile?  Dry run of the tile walk, every voxel checked.
-                const unsigned key = __ldg(&items[item].key);
+                const unsigned key = __ldg(&items[item].key);  // the item's FIRST cube: the tile's origin
+                const int var = (int)__ldg(&items[item].variant);
                 const int T = Gp->T;
                 const unsigned Tx = (unsigned)((nx + T - 1) >> tile_log2), Ty = (unsigned)((ny + T - 1) >> tile_log2),
                                Tz = (unsigned)((P.n[2] + T - 1) >> tile_log2);
@@ -153,8 +155,9 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
                 const int sg1 = (D & 2u) ? -1 : 1, sg2 = (D & 1u) ? -1 : 1;  // signs of axes (a+1)%3 and (a+2)%3
                 const int sgf = a == 1 ? sg2 : sg1, sgs = a == 1 ? sg1 : sg2;
                 const int c0[3] = {(int)(tl % Tx) * T, (int)((tl / Tx) % Ty) * T, (int)(tl / (Tx * Ty)) * T};
-                const int RA = Gp->RA[a], PA = Gp->PA[a], Wf = Gp->W[a][0], Ws = Gp->W[a][1], PS = Gp->PS[a];
-                const signed char *lof = Gp->lo[a][0], *los = Gp->lo[a][1];
+                const int RA = Gp->RA[a], PA = Gp->PA[var][a], Wf = Gp->W[var][a][0], Ws = Gp->W[var][a][1],
+                          PS = Gp->PS[var][a];
+                const signed char *lof = Gp->lo[var][a][0], *los = Gp->lo[var][a][1];
                 int p = sel3i(a, g.i[0], g.i[1], g.i[2]) - sel3i(a, c0[0], c0[1], c0[2]) + RA;
                 const int rf = sel3i(f, g.i[0], g.i[1], g.i[2]) - sel3i(f, c0[0], c0[1], c0[2]);
                 const int rs = sel3i(s, g.i[0], g.i[1], g.i[2]) - sel3i(s, c0[0], c0[1], c0[2]);
@@ -514,14 +517,14 @@ void plan_quantum(const ProjParams &p, double sigma, double &kappa, double &qs, 
 size_t plan_counter_bytes() { return sizeof(PlanCounters); }
 
 void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom, int tile_log2, const EventPtrs &ev,
-                         uint64_t n, const TileItem *items, uint32_t n_items, const RecPtrs &rec, uint32_t *stragglers,
-                         void *d_counters, cudaStream_t s) {
+                         uint64_t n, const TileItem *items, const TileRange *ranges, uint32_t n_ranges,
+                         const RecPtrs &rec, uint32_t *stragglers, void *d_counters, cudaStream_t s) {
     if (n == 0) return;
     double kappa, qs, qi;
     plan_quantum(p, sigma, kappa, qs, qi);
     cudaMemsetAsync(d_counters, 0, sizeof(PlanCounters), s);
     prepare_rays_kernel<<<(unsigned)((n + kBlock - 1) / kBlock), kBlock, 0, s>>>(
-        p, d_geom, tile_log2, ev, n, items, d_geom ? n_items : 0u, qs, qi, rec, stragglers,
+        p, d_geom, tile_log2, ev, n, items, ranges, d_geom ? n_ranges : 0u, qs, qi, rec, stragglers,
         static_cast<PlanCounters *>(d_counters));
 }
 

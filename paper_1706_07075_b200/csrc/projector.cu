@@ -27,7 +27,6 @@
 namespace tofmlem {
 
 constexpr int kBlock = 256;
-constexpr int kMaxDevices = 64;
 
 template <bool TOF>
 __device__ __forceinline__ bool load_and_setup(const ProjParams &P, const EventPtrs &ev, uint64_t e, Ray &r) {
@@ -269,9 +268,11 @@ template <bool TOF, bool BRICK>
 static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
                              float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s) {
     const size_t smem = sizeof(unsigned long long) << kCacheLog2;
-    int dev = 0, n_sm = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    int dev = 0, n_sm = p.n_sm;
+    if (n_sm < 1) {
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
     cudaFuncSetAttribute(em_cached_kernel<TOF, BRICK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     unsigned nseg = (unsigned)n_sm;
     if (nseg > (unsigned)kMaxQueues) nseg = kMaxQueues;
@@ -320,17 +321,15 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
                       float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s, const uint2 *chunks = nullptr,
                       uint32_t n_chunks = 0) {
     if ((p.variant != 1 || chunks) && queues) {
-        // SM count and resident CTAs per SM of THIS instantiation on the CURRENT device (cached per device; a race on
-        // the first use only writes the same values twice)
-        static int sm_of[kMaxDevices] = {0}, per_of[kMaxDevices] = {0};
-        int dev = 0;
-        cudaGetDevice(&dev);
-        const int slot = dev < kMaxDevices ? dev : kMaxDevices - 1;
-        if (!sm_of[slot] || dev >= kMaxDevices) {
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_of[slot], em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
-            cudaDeviceGetAttribute(&sm_of[slot], cudaDevAttrMultiProcessorCount, dev);
+        // SM count of the context's device (queried in tofmlem_create) and resident CTAs per SM of THIS instantiation on
+        // the current device (a host-side table look-up in the runtime: asked on every launch, no cached state)
+        int per_sm = 0, n_sm = p.n_sm;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_persistent_kernel<TOF, VEC, BRICK>, kBlock, 0);
+        if (n_sm < 1) {
+            int dev = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
         }
-        const int n_sm = sm_of[slot], per_sm = per_of[slot];
         // Short windows: the warps of an SM spread over several list segments (measured at 146 M events: 300 ps, 1 / 2 /
         // 3 / 4 / 8 segments per SM -> 21.47 / 21.04 / 20.75 / 22.25 / 23.54 ms; 100 ps, 1 / 2 / 3 / 4 -> 11.35 / 9.57 /
         // 9.44 / 9.32 ms).  Long walks (600 ps: 43.3 -> 45.1 ms, non-TOF: 203 -> 218 ms with 2) keep one.

@@ -278,15 +278,13 @@ void launch_sampled_em(const ProjParams &p, const SampleLutEntry *lut, int K, co
                        const float *evw, const float *image, float *corr, DeviceStats *stats, unsigned *queues,
                        cudaStream_t s) {
     if (!n) return;
-    static int sm_of[64] = {0}, per_of[64] = {0};  // per device (the first use on a device fills its slot)
-    int dev = 0;
-    cudaGetDevice(&dev);
-    const int slot = dev < 64 ? dev : 63;
-    if (!sm_of[slot] || dev >= 64) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_of[slot], sampled_em_kernel, kBlock, 0);
-        cudaDeviceGetAttribute(&sm_of[slot], cudaDevAttrMultiProcessorCount, dev);
+    int per_sm = 0, n_sm = p.n_sm;  // the context's device (tofmlem_create); occupancy asked per launch, no cached state
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sampled_em_kernel, kBlock, 0);
+    if (n_sm < 1) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     }
-    const int n_sm = sm_of[slot], per_sm = per_of[slot];
     constexpr unsigned kSegsPerSm = 2;  // measured 1 / 2 / 3 / 4: 27.8 / 24.1 / 24.3 / 24.6 ms at K = 32's persistent pass for short windows
     unsigned nseg = (unsigned)n_sm * kSegsPerSm;
     if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / kSegsPerSm * kSegsPerSm;

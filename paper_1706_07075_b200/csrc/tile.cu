@@ -40,50 +40,77 @@ size_t tile_smem_bytes(const TileGeom &g) {
     return ((size_t)g.words + 4 * (kTileMaxPlanes + 1) + 8 + 256) * sizeof(float);
 }
 
-void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, TileGeom &g) {
+#ifndef TOFMLEM_TILE_SLACK
+#define TOFMLEM_TILE_SLACK 0
+#endif
+constexpr int kSlack = TOFMLEM_TILE_SLACK;  // voxels of slack around the closed-form envelopes (the plan's dry run decides
+                                            // per event anyway; slack only trades tile size against stragglers)
+
+// CTAs per SM by shared memory (1 KB per CTA is reserved by the system), at most 4 (launch_em_tile's configurations)
+int tile_ctas_per_sm(size_t tile_bytes, size_t smem_per_sm) {
+    const size_t per_sm = smem_per_sm ? smem_per_sm : 233472;
+    const int n = (int)(per_sm / (tile_bytes + 1024));
+    return n > 4 ? 4 : n;
+}
+
+void build_tile_geom(const ProjParams &p, int tile_log2, size_t smem_budget, size_t smem_per_sm, TileGeom &g) {
     memset(&g, 0, sizeof g);
     const int T = 1 << tile_log2;
     g.T = T;
     const double hw = p.half_window;
     if (!(hw > 0.0)) return;
-    int words = 0;
-    for (int a = 0; a < 3; ++a) {
-        const int lat[2] = {a == 0 ? 1 : 0, a == 2 ? 1 : 2};  // f, s
-        const int RA = (int)ceil(hw / p.v[a]) + 1;
-        const int PA = 2 * RA + T;
-        if (PA > kTileMaxPlanes) return;
-        g.RA[a] = RA;
-        g.PA[a] = PA;
-        for (int j = 0; j < 2; ++j) {
-            const int b = lat[j];
-            const double rho = p.v[a] / p.v[b];                   // largest slope d(voxel b) / d(voxel a) in the class
-            const int M = (int)ceil(hw / (sqrt(2.0) * p.v[b]));   // largest lateral excursion: |u_b| <= |u_a| => <= 1/sqrt 2
-            int W = 0;
-            for (int pl = 0; pl < PA; ++pl) {
-                const int pa = pl - RA;  // plane index relative to the cube
-                const int below = (int)ceil(rho * (double)(T - pa));
-                const int above = (int)ceil(rho * (double)(pa + 1));
-                const int lo = pa < T ? -(M < below ? M : below) - 1 : -1;
-                const int hi = pa >= 0 ? (T - 1) + (M < above ? M : above) + 1 : T;
-                if (lo < -127) return;
-                g.lo[a][j][pl] = (signed char)lo;
-                if (hi - lo + 1 > W) W = hi - lo + 1;
+    int words[2] = {0, 0};
+    bool fits[2] = {true, true};
+    for (int v = 0; v < 2; ++v) {
+        const int Ta = (v + 1) * T;  // extent of the item along a
+        for (int a = 0; a < 3; ++a) {
+            const int lat[2] = {a == 0 ? 1 : 0, a == 2 ? 1 : 2};  // f, s
+            const int RA = (int)ceil(hw / p.v[a]) + kSlack;
+            const int PA = 2 * RA + Ta;
+            if (PA > kTileMaxPlanes) { fits[v] = false; break; }
+            g.RA[a] = RA;
+            g.PA[v][a] = PA;
+            for (int j = 0; j < 2 && fits[v]; ++j) {
+                const int b = lat[j];
+                const double rho = p.v[a] / p.v[b];                   // largest slope d(voxel b) / d(voxel a) in the class
+                const int M = (int)ceil(hw / (sqrt(2.0) * p.v[b]));   // largest lateral excursion: |u_b| <= |u_a| => <= 1/sqrt 2
+                int W = 0;
+                for (int pl = 0; pl < PA; ++pl) {
+                    const int pa = pl - RA;  // plane index relative to the (first) cube
+                    const int below = (int)ceil(rho * (double)(Ta - pa));
+                    const int above = (int)ceil(rho * (double)(pa + 1));
+                    const int lo = pa < Ta ? -(M < below ? M : below) - kSlack : -kSlack;
+                    const int hi = pa >= 0 ? (T - 1) + (M < above ? M : above) + kSlack : T - 1 + kSlack;
+                    if (lo < -127) { fits[v] = false; break; }
+                    g.lo[v][a][j][pl] = (signed char)lo;
+                    if (hi - lo + 1 > W) W = hi - lo + 1;
+                }
+                g.W[v][a][j] = W;
             }
-            g.W[a][j] = W;
+            if (!fits[v]) break;
+            int ps = g.W[v][a][0] * g.W[v][a][1];
+            if (!(ps & 1)) ++ps;  // odd plane stride: lanes that differ in the plane only hit different banks
+            g.PS[v][a] = ps;
+            if (PA * ps > words[v]) words[v] = PA * ps;
         }
-        int ps = g.W[a][0] * g.W[a][1];
-        if (!(ps & 1)) ++ps;  // odd plane stride: lanes that differ in the plane only hit different banks
-        g.PS[a] = ps;
-        if (PA * ps > words) words = PA * ps;
     }
-    g.words = words;
-    g.ok = tile_smem_bytes(g) <= smem_budget ? 1 : 0;
+    if (!fits[0]) return;
+    g.words = words[0];
+    // at least two items per SM must fit: with one tile per SM its barriers, load and flush are not overlapped by
+    // anything (measured at cfg-2, 222 KB tiles: 2.50 ms per pass against 2.02 ms for the direct pass on records)
+    g.ok = tile_smem_bytes(g) <= smem_budget && tile_ctas_per_sm(tile_smem_bytes(g), smem_per_sm) >= 2 ? 1 : 0;
+    if (g.ok && fits[1]) {
+        TileGeom h = g;
+        h.words = words[1] > words[0] ? words[1] : words[0];
+        if (tile_smem_bytes(h) <= smem_budget &&
+            tile_ctas_per_sm(tile_smem_bytes(h), smem_per_sm) == tile_ctas_per_sm(tile_smem_bytes(g), smem_per_sm)) {
+            g.pairs = 1;
+            g.words = h.words;
+        }
+    }
 }
 
 __device__ __forceinline__ int sel3(int a, int v0, int v1, int v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
-__device__ __forceinline__ float sel3(int a, float v0, float v1, float v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
-__device__ __forceinline__ double sel3(int a, double v0, double v1, double v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
-
 
 // Geometry of the bin a CTA is working on (uniform over the CTA).
 struct Residency {
@@ -248,6 +275,8 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
         const unsigned it = ctl[0];
         if (it >= n_items) break;
         const TileItem item = items[it];
+        const int var = (int)item.variant;
+        const unsigned n_ev = item.count + item.count2;  // a pair item: the second cube's events follow the first's
         Residency R;
         {
             const unsigned D = item.key / T3, tl = item.key - D * T3;
@@ -261,22 +290,22 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
             R.cf = R.a == 0 ? c0y : c0x;
             R.cs = R.a == 2 ? c0y : c0z;
             R.RA = Gp->RA[R.a];
-            R.PA = Gp->PA[R.a];
-            R.Wf = Gp->W[R.a][0];
-            R.Ws = Gp->W[R.a][1];
-            R.PS = Gp->PS[R.a];
+            R.PA = Gp->PA[var][R.a];
+            R.Wf = Gp->W[var][R.a][0];
+            R.Ws = Gp->W[var][R.a][1];
+            R.PS = Gp->PS[var][R.a];
             R.T = T;
         }
         for (unsigned i = tid; i < 256u; i += NT) hist[i] = 0u;
         for (int p = (int)tid; p <= kTileMaxPlanes; p += NT) {
             int l0 = 0, l1 = 0, u = 0, d = 0;
             if (p < R.PA) {
-                l0 = Gp->lo[R.a][0][p];
-                l1 = Gp->lo[R.a][1][p];
+                l0 = Gp->lo[var][R.a][0][p];
+                l1 = Gp->lo[var][R.a][1][p];
                 if (p + 1 < R.PA)
-                    u = 4 * (R.PS - ((int)Gp->lo[R.a][0][p + 1] - l0) - R.Wf * ((int)Gp->lo[R.a][1][p + 1] - l1));
+                    u = 4 * (R.PS - ((int)Gp->lo[var][R.a][0][p + 1] - l0) - R.Wf * ((int)Gp->lo[var][R.a][1][p + 1] - l1));
                 if (p > 0)
-                    d = -4 * (R.PS - (l0 - (int)Gp->lo[R.a][0][p - 1]) - R.Wf * (l1 - (int)Gp->lo[R.a][1][p - 1]));
+                    d = -4 * (R.PS - (l0 - (int)Gp->lo[var][R.a][0][p - 1]) - R.Wf * (l1 - (int)Gp->lo[var][R.a][1][p - 1]));
             }
             lof[p] = l0;
             los[p] = l1;
@@ -284,13 +313,19 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
             dn[p] = d;
         }
         __syncthreads();
+        // image values of the tile: asynchronous 4-byte copies global -> shared (LDGSTS), all in flight at once
         for_each_tile_voxel<NT>(
             R, lof, los, nx, ny, nz,
-            [&](int ti, int x, int y, int z) { tile[ti] = __ldg(image + ((size_t)(z * ny + y) * nx + x)); },
+            [&](int ti, int x, int y, int z) {
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(tile_addr + 4u * (unsigned)ti),
+                             "l"(image + ((size_t)(z * ny + y) * nx + x))
+                             : "memory");
+            },
             [&](int ti) { tile[ti] = 0.0f; });
+        asm volatile("cp.async.wait_all;" ::: "memory");
         __syncthreads();
 
-        const unsigned nchunk = (item.count + 31u) >> 5;
+        const unsigned nchunk = (n_ev + 31u) >> 5;
         const int Wf = R.Wf;
         const unsigned tile_bytes = (unsigned)(R.PA * R.PS) * 4u;
         // ---- phase A: forward values from the image tile, 32 events per warp at a time
@@ -300,8 +335,8 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
             c = __shfl_sync(0xffffffffu, c, 0);
             if (c >= nchunk) break;
             const unsigned k = c * 32u + lane;
-            if (k >= item.count) continue;
-            const uint64_t e = (uint64_t)item.start + k;
+            if (k >= n_ev) continue;
+            const uint64_t e = k < item.count ? (uint64_t)item.start + k : (uint64_t)item.start2 + (k - item.count);
             const uint4 rc = __ldg(rec.c + e);
             float scale = 0.f;
             if ((rc.y & (kRecValid | kRecTile)) == (kRecValid | kRecTile)) {  // the others (stragglers): direct pass
@@ -400,8 +435,8 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
             c = __shfl_sync(0xffffffffu, c, 0);
             if (c >= nchunk) break;
             const unsigned k = c * 32u + lane;
-            if (k >= item.count) continue;
-            const uint64_t e = (uint64_t)item.start + k;
+            if (k >= n_ev) continue;
+            const uint64_t e = k < item.count ? (uint64_t)item.start + k : (uint64_t)item.start2 + (k - item.count);
             const float scale = ev_scale[e];
             if (!(scale > 0.0f)) continue;
             const uint4 rc = __ldg(rec.c + e);
@@ -523,13 +558,11 @@ void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_ge
     const size_t smem = tile_smem_bytes(g);
     const TileLaunch L{p, d_geom, smem, tile_log2, rec, evw, image, corr, stats, items, n_items, counter, n_sm, fx,
                        ev_scale, s};
-    // CTAs per SM by shared memory (1 KB per CTA is reserved by the system); threads so that 56 registers fit
-    const size_t per_sm = smem_per_sm ? smem_per_sm : 233472;
-    const int ncta = (int)(per_sm / (smem + 1024));
+    // CTAs per SM by shared memory; threads so that 56 registers fit
+    const int ncta = tile_ctas_per_sm(smem, smem_per_sm);
     if (ncta >= 4) launch_tile_cfg<256, 4>(L, check);
     else if (ncta == 3) launch_tile_cfg<384, 3>(L, check);
-    else if (ncta == 2) launch_tile_cfg<512, 2>(L, check);
-    else launch_tile_cfg<1024, 1>(L, check);
+    else launch_tile_cfg<512, 2>(L, check);  // build_tile_geom admits no tile that fits only once per SM
 }
 
 }  // namespace tofmlem

@@ -71,7 +71,8 @@ class Stats(C.Structure):
 
 class Plan(C.Structure):
     _fields_ = [("active", C.c_int32), ("sorted", C.c_int32), ("n_tile_items", C.c_uint32),
-                ("n_direct_chunks", C.c_uint32), ("n_tile_events", C.c_uint64), ("n_direct_events", C.c_uint64)]
+                ("n_direct_chunks", C.c_uint32), ("n_tile_events", C.c_uint64), ("n_direct_events", C.c_uint64),
+                ("n_stragglers", C.c_uint64)]
 
 
 class TofMlemError(RuntimeError):

@@ -31,7 +31,7 @@ def test_struct_layouts_match_header():
 
     assert ctypes.sizeof(pkg.Grid) == 36 and ctypes.sizeof(pkg.Scanner) == 8
     assert ctypes.sizeof(pkg.Events) == 7 * ctypes.sizeof(ctypes.c_void_p)
-    assert ctypes.sizeof(pkg.Stats) == 64 and ctypes.sizeof(pkg.Plan) == 32
+    assert ctypes.sizeof(pkg.Stats) == 64 and ctypes.sizeof(pkg.Plan) == 40
 
 
 def test_argument_errors_without_gpu():

@@ -254,6 +254,18 @@ def test_tile_mode_parity_tiny(pkg):
     assert not ctx.plan_info().active
 
 
+@pytest.mark.parametrize("voxel_mm,fwhm,ctas", [(4.0, 100.0, 4), (4.0, 300.0, 3), (3.0, 300.0, 2)])
+def test_tile_mode_launch_configurations(pkg, voxel_mm, fwhm, ctas):
+    """The tile kernel's three launch configurations (4 x 256, 3 x 384, 2 x 512 threads per SM, chosen by the tile's size;
+    at 100 ps also the items made of a PAIR of cubes) vs oracle.mlem on the cfg-1 phantom, tile accesses bounds-tested."""
+    base = synth.TINY
+    cfg = synth.Config(f"tiny-{voxel_mm}-{fwhm}", 32, 32, 32, voxel_mm, base.radius_mm, base.axial_mm, base.phantom, 150_000,
+                       0.1, fwhm, 2, 400_000, 31)
+    ctx, plan, st, sev, x, sens = _tile_case(pkg, cfg, cfg.n_events, cfg.sens_lors, 48)
+    assert plan.n_tile_items > 0 and st.tile_events > 0.5 * st.n_valid, (plan.n_tile_items, st.tile_events, st.n_valid)
+    print(f"voxel {voxel_mm} mm, {fwhm} ps ({ctas} CTAs per SM): {plan.n_tile_items} items, {st.tile_events} of {st.n_valid} on tiles")
+
+
 def test_tile_mode_anisotropic_voxels_and_weights(pkg):
     """Tile envelopes with three different voxel sizes (the lateral slopes v_a / v_b differ per class), a grid that is not
     a multiple of the 8-voxel cube, events with per-event weights."""
@@ -289,13 +301,14 @@ def test_tile_mode_anisotropic_voxels_and_weights(pkg):
 
 
 def test_plan_without_tiles_when_they_do_not_fit(pkg):
-    """cfg-2 (2 mm voxels: the +-3 sigma window spans 57 voxels, a tile pair would need > 227 KB): the plan holds ray
-    records but no tile items, and the pass is the direct one on records."""
+    """cfg-2 geometry at 600 ps (2 mm voxels: the +-3 sigma window spans 115 voxels, a tile would need far more than
+    227 KB): the plan holds ray records but no tile items, and the pass is the direct one on records."""
     cfg = synth.MID
     g, og = grids(pkg, cfg)
     n = 100_000
+    fwhm = 600.0
     ev = synth.make_events(cfg, n, device="cuda")
-    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
     sev, _ = binned(ctx, ev, n)
     ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 8)
     plan = ctx.plan_events(sev, n)
@@ -305,7 +318,7 @@ def test_plan_without_tiles_when_they_do_not_fit(pkg):
     ctx.set_option(pkg.OPT_CORR_BRICKS, 0)  # a plain image; the plan was made for bricks, so this pass ignores it ...
     ctx.reset_stats()
     ctx.em_correction(sev, n, img, corr)
-    ref, nv, vis = oracle.em_correction(og, oracle.sigma_mm(cfg.tof_fwhm_ps), to_np(sev), img.cpu().numpy().astype(np.float64))
+    ref, nv, vis = oracle.em_correction(og, oracle.sigma_mm(fwhm), to_np(sev), img.cpu().numpy().astype(np.float64))
     assert ctx.get_stats().n_valid == nv and abs(int(ctx.get_stats().visits) - int(vis)) <= 1e-5 * vis
     check_image(corr.cpu().numpy(), ref, l2=1e-5, mx=1e-3, zero_tol=1e-6)
     ctx.plan_events(sev, n)  # ... and this one, planned for the plain layout, runs on the records
