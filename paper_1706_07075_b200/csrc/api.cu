@@ -78,6 +78,7 @@ struct tofmlem_ctx {
     size_t rec_cap = 0;
     uint32_t *d_strag = nullptr;       // events of tile items that do not fit their tile
     size_t strag_cap = 0;
+    uint2 *d_tiny = nullptr;           // one-event pieces of the kRecTiny events (kTinyCap entries)
     float *d_ev_scale = nullptr;       // w_e / fwd_e of the tile events between the two phases of tile.cu (rec_cap floats)
     size_t smem_per_sm = 0;
     void *d_plan_counters = nullptr;
@@ -102,7 +103,7 @@ struct tofmlem_ctx {
         int tile_log2 = 0;          // ... this cube size, for a context with
         double sigma = 0.0, trunc = 0.0;  // ... this TOF kernel
         int brick = 0;              // ... and this layout of the correction image
-        uint32_t n_items = 0, n_chunks = 0, n_strag = 0, max_item_events = 0;
+        uint32_t n_items = 0, n_chunks = 0, n_strag = 0, n_tiny = 0, max_item_events = 0;
         uint64_t tile_events = 0, direct_events = 0, valid_events = 0, visits = 0;
         int sorted = 0;
     } plan;
@@ -110,6 +111,8 @@ struct tofmlem_ctx {
 };
 
 namespace {
+
+constexpr uint32_t kTinyCap = 1u << 20;  // kRecTiny events a plan can hold (more: the list is not planned at all)
 
 int fail(tofmlem_ctx *c, int code, const char *what) {
     if (c) c->err = what ? what : "";
@@ -264,6 +267,8 @@ void free_records(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_rec.c);
     cudaFree(ctx->d_strag);
     cudaFree(ctx->d_ev_scale);
+    cudaFree(ctx->d_tiny);
+    ctx->d_tiny = nullptr;
     ctx->d_rec = RecPtrs{nullptr, nullptr, nullptr};
     ctx->d_strag = nullptr;
     ctx->d_ev_scale = nullptr;
@@ -374,14 +379,19 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         }
         CU(cudaEventRecord(ctx->t_ev[1], s));
         if (ctx->plan.n_chunks) {
-            launch_em_planned(p, ev, ctx->d_rec, ctx->d_chunks, nullptr, ctx->plan.n_chunks, 0, evw, d_image, d_corr, vec,
+            launch_em_planned(p, ctx->d_rec, ctx->d_chunks, nullptr, ctx->plan.n_chunks, 0, evw, d_image, d_corr, vec,
                               ctx->d_stats, ctx->d_queues, n_sm, s);
             CHECK_LAUNCH(1);
         }
         CU(cudaEventRecord(ctx->t_ev[2], s));
         if (ctx->plan.n_strag) {
-            launch_em_planned(p, ev, ctx->d_rec, nullptr, ctx->d_strag, (ctx->plan.n_strag + 31u) / 32u, ctx->plan.n_strag,
+            launch_em_planned(p, ctx->d_rec, nullptr, ctx->d_strag, (ctx->plan.n_strag + 31u) / 32u, ctx->plan.n_strag,
                               evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, n_sm, s);
+            CHECK_LAUNCH(1);
+        }
+        if (ctx->plan.n_tiny) {  // kRecTiny: the unplanned walk (fp64 set-up), one event per piece
+            launch_em_correction_chunks(p, true, ev, n, ctx->d_tiny, ctx->plan.n_tiny, evw, d_image, d_corr, vec,
+                                        ctx->d_stats, ctx->d_queues, s);
             CHECK_LAUNCH(1);
         }
         CU(cudaEventRecord(ctx->t_ev[3], s));
@@ -1008,6 +1018,7 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMalloc(&ctx->d_rec.b, n * sizeof(float4)));
         CU(cudaMalloc(&ctx->d_rec.c, n * sizeof(uint4)));
         CU(cudaMalloc(&ctx->d_ev_scale, n * sizeof(float)));
+        CU(cudaMalloc(&ctx->d_tiny, kTinyCap * sizeof(uint2)));
         ctx->rec_cap = n;
     }
     if (ctx->strag_cap < in_items) {
@@ -1051,13 +1062,16 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMemcpyAsync(ctx->d_chunks, chunks.data(), chunks.size() * sizeof(uint2), cudaMemcpyHostToDevice, s));
     // ---- the records: fp64 set-up, quantisation, dry run against the tile (prepared.cu)
     launch_prepare_rays(p, ctx->sigma, items.empty() ? nullptr : ctx->d_geom, ctx->tile_log2, ev_ptrs(ev), n, ctx->d_items,
-                        ctx->d_ranges, (uint32_t)ranges.size(), ctx->d_rec, ctx->d_strag, ctx->d_plan_counters, s);
+                        ctx->d_ranges, (uint32_t)ranges.size(), ctx->d_rec, ctx->d_strag, ctx->d_tiny, kTinyCap,
+                        ctx->d_plan_counters, s);
     CHECK_LAUNCH(1);
     std::vector<unsigned char> hc(plan_counter_bytes());
     CU(cudaMemcpyAsync(hc.data(), ctx->d_plan_counters, hc.size(), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
-    uint64_t cnt4[4];
+    uint64_t cnt4[5];
     read_plan_counters(hc.data(), cnt4);
+    if (cnt4[4] > kTinyCap) return TOFMLEM_OK;  // a list made of slivers: not worth a plan (stays inactive)
+    ctx->plan.n_tiny = (uint32_t)cnt4[4];
     ctx->plan.valid = true;
     ctx->plan.x1 = ev->x1;
     ctx->plan.n = n;

@@ -117,15 +117,15 @@ void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_ge
 size_t plan_counter_bytes();
 void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom /* NULL: no tiles */, int tile_log2,
                          const EventPtrs &ev, uint64_t n, const TileItem *items, const TileRange *ranges,
-                         uint32_t n_ranges, const RecPtrs &rec,
-                         uint32_t *stragglers, void *d_counters, cudaStream_t s);
-void read_plan_counters(const void *h_counters, uint64_t out[4]);
+                         uint32_t n_ranges, const RecPtrs &rec, uint32_t *stragglers,
+                         uint2 *tiny_list /* (event, 1) pieces of the kRecTiny events */, uint32_t tiny_cap,
+                         void *d_counters, cudaStream_t s);
+void read_plan_counters(const void *h_counters, uint64_t out[5]);  // ... and the kRecTiny events
 // ev: the raw events of the planned list (the kRecTiny records are walked from them)
 void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &ev, const RecPtrs &rec, uint64_t n,
                             const float *image, float *fwd, cudaStream_t s);
 // chunks: n_pieces (first event, count <= 32) pairs; or index: n_index event numbers, 32 per piece
-void launch_em_planned(const ProjParams &p, const EventPtrs &ev, const RecPtrs &rec, const uint2 *chunks,
-                       const uint32_t *index,
+void launch_em_planned(const ProjParams &p, const RecPtrs &rec, const uint2 *chunks, const uint32_t *index,
                        uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
                        bool vec_ok, DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s);
 

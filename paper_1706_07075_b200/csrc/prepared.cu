@@ -105,7 +105,8 @@ struct PlanCounters {
     unsigned long long n_valid;      // events whose window meets the grid
     unsigned long long n_tile;       // of these: running on a tile
     unsigned long long n_straggler;  // events of a tile item that do not fit its tile (appended to the straggler list)
-    unsigned long long visits;       // voxel visits of one pass
+    unsigned long long visits;       // voxel visits of one pass (without the kRecTiny events)
+    unsigned long long n_tiny;       // kRecTiny events (appended to the tiny list as one-event pieces while it has room)
 };
 
 __device__ __forceinline__ int sel3i(int a, int v0, int v1, int v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
@@ -114,10 +115,10 @@ __global__ void __launch_bounds__(kBlock)
 prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, EventPtrs ev, uint64_t n,
                     const TileItem *__restrict__ items, const TileRange *__restrict__ ranges, unsigned n_ranges,
                     double qs, double qi, RecPtrs rec, uint32_t *__restrict__ stragglers,
-                    PlanCounters *__restrict__ counters) {
+                    uint2 *__restrict__ tiny_list, unsigned tiny_cap, PlanCounters *__restrict__ counters) {
     const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
     const unsigned lane = threadIdx.x & 31u;
-    bool valid = false, tile = false, straggler = false;
+    bool valid = false, tile = false, straggler = false, is_tiny = false;
     unsigned visits = 0;
     if (e < n) {
         // the tile item that holds this event, if any (the items' event ranges, sorted by their first event)
@@ -142,7 +143,7 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
             const int nx = P.n[0], ny = P.n[1];
             const int idx0 = (g.i[2] * ny + g.i[1]) * nx + g.i[0];
             const bool tiny = r.te - r.ts < (float)(32768.0 * qi);  // prepared.cuh, kRecTiny
-            if (item >= 0 && tiny) straggler = true;
+            is_tiny = tiny;
             if (item >= 0 && !tiny) {
                 // ---- does the window stay inside the bin's tile?  Dry run of the tile walk, every voxel checked.
                 const unsigned key = __ldg(&items[item].key);  // the item's FIRST cube: the tile's origin
@@ -219,7 +220,7 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
                     ngrp += gg != grp;
                     grp = gg;
                 }
-                visits = nvis;
+                visits = tiny ? 0u : nvis;
                 ra = make_float4(r.ts, r.te, r.t0[0], r.t0[1]);
                 rb = make_float4(r.t0[2], r.td[0], r.td[1], r.td[2]);
                 rc.x = (unsigned)idx0;
@@ -247,6 +248,15 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
     }
     base = __shfl_sync(0xffffffffu, base, 0);
     if (straggler) stragglers[base + __popc(ms & ((1u << lane) - 1u))] = (uint32_t)e;
+    // the slivers: one-event pieces for the unplanned fused pass (projector.cu)
+    const unsigned mt2 = __ballot_sync(0xffffffffu, is_tiny);
+    if (mt2) {
+        unsigned b2 = 0;
+        if (lane == 0) b2 = (unsigned)atomicAdd(&counters->n_tiny, (unsigned long long)__popc(mt2));
+        b2 = __shfl_sync(0xffffffffu, b2, 0);
+        const unsigned slot = b2 + __popc(mt2 & ((1u << lane) - 1u));
+        if (is_tiny && slot < tiny_cap) tiny_list[slot] = make_uint2((unsigned)e, 1u);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -384,21 +394,6 @@ __device__ __noinline__ float tiny_forward(const ProjParams &P, const EventPtrs 
     return ray_gather<true>(P, r, image, visits);  // un-normalised, mm units
 }
 
-template <bool VEC, bool BRICK>
-__device__ __noinline__ int tiny_em(const ProjParams &P, const EventPtrs &ev, uint64_t e, float w_e,
-                                    const float *__restrict__ image, float *__restrict__ corr, bool &valid) {
-    Ray r;
-    int visits;
-    valid = false;
-    if (!ray_setup<true>(P, __ldg(ev.x1 + e), __ldg(ev.y1 + e), __ldg(ev.z1 + e), __ldg(ev.x2 + e), __ldg(ev.y2 + e),
-                         __ldg(ev.z2 + e), __ldg(ev.dt + e), r))
-        return 0;
-    const float fw = ray_gather<true>(P, r, image, visits);
-    if (!(fw > 0.0f)) return 0;
-    valid = true;
-    return ray_scatter<true, VEC, BRICK>(P, r, corr, w_e / fw);
-}
-
 // Forward projection of a planned list: fwd_e = gauss_norm / kappa * sum_j l_j 2^(-mid_j^2) x_j.
 __global__ void __launch_bounds__(kBlock)
 planned_forward_kernel(ProjParams P, EventPtrs ev, RecPtrs rec, uint64_t n, int nx, int ny, float out_scale,
@@ -423,8 +418,7 @@ planned_forward_kernel(ProjParams P, EventPtrs ev, RecPtrs rec, uint64_t n, int 
 // (the stragglers of the tile items).
 template <bool VEC, bool BRICK>
 __global__ void __launch_bounds__(kBlock, 5)
-em_planned_kernel(ProjParams P, EventPtrs ev, RecPtrs rec, int nx, int ny, const uint2 *__restrict__ chunks,
-                  const uint32_t *__restrict__ index,
+em_planned_kernel(RecPtrs rec, int nx, int ny, const uint2 *__restrict__ chunks, const uint32_t *__restrict__ index,
                   uint32_t n_pieces, uint32_t n_index, const float *__restrict__ evw, const float *__restrict__ image,
                   float *__restrict__ corr, DeviceStats *stats, unsigned *queues, unsigned nseg, unsigned per_seg,
                   unsigned segs_per_sm) {
@@ -457,15 +451,8 @@ em_planned_kernel(ProjParams P, EventPtrs ev, RecPtrs rec, int nx, int ny, const
         }
         if (!have) continue;
         const uint4 rc = __ldcs(rec.c + e);
-        if ((rc.y & (kRecValid | kRecTile)) != kRecValid) continue;  // tile records never appear in these lists
-        if (rc.y & kRecTiny) {  // a sliver of a window: the unplanned walk
-            bool valid;
-            const int reds = tiny_em<VEC, BRICK>(P, ev, e, evw ? __ldg(evw + e) : 1.0f, image, corr, valid);
-            vis += rc.z & 0xFFFFu;
-            nv += valid;
-            nr += reds;
-            continue;
-        }
+        // tile records never appear in these lists; the slivers (kRecTiny) have their own pass
+        if ((rc.y & (kRecValid | kRecTile | kRecTiny)) != kRecValid) continue;
         const RecRay r = rec_ray(__ldcs(rec.a + e), __ldcs(rec.b + e));
         const int i0 = (rc.y & kRecNeg0) ? -1 : 1, i1 = (rc.y & kRecNeg1) ? -nx : nx,
                   i2 = (rc.y & kRecNeg2) ? -nx * ny : nx * ny;
@@ -518,22 +505,24 @@ size_t plan_counter_bytes() { return sizeof(PlanCounters); }
 
 void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom, int tile_log2, const EventPtrs &ev,
                          uint64_t n, const TileItem *items, const TileRange *ranges, uint32_t n_ranges,
-                         const RecPtrs &rec, uint32_t *stragglers, void *d_counters, cudaStream_t s) {
+                         const RecPtrs &rec, uint32_t *stragglers, uint2 *tiny_list, uint32_t tiny_cap, void *d_counters,
+                         cudaStream_t s) {
     if (n == 0) return;
     double kappa, qs, qi;
     plan_quantum(p, sigma, kappa, qs, qi);
     cudaMemsetAsync(d_counters, 0, sizeof(PlanCounters), s);
     prepare_rays_kernel<<<(unsigned)((n + kBlock - 1) / kBlock), kBlock, 0, s>>>(
-        p, d_geom, tile_log2, ev, n, items, ranges, d_geom ? n_ranges : 0u, qs, qi, rec, stragglers,
+        p, d_geom, tile_log2, ev, n, items, ranges, d_geom ? n_ranges : 0u, qs, qi, rec, stragglers, tiny_list, tiny_cap,
         static_cast<PlanCounters *>(d_counters));
 }
 
-void read_plan_counters(const void *h, uint64_t out[4]) {
+void read_plan_counters(const void *h, uint64_t out[5]) {
     const PlanCounters *c = static_cast<const PlanCounters *>(h);
     out[0] = c->n_valid;
     out[1] = c->n_tile;
     out[2] = c->n_straggler;
     out[3] = c->visits;
+    out[4] = c->n_tiny;
 }
 
 void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &ev, const RecPtrs &rec, uint64_t n,
@@ -546,8 +535,7 @@ void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &
 }
 
 template <bool VEC, bool BRICK>
-static void launch_planned(const ProjParams &p, const EventPtrs &ev, const RecPtrs &rec, const uint2 *chunks,
-                           const uint32_t *index,
+static void launch_planned(const ProjParams &p, const RecPtrs &rec, const uint2 *chunks, const uint32_t *index,
                            uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
                            DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s) {
     int per_sm = 0;
@@ -561,22 +549,20 @@ static void launch_planned(const ProjParams &p, const EventPtrs &ev, const RecPt
     if (nseg % 61u == 0) nseg -= segs;
     const unsigned per_seg = (n_pieces + nseg - 1) / nseg;
     cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-    em_planned_kernel<VEC, BRICK><<<n_sm * per_sm, kBlock, 0, s>>>(p, ev, rec, p.n[0], p.n[1], chunks, index, n_pieces,
-                                                                  n_index, evw, image, corr, stats, queues, nseg, per_seg,
-                                                                  segs);
+    em_planned_kernel<VEC, BRICK><<<n_sm * per_sm, kBlock, 0, s>>>(rec, p.n[0], p.n[1], chunks, index, n_pieces, n_index,
+                                                                  evw, image, corr, stats, queues, nseg, per_seg, segs);
 }
 
-void launch_em_planned(const ProjParams &p, const EventPtrs &ev, const RecPtrs &rec, const uint2 *chunks,
-                       const uint32_t *index,
+void launch_em_planned(const ProjParams &p, const RecPtrs &rec, const uint2 *chunks, const uint32_t *index,
                        uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
                        bool vec_ok, DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s) {
     if (n_pieces == 0) return;
     if (p.brick && vec_ok)
-        launch_planned<true, true>(p, ev, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<true, true>(p, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
     else if (vec_ok)
-        launch_planned<true, false>(p, ev, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<true, false>(p, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
     else
-        launch_planned<false, false>(p, ev, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<false, false>(p, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
 }
 
 }  // namespace tofmlem
