@@ -473,6 +473,7 @@ def main():
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next", "pipeline"],
                     help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
                          "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
+    ap.add_argument("--l2-persist", type=int, default=-1, help="TOFMLEM_OPT_L2_PERSIST override")
     ap.add_argument("--region-plan", type=int, default=-1, help="TOFMLEM_OPT_REGION_PLAN override (division report)")
     ap.add_argument("--sweep-events", default="10000000,146000000,500000000")
     ap.add_argument("--sweep-fwhm", default="100,300,600,0")
@@ -509,6 +510,8 @@ def main():
         ctx.set_option(pkg.OPT_EM_VARIANT, args.em_variant)
     if args.cache_share >= 0:
         ctx.set_option(pkg.OPT_CACHE_SHARE, args.cache_share)
+    if args.l2_persist >= 0:
+        ctx.set_option(pkg.OPT_L2_PERSIST, args.l2_persist)
     nvox = g.nvox
 
     def timed(fn):

@@ -117,6 +117,9 @@ enum {
     TOFMLEM_OPT_TILE_CHECK = 15,    /* 1: bounds-test every access to the shared-memory tiles and count violations in
                                        tofmlem_stats.tile_oob (a debugging aid; default 0).  The plan has already
                                        dry-run every tile event against its tile, so the count must stay 0 */
+    TOFMLEM_OPT_L2_PERSIST = 19,    /* 1 (default): the fused passes put a persisting L2 access-policy window on their correction
+                                       image (north_star: "the image kept L2-resident where it fits"); 0: no window.
+                                       Performance only. */
     TOFMLEM_OPT_REGION_OVERLAP = 18, /* tofmlem_reconstruct_regions / tofmlem_region_grid: 0 (default) = reading R13, every event in
                                        the ONE region that holds its TOF centre (bit-exact split), extended images summed;
                                        1 = reading R27, an event in every region its window reaches (1 or 2),

@@ -61,6 +61,9 @@ struct tofmlem_ctx {
     uint64_t launches = 0;
     // tile-mode plan of the fused pass (tofmlem_plan_events; tile.cu)
     int tile_min_events = 1024, tile_max_events = 8192, tile_check = 0;
+    int l2_persist = 1;           // TOFMLEM_OPT_L2_PERSIST
+    const float *l2_ptr = nullptr;  // correction image the stream's access-policy window currently covers
+    cudaStream_t l2_stream = nullptr;
     int region_overlap = 0;  // reading R27: an event goes to every region its window meets (TOFMLEM_OPT_REGION_OVERLAP)
     int region_plan = 0;  // tofmlem_reconstruct_regions plans every region's list (TOFMLEM_OPT_REGION_PLAN)
     int n_sm = 0;
@@ -351,12 +354,41 @@ bool plan_matches(const tofmlem_ctx *c, const float *x1, uint64_t n) {
            c->projector == 0 && c->plan.sigma == c->sigma && c->plan.trunc == c->trunc_sigmas;
 }
 
+// BASELINE.json north_star bullet 4: "the image kept L2-resident where it fits".  The correction image is the target of
+// every reduction; a persisting access-policy window on it keeps its sectors from being evicted by the streaming event /
+// record loads (ncu r04: the correction image was written back to DRAM ~20 times per pass).  Set once per (stream,
+// pointer); TOFMLEM_OPT_L2_PERSIST = 0 switches it off.
+void corr_l2_window(tofmlem_ctx *ctx, const float *d_corr, cudaStream_t s) {
+    if (!ctx->l2_persist || (ctx->l2_ptr == d_corr && ctx->l2_stream == s)) return;
+    ctx->l2_ptr = d_corr;
+    ctx->l2_stream = s;
+    int dev = 0, max_persist = 0, max_window = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
+    cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
+    size_t bytes = ctx->nvox * sizeof(float);
+    if (max_persist <= 0 || max_window <= 0) return;
+    size_t want = bytes < (size_t)max_persist ? bytes : (size_t)max_persist;
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want);
+    cudaStreamAttrValue attr;
+    memset(&attr, 0, sizeof attr);
+    attr.accessPolicyWindow.base_ptr = const_cast<float *>(d_corr);
+    attr.accessPolicyWindow.num_bytes = bytes < (size_t)max_window ? bytes : (size_t)max_window;
+    attr.accessPolicyWindow.hitRatio = (float)((double)want / (double)attr.accessPolicyWindow.num_bytes);
+    if (attr.accessPolicyWindow.hitRatio > 1.0f) attr.accessPolicyWindow.hitRatio = 1.0f;
+    attr.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    attr.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    cudaStreamSetAttribute(s, cudaStreamAttributeAccessPolicyWindow, &attr);
+    cudaGetLastError();  // not supported (e.g. MPS / MIG): the pass runs without the window
+}
+
 // One fused EM pass with the context's projector (0 = Siddon x Gaussian, 1 = K-sample kernel).
 int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint64_t n, const float *evw,
             const float *d_image, float *d_corr, bool vec, cudaStream_t s) {
     if (n == 0) return TOFMLEM_OK;
     ProjParams p = p_in;
     p.brick = bricks_on(ctx, d_corr) ? 1 : 0;
+    corr_l2_window(ctx, d_corr, s);
     if (ctx->projector == 1) {
         int rc = ensure_lut(ctx);
         if (rc) return rc;
@@ -601,6 +633,18 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
         case TOFMLEM_OPT_TILE_CHECK:
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "tile_check is 0 or 1");
             ctx->tile_check = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_L2_PERSIST:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "l2_persist is 0 or 1");
+            ctx->l2_persist = (int)value;
+            ctx->l2_ptr = nullptr;
+            if (!ctx->l2_persist) {
+                cudaStreamAttrValue attr;
+                memset(&attr, 0, sizeof attr);
+                cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &attr);
+                cudaCtxResetPersistingL2Cache();
+                cudaGetLastError();
+            }
             return TOFMLEM_OK;
         case TOFMLEM_OPT_REGION_OVERLAP:
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "region_overlap is 0 or 1");

@@ -343,8 +343,11 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
                 const float4 ra = __ldg(rec.a + e), rb = __ldg(rec.b + e);
                 const float te = ra.y, da = rb.y, df = rb.z, ds = rb.w;
                 const bool down = rc.y & kRecNeg0;
-                const int dpq = down ? -4 : 4;
-                const int inc_f = (rc.y & kRecNeg1) ? -4 : 4, inc_s = (rc.y & kRecNeg2) ? -4 * Wf : 4 * Wf;
+                // +-4 by arithmetic on the flag bits: as selects of two constants ptxas turns every use into an
+                // add / predicated add / move triple (ncu: 28 instead of 23 instructions per step)
+                const int dpq = 4 - (int)((rc.y & kRecNeg0) >> 1);   // kRecNeg0 = 16 -> 8
+                const int inc_f = 4 - (int)((rc.y & kRecNeg1) >> 2);  // kRecNeg1 = 32 -> 8
+                const int inc_s = (rc.y & kRecNeg2) ? -4 * Wf : 4 * Wf;
                 vis += rc.z;
                 float t = ra.x, ta = ra.z, tf = ra.w, ts = rb.x;
                 unsigned li = tile_addr + (rc.y >> kRecLiShift) * 4u;
@@ -447,21 +450,38 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
                 ++nt;
                 const float te = ra.y, da = rb.y, df = rb.z, ds = rb.w;
                 const bool down = rc.y & kRecNeg0;
-                const int dpq = down ? -4 : 4;
-                const int inc_f = (rc.y & kRecNeg1) ? -4 : 4, inc_s = (rc.y & kRecNeg2) ? -4 * Wf : 4 * Wf;
+                // +-4 by arithmetic on the flag bits: as selects of two constants ptxas turns every use into an
+                // add / predicated add / move triple (ncu: 28 instead of 23 instructions per step)
+                const int dpq = 4 - (int)((rc.y & kRecNeg0) >> 1);   // kRecNeg0 = 16 -> 8
+                const int inc_f = 4 - (int)((rc.y & kRecNeg1) >> 2);  // kRecNeg1 = 32 -> 8
+                const int inc_s = (rc.y & kRecNeg2) ? -4 * Wf : 4 * Wf;
                 float t = ra.x, ta = ra.z, tf = ra.w, ts = rb.x;
                 unsigned li = tile_addr + (rc.y >> kRecLiShift) * 4u;
                 unsigned pq = (down ? dn_addr : up_addr) + ((rc.y >> kRecPlaneShift) & 127u) * 4u;
                 int na = (int)__float_as_int(lds_f32(pq));
-                while (true) {
-                    const float tn = min3f(ta, tf, ts);
-                    if (!(tn < te)) break;
-                    if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                    red_shared_u32(li, __float_as_uint(fmaf(chord_weight(t, tn), scaleS, 8388608.0f)) - 0x4B000000u);
-                    advance_plane(ta, li, na, pq, tn, da, dpq);
-                    advance_addr(tf, li, tn, df, inc_f);
-                    advance_addr(ts, li, tn, ds, inc_s);
-                    t = tn;
+                while (true) {  // two steps per trip: t and t2 alternate, no register move
+                    float t2;
+                    {
+                        const float tn = min3f(ta, tf, ts);
+                        if (!(tn < te)) break;
+                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                        red_shared_u32(li, __float_as_uint(fmaf(chord_weight(t, tn), scaleS, 8388608.0f)) - 0x4B000000u);
+                        advance_plane(ta, li, na, pq, tn, da, dpq);
+                        advance_addr(tf, li, tn, df, inc_f);
+                        advance_addr(ts, li, tn, ds, inc_s);
+                        t2 = tn;
+                    }
+                    t = t2;
+                    {
+                        const float tn = min3f(ta, tf, ts);
+                        if (!(tn < te)) break;
+                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                        red_shared_u32(li, __float_as_uint(fmaf(chord_weight(t, tn), scaleS, 8388608.0f)) - 0x4B000000u);
+                        advance_plane(ta, li, na, pq, tn, da, dpq);
+                        advance_addr(tf, li, tn, df, inc_f);
+                        advance_addr(ts, li, tn, ds, inc_s);
+                        t = tn;
+                    }
                 }
                 if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
                 red_shared_u32(li, __float_as_uint(fmaf(chord_weight(t, te), scaleS, 8388608.0f)) - 0x4B000000u);

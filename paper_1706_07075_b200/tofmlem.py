@@ -30,6 +30,7 @@ OPT_TILE_CHECK = 15
 OPT_TILE_MAX_EVENTS = 16
 OPT_REGION_PLAN = 17
 OPT_REGION_OVERLAP = 18
+OPT_L2_PERSIST = 19
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
