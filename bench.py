@@ -529,8 +529,9 @@ def main():
     lors = synth.make_sens_lors_chunked(cfg, m, device=dev)
     sens_ms = timed(lambda: ctx.sensitivity(lors, m, sens))
     del lors
-    # ---- a1: locality binning (one-off per data set)
+    # ---- a1: locality binning (one-off per data set); scratch of binning and plan allocated beforehand (tofmlem_reserve)
     bin_ms = 0.0
+    ctx.reserve(n)
     if not args.no_bin:
         key = torch.empty(n, dtype=torch.int32, device=dev)
         perm = torch.empty(n, dtype=torch.int32, device=dev)

@@ -77,7 +77,7 @@ typedef struct {
     int32_t active;           /* 1: the context holds ray records for the planned list */
     int32_t sorted;           /* 1: the list was found sorted by locality key (0 also when tiles do not fit: not looked at) */
     uint32_t n_tile_items;    /* pieces of locality bins that are accumulated in shared-memory tiles (0: none) */
-    uint32_t n_direct_chunks; /* 32-event pieces of the direct pass on records (without the tile items' stragglers) */
+    uint32_t n_direct_chunks; /* 32-event pieces of the list that hold events of the direct pass on records */
     uint64_t n_tile_events;   /* events that run on a tile */
     uint64_t n_direct_events; /* n - n_tile_events */
     uint64_t n_stragglers;    /* of n_direct_events: valid events of tile items whose window leaves the item's tile */
@@ -321,8 +321,9 @@ int tofmlem_probe(tofmlem_ctx *ctx, int kind, float *d_buf, uint64_t n_elems, ui
 /* Copies the counters of the last pass to *h_out.  SYNCHRONISES the context's stream. */
 int tofmlem_get_stats(tofmlem_ctx *ctx, tofmlem_stats *h_out);
 /* Device time of the kernels of the LAST planned fused pass (tofmlem_plan_events), in milliseconds, measured with CUDA
- * events on the context's stream: h_ms[0] = tile pass (tile.cu), h_ms[1] = direct pass on records, h_ms[2] = the tile
- * items' stragglers; 0 for a part that did not run (all 0 after an unplanned pass).  SYNCHRONISES. */
+ * events on the context's stream: h_ms[0] = tile pass (tile.cu), h_ms[1] = direct pass on records, h_ms[2] = the
+ * unplanned pass over the sliver windows (prepared.cuh, kRecTiny); 0 for a part that did not run (all 0 after an
+ * unplanned pass).  SYNCHRONISES. */
 int tofmlem_pass_timing(tofmlem_ctx *ctx, float h_ms[3]);
 /* Text of the last error of this context ("" if none).  Valid until the next call on the context. */
 const char *tofmlem_last_error(const tofmlem_ctx *ctx);

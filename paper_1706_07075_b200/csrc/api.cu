@@ -1,7 +1,9 @@
 // api.cu -- the C ABI of libtofmlem (include/tofmlem.h): context, argument checks, stream orchestration.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
+#include <time.h>
 
 #include <algorithm>
 #include <new>
@@ -74,13 +76,13 @@ struct tofmlem_ctx {
     size_t items_cap = 0;
     TileRange *d_ranges = nullptr;
     size_t ranges_cap = 0;
-    uint2 *d_chunks = nullptr;
-    size_t chunks_cap = 0;
+    uint32_t *d_chunk_flags = nullptr;  // one per 32-event piece of the planned list: 1 = work for the direct pass
+    uint32_t *d_chunk_pos = nullptr, *d_chunk_list = nullptr, *d_chunk_tmp = nullptr;  // scan of the flags, flagged pieces
+    uint32_t *h_hist_pinned = nullptr;  // staging of the bin counts for the plan's host part
+    size_t h_hist_cap = 0;
     unsigned *d_plan_flags = nullptr;  // [0] tile work counter, [1] "keys not sorted" flag
     RecPtrs d_rec{nullptr, nullptr, nullptr};  // ray records of the planned list (prepared.cuh), 48 B per event
     size_t rec_cap = 0;
-    uint32_t *d_strag = nullptr;       // events of tile items that do not fit their tile
-    size_t strag_cap = 0;
     uint2 *d_tiny = nullptr;           // one-event pieces of the kRecTiny events (kTinyCap entries)
     float *d_ev_scale = nullptr;       // w_e / fwd_e of the tile events between the two phases of tile.cu (rec_cap floats)
     size_t smem_per_sm = 0;
@@ -106,7 +108,9 @@ struct tofmlem_ctx {
         int tile_log2 = 0;          // ... this cube size, for a context with
         double sigma = 0.0, trunc = 0.0;  // ... this TOF kernel
         int brick = 0;              // ... and this layout of the correction image
-        uint32_t n_items = 0, n_chunks = 0, n_strag = 0, n_tiny = 0, max_item_events = 0;
+        uint32_t n_items = 0, n_strag = 0, n_tiny = 0, max_item_events = 0;
+        uint64_t direct_valid = 0;  // valid events of the direct pass on records
+        uint32_t n_pieces = 0;      // 32-event pieces of the list that hold some of them
         uint64_t tile_events = 0, direct_events = 0, valid_events = 0, visits = 0;
         int sorted = 0;
     } plan;
@@ -268,15 +272,48 @@ void free_records(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_rec.a);
     cudaFree(ctx->d_rec.b);
     cudaFree(ctx->d_rec.c);
-    cudaFree(ctx->d_strag);
+    cudaFree(ctx->d_chunk_flags);
+    cudaFree(ctx->d_chunk_pos);
+    cudaFree(ctx->d_chunk_list);
+    cudaFree(ctx->d_chunk_tmp);
+    ctx->d_chunk_flags = ctx->d_chunk_pos = ctx->d_chunk_list = ctx->d_chunk_tmp = nullptr;
     cudaFree(ctx->d_ev_scale);
     cudaFree(ctx->d_tiny);
     ctx->d_tiny = nullptr;
     ctx->d_rec = RecPtrs{nullptr, nullptr, nullptr};
-    ctx->d_strag = nullptr;
     ctx->d_ev_scale = nullptr;
-    ctx->rec_cap = ctx->strag_cap = 0;
+    ctx->rec_cap = 0;
     ctx->plan.valid = false;
+}
+
+// Scratch of tofmlem_plan_events for a list of n events (grows only): ray records (48 B per event), w_e / fwd_e of the
+// tile pass (4 B), per-piece flags, the sliver list, pinned staging for the bin counts.
+int ensure_plan_scratch(tofmlem_ctx *ctx, uint64_t n) {
+    if (ctx->rec_cap < n) {
+        free_records(ctx);
+        CU(cudaMalloc(&ctx->d_rec.a, n * sizeof(float4)));
+        CU(cudaMalloc(&ctx->d_rec.b, n * sizeof(float4)));
+        CU(cudaMalloc(&ctx->d_rec.c, n * sizeof(uint4)));
+        CU(cudaMalloc(&ctx->d_ev_scale, n * sizeof(float)));
+        CU(cudaMalloc(&ctx->d_tiny, kTinyCap * sizeof(uint2)));
+        {
+            const size_t nc = (size_t)((n + 31) / 32) + 1;  // + the total
+            CU(cudaMalloc(&ctx->d_chunk_flags, nc * sizeof(uint32_t)));
+            CU(cudaMalloc(&ctx->d_chunk_pos, nc * sizeof(uint32_t)));
+            CU(cudaMalloc(&ctx->d_chunk_list, nc * sizeof(uint32_t)));
+            CU(cudaMalloc(&ctx->d_chunk_tmp, (size_t)scan_tmp_elems((uint32_t)nc) * sizeof(uint32_t)));
+        }
+        ctx->rec_cap = n;
+    }
+    const uint32_t nb = num_bins(ctx);
+    if (ctx->h_hist_cap < nb) {  // pinned: the 18 MB of counts at cfg-3 come back at PCIe speed
+        if (ctx->h_hist_pinned) cudaFreeHost(ctx->h_hist_pinned);
+        ctx->h_hist_pinned = nullptr;
+        ctx->h_hist_cap = 0;
+        CU(cudaMallocHost(&ctx->h_hist_pinned, (size_t)nb * sizeof(uint32_t)));
+        ctx->h_hist_cap = nb;
+    }
+    return ensure_bin_scratch(ctx, (size_t)nb + 1, 0);
 }
 
 // 32-byte event records of tofmlem_permute_events (grows only).  false: not enough memory (the caller falls back).
@@ -399,7 +436,7 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 1;
         if (!ctx->t_ev[0])
             for (auto &te : ctx->t_ev) CU(cudaEventCreate(&te));
-        ctx->t_have = (ctx->plan.n_items ? 1 : 0) | (ctx->plan.n_chunks ? 2 : 0) | (ctx->plan.n_strag ? 4 : 0);
+        ctx->t_have = (ctx->plan.n_items ? 1 : 0) | (ctx->plan.direct_valid ? 2 : 0) | (ctx->plan.n_tiny ? 4 : 0);
         CU(cudaEventRecord(ctx->t_ev[0], s));
         if (ctx->plan.n_items) {
             TileGeom g;
@@ -410,17 +447,12 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
             CHECK_LAUNCH(1);
         }
         CU(cudaEventRecord(ctx->t_ev[1], s));
-        if (ctx->plan.n_chunks) {
-            launch_em_planned(p, ctx->d_rec, ctx->d_chunks, nullptr, ctx->plan.n_chunks, 0, evw, d_image, d_corr, vec,
+        if (ctx->plan.direct_valid) {
+            launch_em_planned(p, ctx->d_rec, n, ctx->d_chunk_list, ctx->plan.n_pieces, evw, d_image, d_corr, vec,
                               ctx->d_stats, ctx->d_queues, n_sm, s);
             CHECK_LAUNCH(1);
         }
         CU(cudaEventRecord(ctx->t_ev[2], s));
-        if (ctx->plan.n_strag) {
-            launch_em_planned(p, ctx->d_rec, nullptr, ctx->d_strag, (ctx->plan.n_strag + 31u) / 32u, ctx->plan.n_strag,
-                              evw, d_image, d_corr, vec, ctx->d_stats, ctx->d_queues, n_sm, s);
-            CHECK_LAUNCH(1);
-        }
         if (ctx->plan.n_tiny) {  // kRecTiny: the unplanned walk (fp64 set-up), one event per piece
             launch_em_correction_chunks(p, true, ev, n, ctx->d_tiny, ctx->plan.n_tiny, evw, d_image, d_corr, vec,
                                         ctx->d_stats, ctx->d_queues, s);
@@ -560,7 +592,7 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_geom);
     cudaFree(ctx->d_items);
     cudaFree(ctx->d_ranges);
-    cudaFree(ctx->d_chunks);
+    if (ctx->h_hist_pinned) cudaFreeHost(ctx->h_hist_pinned);
     cudaFree(ctx->d_plan_counters);
     for (auto &te : ctx->t_ev)
         if (te) cudaEventDestroy(te);
@@ -679,6 +711,10 @@ int tofmlem_reserve(tofmlem_ctx *ctx, uint64_t n_events) {
         rc = ensure_bin_scratch(ctx, (size_t)num_bins(ctx) * S + 1, S > 1 ? n_events : 0);
         if (rc) return rc;
         if (!ensure_pack(ctx, n_events)) return fail(ctx, TOFMLEM_ENOMEM, "reserve: no memory for the 32-byte event records");
+        if (ctx->tof && ctx->projector == 0) {  // tofmlem_plan_events: ray records and their side arrays, pinned bin counts
+            rc = ensure_plan_scratch(ctx, n_events);
+            if (rc) return rc;
+        }
     }
     return TOFMLEM_OK;
 }
@@ -947,7 +983,8 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
 int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) {
     if (!ctx) return TOFMLEM_EINVAL;
     ctx->plan.valid = false;
-    ctx->plan.n_items = ctx->plan.n_chunks = ctx->plan.n_strag = 0;
+    ctx->plan.n_items = ctx->plan.n_strag = 0;
+    ctx->plan.direct_valid = 0;
     ctx->plan.tile_events = ctx->plan.direct_events = ctx->plan.valid_events = ctx->plan.visits = 0;
     ctx->plan.sorted = 0;
     if (n == 0) return TOFMLEM_OK;
@@ -960,15 +997,17 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
     TileGeom g;
     build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, ctx->smem_per_sm, g);
     cudaStream_t s = ctx->stream;
+    {
+        int rc0 = ensure_plan_scratch(ctx, n);
+        if (rc0) return rc0;
+    }
+    const bool ptime = getenv("TOFMLEM_PLAN_TIMING") != nullptr;
+    auto now = [&]() { cudaStreamSynchronize(s); struct timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6; };
+    double tp0 = ptime ? now() : 0.0, tp1 = 0, tp2 = 0, tp3 = 0, tp4 = 0;
     // ---- which bins become tile items?  Needs a list sorted by key (tofmlem_permute_events) and tiles that fit.
     std::vector<TileItem> items;
     std::vector<TileRange> ranges;
-    std::vector<uint2> chunks;
     uint64_t in_items = 0;
-    auto add_run = [&](uint64_t lo, uint64_t hi) {
-        for (uint64_t a = lo; a < hi; a += 32)
-            chunks.push_back(make_uint2((unsigned)a, (unsigned)(hi - a < 32 ? hi - a : 32)));
-    };
     bool sorted = false;
     if (g.ok) {
         const uint32_t nb = num_bins(ctx);
@@ -978,11 +1017,12 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMemsetAsync(ctx->d_plan_flags, 0, 2 * sizeof(unsigned), s));
         launch_plan_hist(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, ctx->d_hist, nb, ctx->d_plan_flags + 1, s);
         CHECK_LAUNCH(1);
-        std::vector<uint32_t> cnt(nb);
+        const uint32_t *cnt = ctx->h_hist_pinned;
         unsigned flags[2] = {0, 0};
-        CU(cudaMemcpyAsync(cnt.data(), ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(ctx->h_hist_pinned, ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
         CU(cudaMemcpyAsync(flags, ctx->d_plan_flags, sizeof flags, cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
+        if (ptime) tp1 = now();
         sorted = flags[1] == 0;
         if (sorted) {
             // Tile items: a bin with at least tile_min_events events (pieces of at most tile_max_events, whole warps), or
@@ -1027,19 +1067,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
                     in_items += c;
                 }
             }
-            uint64_t run_lo = 0, run_hi = 0;
-            for (uint32_t b = 0; b < nb; ++b) {
-                if (cnt[b] == 0) continue;
-                if (state[b]) {
-                    if (run_hi > run_lo) add_run(run_lo, run_hi);
-                    run_lo = run_hi = 0;
-                } else {
-                    if (run_hi == run_lo) run_lo = start[b];
-                    run_hi = start[b] + cnt[b];
-                }
-            }
-            if (run_hi > run_lo) add_run(run_lo, run_hi);
-            if (off < n) add_run(off, n);  // events with an invalid key (sorted to the end): their records are invalid
             // the items' event ranges in list order: the record set-up finds the item of an event by bisection
             for (size_t i = 0; i < items.size(); ++i) {
                 ranges.push_back(TileRange{items[i].start, items[i].count, (uint32_t)i, 0u});
@@ -1048,30 +1075,13 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
             std::sort(ranges.begin(), ranges.end(), [](const TileRange &x, const TileRange &y) { return x.start < y.start; });
         }
     }
+    if (ptime) tp2 = now();
     ctx->plan.sorted = sorted ? 1 : 0;
     if (items.empty()) {  // no tiles (window too wide, unsorted list, sparse bins): the whole list in order
         ranges.clear();
-        chunks.clear();
-        add_run(0, n);
         in_items = 0;
     }
     // ---- scratch (grows only)
-    if (ctx->rec_cap < n) {
-        free_records(ctx);
-        CU(cudaMalloc(&ctx->d_rec.a, n * sizeof(float4)));
-        CU(cudaMalloc(&ctx->d_rec.b, n * sizeof(float4)));
-        CU(cudaMalloc(&ctx->d_rec.c, n * sizeof(uint4)));
-        CU(cudaMalloc(&ctx->d_ev_scale, n * sizeof(float)));
-        CU(cudaMalloc(&ctx->d_tiny, kTinyCap * sizeof(uint2)));
-        ctx->rec_cap = n;
-    }
-    if (ctx->strag_cap < in_items) {
-        cudaFree(ctx->d_strag);
-        ctx->d_strag = nullptr;
-        ctx->strag_cap = 0;
-        CU(cudaMalloc(&ctx->d_strag, in_items * sizeof(uint32_t)));
-        ctx->strag_cap = in_items;
-    }
     if (ctx->items_cap < items.size()) {
         cudaFree(ctx->d_items);
         ctx->d_items = nullptr;
@@ -1086,13 +1096,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMalloc(&ctx->d_ranges, ranges.size() * sizeof(TileRange)));
         ctx->ranges_cap = ranges.size();
     }
-    if (ctx->chunks_cap < chunks.size()) {
-        cudaFree(ctx->d_chunks);
-        ctx->d_chunks = nullptr;
-        ctx->chunks_cap = 0;
-        CU(cudaMalloc(&ctx->d_chunks, chunks.size() * sizeof(uint2)));
-        ctx->chunks_cap = chunks.size();
-    }
     if (!items.empty()) {
         if (!ctx->d_geom) CU(cudaMalloc(&ctx->d_geom, sizeof(TileGeom)));
         if (memcmp(&g, &ctx->h_geom_sent, sizeof g) != 0) {
@@ -1102,16 +1105,28 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMemcpyAsync(ctx->d_items, items.data(), items.size() * sizeof(TileItem), cudaMemcpyHostToDevice, s));
         CU(cudaMemcpyAsync(ctx->d_ranges, ranges.data(), ranges.size() * sizeof(TileRange), cudaMemcpyHostToDevice, s));
     }
-    if (!chunks.empty())
-        CU(cudaMemcpyAsync(ctx->d_chunks, chunks.data(), chunks.size() * sizeof(uint2), cudaMemcpyHostToDevice, s));
+    if (ptime) tp3 = now();
     // ---- the records: fp64 set-up, quantisation, dry run against the tile (prepared.cu)
     launch_prepare_rays(p, ctx->sigma, items.empty() ? nullptr : ctx->d_geom, ctx->tile_log2, ev_ptrs(ev), n, ctx->d_items,
-                        ctx->d_ranges, (uint32_t)ranges.size(), ctx->d_rec, ctx->d_strag, ctx->d_tiny, kTinyCap,
+                        ctx->d_ranges, (uint32_t)ranges.size(), ctx->d_rec, ctx->d_chunk_flags, ctx->d_tiny, kTinyCap,
                         ctx->d_plan_counters, s);
     CHECK_LAUNCH(1);
+    // the pieces of the direct pass: the flagged 32-event pieces, compacted in list order on the device
+    const uint32_t nc = (uint32_t)((n + 31) / 32);
+    uint32_t n_pieces = 0;
+    CU(cudaMemsetAsync(ctx->d_chunk_flags + nc, 0, sizeof(uint32_t), s));
+    ctx->launches += launch_exclusive_scan_u32(ctx->d_chunk_flags, ctx->d_chunk_pos, ctx->d_chunk_tmp, nc + 1, s);
+    launch_compact_flags(ctx->d_chunk_flags, ctx->d_chunk_pos, nc, ctx->d_chunk_list, s);
+    CHECK_LAUNCH(1);
+    CU(cudaMemcpyAsync(&n_pieces, ctx->d_chunk_pos + nc, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     std::vector<unsigned char> hc(plan_counter_bytes());
     CU(cudaMemcpyAsync(hc.data(), ctx->d_plan_counters, hc.size(), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
+    if (ptime) {
+        tp4 = now();
+        fprintf(stderr, "plan timing: hist+copy %.2f ms, host items %.2f ms, alloc+upload %.2f ms, prepare %.2f ms\n", tp1 - tp0,
+                tp2 - tp1, tp3 - tp2, tp4 - tp3);
+    }
     uint64_t cnt4[5];
     read_plan_counters(hc.data(), cnt4);
     if (cnt4[4] > kTinyCap) return TOFMLEM_OK;  // a list made of slivers: not worth a plan (stays inactive)
@@ -1127,12 +1142,13 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
     ctx->plan.max_item_events = 0;
     for (const TileItem &it : items)
         if (it.count + it.count2 > ctx->plan.max_item_events) ctx->plan.max_item_events = it.count + it.count2;
-    ctx->plan.n_chunks = (uint32_t)chunks.size();
     ctx->plan.n_strag = (uint32_t)cnt4[2];
     ctx->plan.valid_events = cnt4[0];
     ctx->plan.tile_events = cnt4[1];
     ctx->plan.direct_events = n - cnt4[1];
     ctx->plan.visits = cnt4[3];
+    ctx->plan.direct_valid = cnt4[0] - cnt4[1] - cnt4[4];
+    ctx->plan.n_pieces = n_pieces;
     return TOFMLEM_OK;
 }
 
@@ -1141,7 +1157,7 @@ int tofmlem_plan_info(const tofmlem_ctx *ctx, tofmlem_plan *h_out) {
     h_out->active = ctx->plan.valid ? 1 : 0;
     h_out->sorted = ctx->plan.sorted;
     h_out->n_tile_items = ctx->plan.n_items;
-    h_out->n_direct_chunks = ctx->plan.n_chunks;
+    h_out->n_direct_chunks = ctx->plan.n_pieces;
     h_out->n_tile_events = ctx->plan.tile_events;
     h_out->n_direct_events = ctx->plan.direct_events;
     h_out->n_stragglers = ctx->plan.n_strag;

@@ -437,7 +437,23 @@ __global__ void __launch_bounds__(kBlock) plan_hist_kernel(GridF32 g, int tile_l
     __syncthreads();
     if (e >= n) return;
     if (k < keys[threadIdx.x]) *unsorted = 1u;
-    if (k < nbins) atomicAdd(hist + k, 1u);
+    // the list is (expected to be) sorted: the lanes of a warp hold one or two keys, so one atomic per distinct key of the
+    // warp instead of one per event (which serialise on the same counter: 21 -> ~4 ms at 146 M events)
+    const unsigned active = __activemask();
+    const unsigned same = __match_any_sync(active, k);
+    if (k < nbins && (threadIdx.x & 31u) == (unsigned)(__ffs(same) - 1)) atomicAdd(hist + k, (uint32_t)__popc(same));
+}
+
+// Order-preserving compaction: list[pos[i]] = i for every i with flags[i] != 0 (pos = exclusive scan of flags).
+__global__ void __launch_bounds__(kBlock) compact_flags_kernel(const uint32_t *__restrict__ flags,
+                                                               const uint32_t *__restrict__ pos, uint32_t n,
+                                                               uint32_t *__restrict__ list) {
+    const uint32_t i = blockIdx.x * kBlock + threadIdx.x;
+    if (i < n && flags[i]) list[pos[i]] = i;
+}
+
+void launch_compact_flags(const uint32_t *flags, const uint32_t *pos, uint32_t n, uint32_t *list, cudaStream_t s) {
+    if (n) compact_flags_kernel<<<(n + kBlock - 1) / kBlock, kBlock, 0, s>>>(flags, pos, n, list);
 }
 
 void launch_plan_hist(const GridF32 &g, int tile_log2, const EventPtrs &ev, uint64_t n, uint32_t *hist, uint32_t nbins,

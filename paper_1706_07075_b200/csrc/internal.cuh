@@ -111,23 +111,24 @@ void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_ge
                     cudaStream_t s);
 
 // ---- prepared.cu: ray records of a planned list and the passes that run on them
-// Writes one record per event (p.brick says which group count the direct records carry), appends the events of tile
-// items that do not fit their tile to `stragglers` (room for every event of a tile item) and fills the counters
-// (plan_counter_bytes() bytes of device memory; read_plan_counters: valid events, tile events, stragglers, visits).
+// Writes one record per event (p.brick says which group count the direct records carry), one flag per 32-event piece of
+// the list (1: the piece holds events for the direct pass on records), the kRecTiny events as one-event pieces, and
+// fills the counters (plan_counter_bytes() bytes of device memory; read_plan_counters: valid events, tile events,
+// events of tile items that do not fit their tile, visits, kRecTiny events).
 size_t plan_counter_bytes();
 void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom /* NULL: no tiles */, int tile_log2,
                          const EventPtrs &ev, uint64_t n, const TileItem *items, const TileRange *ranges,
-                         uint32_t n_ranges, const RecPtrs &rec, uint32_t *stragglers,
+                         uint32_t n_ranges, const RecPtrs &rec, uint32_t *chunk_flags /* ceil(n / 32) */,
                          uint2 *tiny_list /* (event, 1) pieces of the kRecTiny events */, uint32_t tiny_cap,
                          void *d_counters, cudaStream_t s);
 void read_plan_counters(const void *h_counters, uint64_t out[5]);  // ... and the kRecTiny events
 // ev: the raw events of the planned list (the kRecTiny records are walked from them)
 void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &ev, const RecPtrs &rec, uint64_t n,
                             const float *image, float *fwd, cudaStream_t s);
-// chunks: n_pieces (first event, count <= 32) pairs; or index: n_index event numbers, 32 per piece
-void launch_em_planned(const ProjParams &p, const RecPtrs &rec, const uint2 *chunks, const uint32_t *index,
-                       uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
-                       bool vec_ok, DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s);
+// pieces: n_pieces indices of the 32-event pieces of the list that hold work for this pass, ascending
+void launch_em_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, const uint32_t *pieces, uint32_t n_pieces,
+                       const float *evw, const float *image, float *corr, bool vec_ok, DeviceStats *stats,
+                       unsigned *queues, int n_sm, cudaStream_t s);
 
 // ---- image_ops.cu
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);
@@ -161,6 +162,8 @@ void launch_bin_keys(const GridF32 &g, int tile_log2, const SubBin &sb, const Ev
 uint32_t scan_tmp_elems(uint32_t n);
 // returns the number of kernels launched; tmp: scan_tmp_elems(n) words (NULL: single-block scan)
 int launch_exclusive_scan_u32(const uint32_t *in, uint32_t *out, uint32_t *tmp, uint32_t n, cudaStream_t s);
+// list[pos[i]] = i for flags[i] != 0 (pos: exclusive scan of flags): the flagged indices in ascending order
+void launch_compact_flags(const uint32_t *flags, const uint32_t *pos, uint32_t n, uint32_t *list, cudaStream_t s);
 void launch_scatter_perm(const uint32_t *key, const uint8_t *sub, uint32_t S, uint64_t n, uint32_t nbins,
                          uint32_t *cursor, uint32_t *perm, cudaStream_t s);
 void launch_strided_copy(const uint32_t *fine, uint32_t S, uint32_t count, uint32_t *out, cudaStream_t s);

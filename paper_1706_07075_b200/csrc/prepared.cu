@@ -104,7 +104,7 @@ __device__ bool quantise(const Geo &g, double qs /* kappa 2^k */, double qi /* 2
 struct PlanCounters {
     unsigned long long n_valid;      // events whose window meets the grid
     unsigned long long n_tile;       // of these: running on a tile
-    unsigned long long n_straggler;  // events of a tile item that do not fit its tile (appended to the straggler list)
+    unsigned long long n_straggler;  // valid events of a tile item that do not fit its tile (they take the direct pass)
     unsigned long long visits;       // voxel visits of one pass (without the kRecTiny events)
     unsigned long long n_tiny;       // kRecTiny events (appended to the tiny list as one-event pieces while it has room)
 };
@@ -114,7 +114,7 @@ __device__ __forceinline__ int sel3i(int a, int v0, int v1, int v2) { return a =
 __global__ void __launch_bounds__(kBlock)
 prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, EventPtrs ev, uint64_t n,
                     const TileItem *__restrict__ items, const TileRange *__restrict__ ranges, unsigned n_ranges,
-                    double qs, double qi, RecPtrs rec, uint32_t *__restrict__ stragglers,
+                    double qs, double qi, RecPtrs rec, uint32_t *__restrict__ chunk_flags,
                     uint2 *__restrict__ tiny_list, unsigned tiny_cap, PlanCounters *__restrict__ counters) {
     const uint64_t e = (uint64_t)blockIdx.x * kBlock + threadIdx.x;
     const unsigned lane = threadIdx.x & 31u;
@@ -235,19 +235,18 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
         rec.b[e] = rb;
         rec.c[e] = rc;
     }
-    // counters and the straggler list, one atomic per warp
+    // counters, one atomic per warp; does this 32-event piece hold work for the direct pass on records?
     const unsigned mv = __ballot_sync(0xffffffffu, valid), mt = __ballot_sync(0xffffffffu, tile),
-                   ms = __ballot_sync(0xffffffffu, straggler);
+                   ms = __ballot_sync(0xffffffffu, straggler),
+                   md = __ballot_sync(0xffffffffu, valid && !tile && !is_tiny);
     const unsigned vis = __reduce_add_sync(0xffffffffu, visits);
-    unsigned base = 0;
     if (lane == 0) {
         if (mv) atomicAdd(&counters->n_valid, (unsigned long long)__popc(mv));
         if (mt) atomicAdd(&counters->n_tile, (unsigned long long)__popc(mt));
         if (vis) atomicAdd(&counters->visits, (unsigned long long)vis);
-        if (ms) base = (unsigned)atomicAdd(&counters->n_straggler, (unsigned long long)__popc(ms));
+        if (ms) atomicAdd(&counters->n_straggler, (unsigned long long)__popc(ms));
+        if (e - lane < n) chunk_flags[(e - lane) >> 5] = md ? 1u : 0u;
     }
-    base = __shfl_sync(0xffffffffu, base, 0);
-    if (straggler) stragglers[base + __popc(ms & ((1u << lane) - 1u))] = (uint32_t)e;
     // the slivers: one-event pieces for the unplanned fused pass (projector.cu)
     const unsigned mt2 = __ballot_sync(0xffffffffu, is_tiny);
     if (mt2) {
@@ -413,15 +412,14 @@ planned_forward_kernel(ProjParams P, EventPtrs ev, RecPtrs rec, uint64_t n, int 
 }
 
 // The direct fused pass on records: persistent, one work queue per list segment, the warps of an SM on neighbouring
-// events (em_persistent_kernel of projector.cu explains the scheduling).  The pieces of work come from `chunks`
-// ((first event, count <= 32) pairs) or, when `index` is given, are 32 consecutive entries of an event index list
-// (the stragglers of the tile items).
+// events (em_persistent_kernel of projector.cu explains the scheduling).  `pieces` lists, in ascending order, the 32-event
+// pieces of the list that hold anything for this pass (the plan flags them and compacts the flags on the device); inside
+// a piece the records say which events run on tiles (skipped here).
 template <bool VEC, bool BRICK>
 __global__ void __launch_bounds__(kBlock, 5)
-em_planned_kernel(RecPtrs rec, int nx, int ny, const uint2 *__restrict__ chunks, const uint32_t *__restrict__ index,
-                  uint32_t n_pieces, uint32_t n_index, const float *__restrict__ evw, const float *__restrict__ image,
-                  float *__restrict__ corr, DeviceStats *stats, unsigned *queues, unsigned nseg, unsigned per_seg,
-                  unsigned segs_per_sm) {
+em_planned_kernel(RecPtrs rec, uint64_t n, int nx, int ny, const uint32_t *__restrict__ pieces, uint32_t n_pieces,
+                  const float *__restrict__ evw, const float *__restrict__ image, float *__restrict__ corr,
+                  DeviceStats *stats, unsigned *queues, unsigned nseg, unsigned per_seg, unsigned segs_per_sm) {
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
@@ -438,18 +436,8 @@ em_planned_kernel(RecPtrs rec, int nx, int ny, const uint2 *__restrict__ chunks,
         }
         const uint64_t wc = (uint64_t)seg * per_seg + c;
         if (wc >= n_pieces) continue;
-        uint32_t e = 0;
-        bool have = false;
-        if (index) {
-            const uint64_t k = wc * 32u + lane;
-            have = k < n_index;
-            if (have) e = __ldg(index + k);
-        } else {
-            const uint2 ch = __ldg(chunks + wc);
-            have = lane < ch.y;
-            e = ch.x + lane;
-        }
-        if (!have) continue;
+        const uint64_t e = (uint64_t)__ldg(pieces + wc) * 32u + lane;
+        if (e >= n) continue;
         const uint4 rc = __ldcs(rec.c + e);
         // tile records never appear in these lists; the slivers (kRecTiny) have their own pass
         if ((rc.y & (kRecValid | kRecTile | kRecTiny)) != kRecValid) continue;
@@ -505,14 +493,14 @@ size_t plan_counter_bytes() { return sizeof(PlanCounters); }
 
 void launch_prepare_rays(const ProjParams &p, double sigma, const TileGeom *d_geom, int tile_log2, const EventPtrs &ev,
                          uint64_t n, const TileItem *items, const TileRange *ranges, uint32_t n_ranges,
-                         const RecPtrs &rec, uint32_t *stragglers, uint2 *tiny_list, uint32_t tiny_cap, void *d_counters,
+                         const RecPtrs &rec, uint32_t *chunk_flags, uint2 *tiny_list, uint32_t tiny_cap, void *d_counters,
                          cudaStream_t s) {
     if (n == 0) return;
     double kappa, qs, qi;
     plan_quantum(p, sigma, kappa, qs, qi);
     cudaMemsetAsync(d_counters, 0, sizeof(PlanCounters), s);
     prepare_rays_kernel<<<(unsigned)((n + kBlock - 1) / kBlock), kBlock, 0, s>>>(
-        p, d_geom, tile_log2, ev, n, items, ranges, d_geom ? n_ranges : 0u, qs, qi, rec, stragglers, tiny_list, tiny_cap,
+        p, d_geom, tile_log2, ev, n, items, ranges, d_geom ? n_ranges : 0u, qs, qi, rec, chunk_flags, tiny_list, tiny_cap,
         static_cast<PlanCounters *>(d_counters));
 }
 
@@ -535,9 +523,9 @@ void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &
 }
 
 template <bool VEC, bool BRICK>
-static void launch_planned(const ProjParams &p, const RecPtrs &rec, const uint2 *chunks, const uint32_t *index,
-                           uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
-                           DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s) {
+static void launch_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, const uint32_t *pieces, uint32_t n_pieces,
+                           const float *evw, const float *image, float *corr, DeviceStats *stats, unsigned *queues,
+                           int n_sm, cudaStream_t s) {
     int per_sm = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_planned_kernel<VEC, BRICK>, kBlock, 0);
     if (per_sm < 1) per_sm = 1;
@@ -549,20 +537,20 @@ static void launch_planned(const ProjParams &p, const RecPtrs &rec, const uint2 
     if (nseg % 61u == 0) nseg -= segs;
     const unsigned per_seg = (n_pieces + nseg - 1) / nseg;
     cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-    em_planned_kernel<VEC, BRICK><<<n_sm * per_sm, kBlock, 0, s>>>(rec, p.n[0], p.n[1], chunks, index, n_pieces, n_index,
-                                                                  evw, image, corr, stats, queues, nseg, per_seg, segs);
+    em_planned_kernel<VEC, BRICK><<<n_sm * per_sm, kBlock, 0, s>>>(rec, n, p.n[0], p.n[1], pieces, n_pieces, evw, image,
+                                                                  corr, stats, queues, nseg, per_seg, segs);
 }
 
-void launch_em_planned(const ProjParams &p, const RecPtrs &rec, const uint2 *chunks, const uint32_t *index,
-                       uint32_t n_pieces, uint32_t n_index, const float *evw, const float *image, float *corr,
-                       bool vec_ok, DeviceStats *stats, unsigned *queues, int n_sm, cudaStream_t s) {
-    if (n_pieces == 0) return;
+void launch_em_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, const uint32_t *pieces, uint32_t n_pieces,
+                       const float *evw, const float *image, float *corr, bool vec_ok, DeviceStats *stats,
+                       unsigned *queues, int n_sm, cudaStream_t s) {
+    if (n == 0 || n_pieces == 0) return;
     if (p.brick && vec_ok)
-        launch_planned<true, true>(p, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<true, true>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, s);
     else if (vec_ok)
-        launch_planned<true, false>(p, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<true, false>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, s);
     else
-        launch_planned<false, false>(p, rec, chunks, index, n_pieces, n_index, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<false, false>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, s);
 }
 
 }  // namespace tofmlem
