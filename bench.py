@@ -25,8 +25,9 @@ if ROOT not in sys.path:
 
 METRIC = "events/s per TOF-MLEM iteration (fwd+backproj)"
 # DRAM bytes of one launch of the dominant kernel at cfg-3 (ncu --set full; refresh with the capture)
-TRAFFIC_BYTES = 8.177348e9
-TRAFFIC_SOURCE = "profiles/r04_em_persistent_ncu_full_metrics.txt (6.894 GB read + 1.283 GB written per launch)"
+TRAFFIC_BYTES = 6.868e9
+TRAFFIC_SOURCE = ("profiles/r05_em_tile_ncu_full_metrics.txt: em_tile_kernel 6.411 GB read + 0.456 GB written per launch "
+                  "(algorithmic: 56 B x 97.9 M tile events = 5.48 GB of records + scale scratch)")
 UNIT = "events/s"
 
 
@@ -204,6 +205,7 @@ def run_report(args):
                 if fwhm <= 0:
                     ev["dt"].zero_()
                 ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
+                ctx.reserve(n)  # scratch of binning and plan: allocated outside the timed calls
                 sev, _, bin_ms = binned(ctx, ev, n)
                 del ev
                 plan_ms = timed(lambda: ctx.plan_events(sev, n)) if args.tile else 0.0  # inactive for non-TOF
@@ -355,6 +357,8 @@ def run_report(args):
             # on the binned events: neighbouring LORs are nearly parallel and close, so the mu-map gathers hit L1
             sw = torch.empty(kept, dtype=torch.float32, device=dev)
             stage("attenuation_weights", lambda: base.attenuation_weights(sev, kept, mu, sw))
+            if args.tile:
+                stage("plan_ray_records", lambda: base.plan_events(sev, kept))
             stage("mlem_20_iterations_with_median", lambda: base.iterate_weighted(sev, kept, sw, x, sens, iters))
             return kept, x
 
@@ -412,6 +416,9 @@ def run_report(args):
             base.em_correction_weighted(sev, n, sw, image, corr)
             base.update(image, corr, sens)
 
+        if args.tile:
+            base.reserve(n)
+            res["plan_events"] = {"ms": timed(lambda: base.plan_events(sev, n))}
         pass_w()
         ms = timed(pass_w, reps=3)
         res["weighted_iteration"] = {"ms": ms, "events_per_s": n / (ms * 1e-3)}

@@ -114,6 +114,9 @@ enum {
     TOFMLEM_OPT_TILE_MIN_EVENTS = 14, /* tofmlem_plan_events: a locality bin with at least this many events is
                                        accumulated in a shared-memory tile (default 1024; performance only) */
     TOFMLEM_OPT_TILE_MAX_EVENTS = 16, /* ... in pieces of at most this many events per CTA (default 8192) */
+    TOFMLEM_OPT_TILE_MIN_ITEMS = 20, /* tofmlem_plan_events: with fewer tile items than this the list is planned without tiles
+                                       (default -1: twice the number of tile CTAs the GPU holds at once -- fewer would
+                                       run on a fraction of the SMs before the direct pass starts; performance only) */
     TOFMLEM_OPT_TILE_CHECK = 15,    /* 1: bounds-test every access to the shared-memory tiles and count violations in
                                        tofmlem_stats.tile_oob (a debugging aid; default 0).  The plan has already
                                        dry-run every tile event against its tile, so the count must stay 0 */

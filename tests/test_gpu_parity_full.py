@@ -61,6 +61,7 @@ def test_full_grid_five_iterations_subsample(pkg, full_sens):
     # tile mode on every bin with >= 8 events (2 M events on 384 k bins are sparse; the default threshold is 1024),
     # every tile access bounds-tested
     ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 8)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)  # small test problems: tiles whatever the item count
     ctx.set_option(pkg.OPT_TILE_CHECK, 1)
     plan = ctx.plan_events(sev, n)
     assert plan.active and plan.sorted and plan.n_tile_events + plan.n_direct_events == n
@@ -191,6 +192,7 @@ def _tile_case(pkg, cfg, n, m, min_events, iters=2, expect_active=True, seed_img
     ctx.sensitivity(lors, m, sens)
     sev, _ = binned(ctx, ev, n)
     ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, min_events)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)  # small test problems: tiles whatever the item count
     ctx.set_option(pkg.OPT_TILE_CHECK, 1)
     plan = ctx.plan_events(sev, n)
     assert bool(plan.active) == expect_active, (plan.active, plan.sorted, plan.n_tile_items)
@@ -280,6 +282,7 @@ def test_tile_mode_anisotropic_voxels_and_weights(pkg):
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
     sev, perm = binned(ctx, ev, n)
     ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 32)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)  # small test problems: tiles whatever the item count
     ctx.set_option(pkg.OPT_TILE_CHECK, 1)
     ctx.set_option(pkg.OPT_CORR_BRICKS, 0)  # read the correction image directly (set before the plan: it is part of it)
     plan = ctx.plan_events(sev, n)
@@ -311,6 +314,7 @@ def test_plan_without_tiles_when_they_do_not_fit(pkg):
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
     sev, _ = binned(ctx, ev, n)
     ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 8)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)  # small test problems: tiles whatever the item count
     plan = ctx.plan_events(sev, n)
     assert plan.active and plan.n_tile_items == 0 and plan.n_tile_events == 0 and plan.n_direct_events == n
     img = synth.random_image((g.nvox,), 31, device="cuda")
@@ -359,6 +363,7 @@ def test_planned_forward_parity(pkg, case):
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, fwhm)
     sev, _ = binned(ctx, ev, n)
     ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, tmin)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)  # small test problems: tiles whatever the item count
     plan = ctx.plan_events(sev, n)
     assert plan.active
     if case in ("tiny", "full-100ps", "full-300ps", "aniso"):
