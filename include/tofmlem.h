@@ -132,9 +132,16 @@ enum {
                                        passes -- nine plans synchronise nine times, which costs more than five planned
                                        iterations save (measured: 184 vs 142 ms at cfg-4) */
     TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
-                                       generated an identically reconstructed image").  0 (default) is accepted; 1
-                                       returns TOFMLEM_EUNSUPPORTED: the correction image is summed with float32
-                                       reductions whose order is not fixed (run-to-run differences ~1e-7 relative) */
+                                       generated an identically reconstructed image").  1: the iterations of
+                                       tofmlem_iterate[_weighted] on a PLANNED list (tofmlem_plan_events; else
+                                       TOFMLEM_EUNSUPPORTED) round every contribution a_ej w_e / fwd_e to an integer number
+                                       of quanta -- a power of two fixed per iteration by max(image) alone, ~2^26 per
+                                       typical contribution, clamped at 2^48 -- and add it to a 64-bit integer correction
+                                       image: integer sums do not depend on the order of the events, so the image is the
+                                       same bit for bit in every run and for every ordering of the list.  About 2.5 x
+                                       the time of the default pass (scalar 64-bit reductions, no tiles).  0 (default):
+                                       float32 sums, order not fixed (run-to-run differences ~1e-7 relative).  TOF Siddon
+                                       projector only.  tofmlem_em_correction / tofmlem_iterate_host are not affected. */
     TOFMLEM_OPT_SUBBINS = 9         /* tofmlem_bin_events: order the events INSIDE each locality bin by predicted
                                        voxel-visit count, in `value` sub-bins (1..64, default 16; 1 = off), so that
                                        the events of a warp walk windows of nearly equal length.  Keys, bin offsets

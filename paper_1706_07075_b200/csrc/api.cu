@@ -63,6 +63,9 @@ struct tofmlem_ctx {
     uint64_t launches = 0;
     // tile-mode plan of the fused pass (tofmlem_plan_events; tile.cu)
     int tile_min_events = 1024, tile_max_events = 8192, tile_check = 0;
+    int deterministic = 0;        // TOFMLEM_OPT_DETERMINISTIC: integer accumulation (prepared.cu, em_det_kernel)
+    unsigned long long *d_corr_q = nullptr;  // its 64-bit correction image
+    float *d_gscale = nullptr;               // [0] quanta per unit, [1] its reciprocal, [2] max(image) of the pass
     int l2_persist = 1;           // TOFMLEM_OPT_L2_PERSIST
     const float *l2_ptr = nullptr;  // correction image the stream's access-policy window currently covers
     cudaStream_t l2_stream = nullptr;
@@ -487,13 +490,35 @@ int iterate_device(tofmlem_ctx *ctx, const EventPtrs &ev, uint64_t n, const floa
         launch_max_nonneg(d_sens, ctx->nvox, ctx->d_max, ctx->stream);
         CHECK_LAUNCH(1);
     }
+    const bool det = ctx->deterministic && n > 0 && iters > 0;
+    if (det) {
+        if (!plan_matches(ctx, ev.x1, n))
+            return fail(ctx, TOFMLEM_EUNSUPPORTED, "deterministic iterations need a planned list (tofmlem_plan_events)");
+        if (!ctx->d_corr_q) {
+            CU(cudaMalloc(&ctx->d_corr_q, ctx->nvox * sizeof(unsigned long long)));
+            CU(cudaMalloc(&ctx->d_gscale, 4 * sizeof(float)));
+        }
+        CU(cudaMemsetAsync(ctx->d_corr_q, 0, ctx->nvox * sizeof(unsigned long long), ctx->stream));
+    }
     CU(cudaMemsetAsync(ctx->d_corr, 0, ctx->nvox * sizeof(float), ctx->stream));
     for (int it = 0; it < iters; ++it) {
         CU(cudaMemsetAsync(ctx->d_stats, 0, kStatsCounters * sizeof(unsigned long long), ctx->stream));
-        rc = em_pass(ctx, p, ev, n, evw, d_image, ctx->d_corr, true, ctx->stream);
-        if (rc) return rc;
-        update_any(ctx, d_image, ctx->d_corr, d_sens, dmax, ctx->stream);
-        CHECK_LAUNCH(1);
+        if (det) {
+            // quanta per unit from max(image) alone (order-independent), integer pass, integer update
+            launch_max_nonneg(d_image, ctx->nvox, ctx->d_gscale + 2, ctx->stream);
+            launch_det_scale(ctx->d_gscale + 2, ctx->d_gscale, ctx->stream);
+            launch_em_det(p, ctx->d_rec, n, evw, d_image, ctx->d_corr_q, ctx->d_gscale, ctx->d_stats, ctx->d_queues,
+                          ctx->n_sm, ctx->stream);
+            launch_update_det(d_image, ctx->d_corr_q, d_sens, dmax, (float)ctx->sens_floor_rel, ctx->d_gscale, ctx->nvox,
+                              ctx->stream);
+            CHECK_LAUNCH(4);
+            ctx->t_have = 0;
+        } else {
+            rc = em_pass(ctx, p, ev, n, evw, d_image, ctx->d_corr, true, ctx->stream);
+            if (rc) return rc;
+            update_any(ctx, d_image, ctx->d_corr, d_sens, dmax, ctx->stream);
+            CHECK_LAUNCH(1);
+        }
         if (ctx->median) {  // the filter is applied to the image estimate after each iteration (R23)
             rc = median_in_place(ctx, d_image, ctx->stream);
             if (rc) return rc;
@@ -595,6 +620,8 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_ranges);
     if (ctx->h_hist_pinned) cudaFreeHost(ctx->h_hist_pinned);
     cudaFree(ctx->d_plan_counters);
+    cudaFree(ctx->d_corr_q);
+    cudaFree(ctx->d_gscale);
     for (auto &te : ctx->t_ev)
         if (te) cudaEventDestroy(te);
     free_records(ctx);
@@ -692,13 +719,13 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             ctx->region_plan = (int)value;
             return TOFMLEM_OK;
         case TOFMLEM_OPT_DETERMINISTIC:
-            // the paper's LUT kernel "always generated an identically reconstructed image".  Here the
-            // accumulation is a float32 reduction at L2 / in shared memory whose order is not fixed, so a run-to-run
-            // bit-identical image cannot be promised: the key exists, 0 is accepted, 1 is refused.
+            // the paper's LUT kernel "always generated an identically reconstructed image".  1: the
+            // iterations of tofmlem_iterate[_weighted] on a PLANNED list accumulate in 64-bit integers (prepared.cu,
+            // em_det_kernel): run-to-run bit-identical images.  The float32 paths stay unordered.
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "deterministic is 0 or 1");
-            if (value == 1.0)
-                return fail(ctx, TOFMLEM_EUNSUPPORTED,
-                            "deterministic accumulation is not available: float32 reductions are unordered");
+            if (value == 1.0 && (!ctx->tof || ctx->projector != 0))
+                return fail(ctx, TOFMLEM_EUNSUPPORTED, "deterministic accumulation exists for the TOF Siddon projector only");
+            ctx->deterministic = (int)value;
             return TOFMLEM_OK;
         default:
             return fail(ctx, TOFMLEM_EINVAL, "unknown option key");

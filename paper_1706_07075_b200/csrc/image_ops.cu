@@ -105,6 +105,39 @@ __global__ void __launch_bounds__(kBlock) update_brick_kernel(float *__restrict_
     }
 }
 
+// Reproducible accumulation (prepared.cu, em_det_kernel): quanta per unit of the correction image, a power of two fixed
+// by max(image) alone: a ray through max(image) everywhere contributes ~0.1 / max per voxel -> 2^26 quanta.
+__global__ void det_scale_kernel(const float *__restrict__ d_img_max, float *__restrict__ gscale) {
+    const float m = *d_img_max;
+    int e = 0;
+    if (m > 0.0f && m < 3.0e38f) e = ilogbf(0.1f / m);
+    e = max(-60, min(60, 26 - e));
+    gscale[0] = ldexpf(1.0f, e);
+    gscale[1] = ldexpf(1.0f, -e);
+}
+
+__global__ void __launch_bounds__(kBlock) update_det_kernel(float *__restrict__ image,
+                                                            unsigned long long *__restrict__ corr_q,
+                                                            const float *__restrict__ sens,
+                                                            const float *__restrict__ d_max, float floor_rel,
+                                                            const float *__restrict__ gscale, uint64_t n) {
+    const float thr = __fmul_rn(floor_rel, *d_max);
+    const double inv_g = (double)gscale[1];
+    const uint64_t stride = (uint64_t)gridDim.x * kBlock;
+    for (uint64_t i = (uint64_t)blockIdx.x * kBlock + threadIdx.x; i < n; i += stride) {
+        const float c = (float)((double)corr_q[i] * inv_g);
+        image[i] = update_one(image[i], c, __ldg(sens + i), thr);
+        corr_q[i] = 0ull;
+    }
+}
+
+void launch_det_scale(const float *d_img_max, float *gscale, cudaStream_t s) { det_scale_kernel<<<1, 1, 0, s>>>(d_img_max, gscale); }
+
+void launch_update_det(float *image, unsigned long long *corr_q, const float *sens, const float *d_max, float floor_rel,
+                       const float *gscale, uint64_t n, cudaStream_t s) {
+    if (n) update_det_kernel<<<grid_for(n), kBlock, 0, s>>>(image, corr_q, sens, d_max, floor_rel, gscale, n);
+}
+
 // x0 = mask (the harness' initial image, R15)
 __global__ void __launch_bounds__(kBlock) mask_init_kernel(float *__restrict__ image, const float *__restrict__ sens,
                                                            const float *__restrict__ d_max, float floor_rel,

@@ -130,7 +130,15 @@ void launch_em_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, cons
                        const float *evw, const float *image, float *corr, bool vec_ok, DeviceStats *stats,
                        unsigned *queues, int n_sm, cudaStream_t s);
 
+// reproducible accumulation (TOFMLEM_OPT_DETERMINISTIC): every event of the planned list, 64-bit integer correction image
+void launch_em_det(const ProjParams &p, const RecPtrs &rec, uint64_t n, const float *evw, const float *image,
+                   unsigned long long *corr_q, const float *gscale /* [0] quanta per unit */, DeviceStats *stats,
+                   unsigned *queues, int n_sm, cudaStream_t s);
+
 // ---- image_ops.cu
+void launch_det_scale(const float *d_img_max, float *gscale /* [2]: G, 1 / G */, cudaStream_t s);
+void launch_update_det(float *image, unsigned long long *corr_q, const float *sens, const float *d_max, float floor_rel,
+                       const float *gscale, uint64_t n, cudaStream_t s);
 void launch_max_nonneg(const float *x, uint64_t n, float *d_max /* zeroed by the call */, cudaStream_t s);
 void launch_update(float *image, float *corr, const float *sens, const float *d_max, float floor_rel, uint64_t n,
                    cudaStream_t s);

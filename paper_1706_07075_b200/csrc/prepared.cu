@@ -477,6 +477,95 @@ em_planned_kernel(RecPtrs rec, uint64_t n, int nx, int ny, const uint32_t *__res
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Reproducible accumulation (TOFMLEM_OPT_DETERMINISTIC; "This approach always generated an identically
+// reconstructed image").  Every contribution w_ej w_e / fwd_e is rounded to an integer number of quanta 1 / G and added
+// to a 64-bit integer correction image: integer additions commute, so the image does not depend on the order in which
+// the GPU happens to run the events.  The forward value of an event is summed by one thread in walk order (fixed).
+// G is a power of two fixed per pass from max(image) alone (image_ops.cu, det_scale_kernel), a contribution is clamped
+// to 2^48 quanta (fwd_e below ~2e-7 of what a ray through max(image) would see: the voxel's correction is huge either
+// way).  One thread per event on the ray records, every event through this kernel (no tiles: their flush order would
+// not matter either, but one code path keeps the mode simple); scalar 64-bit reductions, about 2.5 x the time of the
+// default pass.
+__global__ void __launch_bounds__(kBlock, 5)
+em_det_kernel(RecPtrs rec, uint64_t n, int nx, int ny, const float *__restrict__ evw, const float *__restrict__ image,
+              unsigned long long *__restrict__ corr_q, const float *__restrict__ gscale, DeviceStats *stats,
+              unsigned *queues, unsigned nseg, unsigned per_seg) {
+    unsigned smid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    const unsigned lane = threadIdx.x & 31u;
+    const float G = __ldg(gscale);
+    const uint64_t n_pieces = (n + 31u) >> 5;
+    unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0;
+    while (true) {
+        unsigned c = per_seg;
+        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= per_seg) {
+            if (++tries >= nseg) break;
+            seg = (seg + 61u) % nseg;
+            continue;
+        }
+        const uint64_t wc = (uint64_t)seg * per_seg + c;
+        if (wc >= n_pieces) continue;
+        const uint64_t e = wc * 32u + lane;
+        if (e >= n) continue;
+        const uint4 rc = __ldcs(rec.c + e);
+        if (!(rc.y & kRecValid)) continue;
+        RecRay r = rec_ray(__ldcs(rec.a + e), __ldcs(rec.b + e));
+        int i0, i1, i2;
+        rec_increments(rc, nx, ny, i0, i1, i2);
+        vis += rc.z & 0xFFFFu;
+        const float fw = rec_gather(r, (int)rc.x, i0, i1, i2, image);
+        if (!(fw > 0.0f)) continue;  // R9
+        ++nv;
+        const float sg = (evw ? __ldg(evw + e) : 1.0f) / fw * G;
+        auto put = [&](int at, float w) {
+            const float q = fminf(w * sg, 281474976710656.0f);  // 2^48
+            atomicAdd(corr_q + at, (unsigned long long)__float2ll_rn(q));
+        };
+        int at = (int)rc.x;
+        float t = r.t;
+        while (true) {
+            const float tn = min3f(r.tx, r.ty, r.tz);
+            if (!(tn < r.te)) break;
+            put(at, chord_weight(t, tn));
+            advance_axis(r.tx, at, tn, r.dx, i0);
+            advance_axis(r.ty, at, tn, r.dy, i1);
+            advance_axis(r.tz, at, tn, r.dz, i2);
+            t = tn;
+        }
+        put(at, chord_weight(t, r.te));
+    }
+    nv = __reduce_add_sync(0xffffffffu, nv);
+    vis = __reduce_add_sync(0xffffffffu, vis);
+    if (lane == 0 && stats) {
+        if (nv) atomicAdd(&stats->n_valid, (unsigned long long)nv);
+        if (vis) {
+            atomicAdd(&stats->visits, (unsigned long long)vis);
+            atomicAdd(&stats->reds, (unsigned long long)vis);
+        }
+    }
+}
+
+void launch_em_det(const ProjParams &p, const RecPtrs &rec, uint64_t n, const float *evw, const float *image,
+                   unsigned long long *corr_q, const float *gscale, DeviceStats *stats, unsigned *queues, int n_sm,
+                   cudaStream_t s) {
+    if (n == 0) return;
+    int per_sm = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_det_kernel, kBlock, 0);
+    if (per_sm < 1) per_sm = 1;
+    if (n_sm < 1) n_sm = 1;
+    unsigned nseg = (unsigned)n_sm;
+    if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues;
+    if (nseg % 61u == 0) nseg -= 1;
+    const uint64_t n_pieces = (n + 31) / 32;
+    const unsigned per_seg = (unsigned)((n_pieces + nseg - 1) / nseg);
+    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    em_det_kernel<<<n_sm * per_sm, kBlock, 0, s>>>(rec, n, p.n[0], p.n[1], evw, image, corr_q, gscale, stats, queues, nseg,
+                                                   per_seg);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Host side.
 
 void plan_quantum(const ProjParams &p, double sigma, double &kappa, double &qs, double &qi) {

@@ -167,19 +167,61 @@ def test_context_reuse_growing_and_shrinking_n(pkg):
     assert torch.zeros(1, device="cuda").item() == 0.0
 
 
-def test_deterministic_option_is_declared_and_refused(pkg):
-    """SURVEY.md 8(b) lists a `deterministic` key.  It exists; 0 is accepted, 1 is refused with
-    TOFMLEM_EUNSUPPORTED (float32 reductions are unordered)."""
+def test_deterministic_iterations_are_bit_identical(pkg):
+    """SURVEY.md 8(b) `deterministic` key ("This approach always generated an identically reconstructed
+    image"): with the option on, the iterations of a planned list accumulate in 64-bit integers -- two runs give the same
+    bits, whatever order the GPU ran the events in, and the image still matches oracle.mlem within north_star's tolerance.
+    Unplanned lists, non-TOF contexts and bad values are refused."""
     cfg = synth.TINY
-    g, _ = grids(pkg, cfg)
+    n, m, iters = 120_000, 400_000, 3
+    g, og = grids(pkg, cfg)
+    ev = synth.make_events(cfg, n, device="cuda")
+    lors = synth.make_sens_lors(cfg, m, device="cuda")
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    sens = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.sensitivity(lors, m, sens)
+    sev, _ = binned(ctx, ev, n)
+    sens_np = sens.cpu().numpy()
+    mask = oracle.mask_f32(sens_np)
     ctx.set_option(pkg.OPT_DETERMINISTIC, 0)
-    with pytest.raises(pkg.TofMlemError) as e:
-        ctx.set_option(pkg.OPT_DETERMINISTIC, 1)
-    assert e.value.code == -5
     with pytest.raises(pkg.TofMlemError) as e:
         ctx.set_option(pkg.OPT_DETERMINISTIC, 2)
     assert e.value.code == -1
+    ctx.set_option(pkg.OPT_DETERMINISTIC, 1)
+    x = torch.from_numpy(mask.astype(np.float32)).cuda()
+    with pytest.raises(pkg.TofMlemError) as e:  # no plan yet
+        ctx.iterate(sev, n, x, sens, iters)
+    assert e.value.code == -5
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 64)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)
+    assert ctx.plan_events(sev, n).active
+    runs = []
+    for _ in range(3):
+        x = torch.from_numpy(mask.astype(np.float32)).cuda()
+        ctx.iterate(sev, n, x, sens, iters)
+        runs.append(x.clone())
+    assert torch.equal(runs[0], runs[1]) and torch.equal(runs[0], runs[2])
+    st = ctx.get_stats()
+    ref, ost = oracle.mlem(og, oracle.sigma_mm(cfg.tof_fwhm_ps), to_np(ev), mask.astype(np.float64), sens_np, iters)
+    l2, mx = check_image(runs[0].cpu().numpy(), ref, zero_tol=1e-6)
+    print(f"deterministic mode: rel-L2 {l2:.2e}, max rel {mx:.2e} against the oracle")
+    assert st.n_valid == ost.n_valid and st.tile_events == 0
+    assert abs(st.sum_image_sens - st.n_valid) / st.n_valid < 1e-5  # P7
+    # the same list in another order (a different plan, other thread-to-event mapping): still the same bits
+    rev = {k: v.flip(0).contiguous() for k, v in sev.items()}
+    assert ctx.plan_events(rev, n).active
+    x = torch.from_numpy(mask.astype(np.float32)).cuda()
+    ctx.iterate(rev, n, x, sens, iters)
+    assert torch.equal(x, runs[0])
+    # the default mode on the same plan stays within tolerance of it (float32 sums, order not fixed)
+    ctx.set_option(pkg.OPT_DETERMINISTIC, 0)
+    x = torch.from_numpy(mask.astype(np.float32)).cuda()
+    ctx.iterate(rev, n, x, sens, iters)
+    assert float((x - runs[0]).double().norm() / runs[0].double().norm()) < 1e-4
+    nt = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, 0.0)
+    with pytest.raises(pkg.TofMlemError) as e:
+        nt.set_option(pkg.OPT_DETERMINISTIC, 1)
+    assert e.value.code == -5
 
 
 # ------------------------------------------------------------------ tile mode (tofmlem_plan_events, tile.cu)
