@@ -70,6 +70,8 @@ struct tofmlem_ctx {
     const float *l2_ptr = nullptr;  // correction image the stream's access-policy window currently covers
     cudaStream_t l2_stream = nullptr;
     int region_overlap = 0;  // reading R27: an event goes to every region its window meets (TOFMLEM_OPT_REGION_OVERLAP)
+    int sens_sort = 0;            // TOFMLEM_OPT_SENS_SORT: tofmlem_sensitivity orders the LORs by locality and chord length
+    bool bin_whole_chords = false;  // tofmlem_bin_events: sub-bins by the visits of the WHOLE chord (non-TOF walks)
     int tile_min_items = -1;  // TOFMLEM_OPT_TILE_MIN_ITEMS (-1: twice the number of tile CTAs the GPU holds)
     int region_plan = 0;  // tofmlem_reconstruct_regions plans every region's list (TOFMLEM_OPT_REGION_PLAN)
     int n_sm = 0;
@@ -690,6 +692,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             if (value < 32 || value > 1e9 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "tile_max_events in 32..1e9");
             ctx->tile_max_events = (int)value;
             return TOFMLEM_OK;
+        case TOFMLEM_OPT_SENS_SORT:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "sens_sort is 0 or 1");
+            ctx->sens_sort = (int)value;
+            return TOFMLEM_OK;
         case TOFMLEM_OPT_TILE_MIN_ITEMS:
             if (value < -1 || value > 1e9 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "tile_min_items in -1..1e9");
             ctx->tile_min_items = (int)value;
@@ -785,7 +791,40 @@ int tofmlem_sensitivity(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t m
     CU(cudaMemsetAsync(d_sens, 0, ctx->nvox * sizeof(float), ctx->stream));
     EventPtrs ev = ev_ptrs(lors);
     ev.dt = nullptr;
+    // Random detector pairs give chords of 0 .. 900 voxels side by side in a warp (ncu r05: 11 of 32 lanes active, the
+    // sensitivity image written back to DRAM 700 times).  Order the LORs first: locality key of the chord's midpoint,
+    // sub-bins by the chord's visit count (the binning of a1 with dt = 0 and whole-chord sub-bins), 32 B per LOR of scratch
+    // for the duration of the call.  The result is the same up to the order of the float32 sums.
+    uint32_t *d_key = nullptr, *d_perm = nullptr;
+    float *d_sorted = nullptr;
+    if (ctx->sens_sort && m >= (1u << 18)) {
+        const uint64_t stride = (m + 3) & ~3ull;
+        if (cudaMalloc(&d_key, m * sizeof(uint32_t)) == cudaSuccess && cudaMalloc(&d_perm, m * sizeof(uint32_t)) == cudaSuccess &&
+            cudaMalloc(&d_sorted, 6 * stride * sizeof(float)) == cudaSuccess) {
+            tofmlem_events in = *lors;
+            in.dt = nullptr;
+            tofmlem_events_mut out{d_sorted, d_sorted + stride, d_sorted + 2 * stride, d_sorted + 3 * stride,
+                                   d_sorted + 4 * stride, d_sorted + 5 * stride, nullptr};
+            ctx->bin_whole_chords = true;
+            int rc = tofmlem_bin_events(ctx, &in, m, d_key, d_perm, nullptr);
+            ctx->bin_whole_chords = false;
+            if (rc == TOFMLEM_OK) rc = tofmlem_permute_events(ctx, &in, d_perm, m, &out);
+            if (rc == TOFMLEM_OK) {
+                ev = EventPtrs{out.x1, out.y1, out.z1, out.x2, out.y2, out.z2, nullptr};
+            } else {
+                cudaGetLastError();
+            }
+        } else {
+            cudaGetLastError();  // not enough memory for the scratch: the LORs as they come
+        }
+    }
     launch_backproject(p, false, ev, m, nullptr, d_sens, vec_ok(ctx, d_sens), ctx->stream);
+    if (d_key || d_perm || d_sorted) {
+        cudaStreamSynchronize(ctx->stream);
+        cudaFree(d_key);
+        cudaFree(d_perm);
+        cudaFree(d_sorted);
+    }
     CHECK_LAUNCH(1);
     launch_scale(d_sens, (float)(1.0 / (double)m), ctx->nvox, ctx->stream);
     CHECK_LAUNCH(1);
@@ -1220,12 +1259,13 @@ int tofmlem_bin_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, u
     if (rc) return rc;
     SubBin sb;
     sb.S = S;
-    sb.half_window = ctx->tof ? (float)(ctx->trunc_sigmas * ctx->sigma) : 0.0f;
+    const bool tof_window = ctx->tof && !ctx->bin_whole_chords;
+    sb.half_window = tof_window ? (float)(ctx->trunc_sigmas * ctx->sigma) : 0.0f;
     {
         // largest visit count of a window: its length times the l1 norm of u / v, plus the first voxel
         const tofmlem_grid &g = ctx->grid;
         const double diag = sqrt(pow(g.nx * (double)g.vx, 2) + pow(g.ny * (double)g.vy, 2) + pow(g.nz * (double)g.vz, 2));
-        const double len = ctx->tof ? fmin(2.0 * sb.half_window, diag) : diag;
+        const double len = tof_window ? fmin(2.0 * sb.half_window, diag) : diag;
         const double vmax = fmin(len * sqrt(1.0 / (g.vx * g.vx) + 1.0 / (g.vy * g.vy) + 1.0 / (g.vz * g.vz)) + 3.0,
                                  (double)g.nx + g.ny + g.nz);
         sb.quantum = S > 2 ? (uint32_t)fmax(1.0, ceil(vmax / (double)(S - 2))) : 1u << 30;

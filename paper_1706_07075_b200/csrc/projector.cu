@@ -335,14 +335,26 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         // 9.44 / 9.32 ms).  Long walks (600 ps: 43.3 -> 45.1 ms, non-TOF: 203 -> 218 ms with 2) keep one.
         const double reach = 2.0 * p.half_window * sqrt(p.iv[0] * p.iv[0] + p.iv[1] * p.iv[1] + p.iv[2] * p.iv[2]);
         const unsigned kSegsPerSm = !TOF || reach > 80.0 ? 1u : (reach > 30.0 ? 3u : 4u);  // reach = largest visit count
-        unsigned nseg = (unsigned)n_sm * kSegsPerSm;
-        if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / kSegsPerSm * kSegsPerSm;
-        if (nseg % 61u == 0) nseg -= kSegsPerSm;  // the stealing stride 61 must not divide the number of segments
+        unsigned segs = kSegsPerSm;
+        unsigned nseg = (unsigned)n_sm * segs;
+        unsigned grid = (unsigned)n_sm * (unsigned)(per_sm > 0 ? per_sm : 1);
         const uint64_t wchunks = chunks ? (uint64_t)n_chunks : (n + 31) / 32;
+        if (wchunks < 8ull * nseg) {
+            // a short list (the sliver windows of a planned list: a few thousand one-event pieces): a few queues and CTAs
+            // only -- a full-size launch spends 0.26 ms polling 444 empty queues
+            segs = 1;
+            nseg = (unsigned)((wchunks + 7) / 8);
+            if (nseg > (unsigned)n_sm) nseg = (unsigned)n_sm;
+            if (nseg < 1) nseg = 1;
+            const unsigned want = (unsigned)((wchunks * 32 + kBlock - 1) / kBlock);
+            if (want < grid) grid = want < 1 ? 1 : want;
+        }
+        if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / segs * segs;
+        if (nseg > segs && nseg % 61u == 0) nseg -= segs;  // the stealing stride 61 must not divide the number of segments
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
         cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
-        em_persistent_kernel<TOF, VEC, BRICK><<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(
-            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, kSegsPerSm, chunks, n_chunks);
+        em_persistent_kernel<TOF, VEC, BRICK><<<grid, kBlock, 0, s>>>(
+            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, segs, chunks, n_chunks);
     } else {
         em_correction_kernel<TOF, VEC, BRICK><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
     }

@@ -122,6 +122,19 @@ def test_backproject_parity_tiny(pkg, tiny):
     check_image(out.cpu().numpy(), ref2, l2=1e-5, mx=1e-4)
 
 
+def test_sensitivity_sorted_lors_same_image(pkg, tiny, tiny_sens):
+    """TOFMLEM_OPT_SENS_SORT: the LORs ordered by locality key and chord length inside the call give the same image (up
+    to the order of the float32 sums)."""
+    cfg, ev, ev_np, g, og, _ = tiny
+    lors, sens = tiny_sens
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ctx.set_option(pkg.OPT_SENS_SORT, 1)
+    s2 = torch.empty_like(sens)
+    ctx.sensitivity(lors, cfg.sens_lors, s2)
+    d = float((s2.double() - sens.double()).norm() / sens.double().norm())
+    assert d < 1e-6, d
+
+
 def test_sensitivity_parity_tiny(pkg, tiny, tiny_sens):
     cfg, ev, ev_np, g, og, ctx = tiny
     lors, sens = tiny_sens
