@@ -480,6 +480,7 @@ def main():
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next", "pipeline"],
                     help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
                          "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
+    ap.add_argument("--concurrent", type=int, default=-1, help="TOFMLEM_OPT_CONCURRENT override")
     ap.add_argument("--l2-persist", type=int, default=-1, help="TOFMLEM_OPT_L2_PERSIST override")
     ap.add_argument("--region-plan", type=int, default=-1, help="TOFMLEM_OPT_REGION_PLAN override (division report)")
     ap.add_argument("--sweep-events", default="10000000,146000000,500000000")
@@ -519,6 +520,8 @@ def main():
         ctx.set_option(pkg.OPT_CACHE_SHARE, args.cache_share)
     if args.l2_persist >= 0:
         ctx.set_option(pkg.OPT_L2_PERSIST, args.l2_persist)
+    if args.concurrent >= 0:
+        ctx.set_option(pkg.OPT_CONCURRENT, args.concurrent)
     nvox = g.nvox
 
     def timed(fn):

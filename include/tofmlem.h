@@ -114,6 +114,9 @@ enum {
     TOFMLEM_OPT_TILE_MIN_EVENTS = 14, /* tofmlem_plan_events: a locality bin with at least this many events is
                                        accumulated in a shared-memory tile (default 1024; performance only) */
     TOFMLEM_OPT_TILE_MAX_EVENTS = 16, /* ... in pieces of at most this many events per CTA (default 8192) */
+    TOFMLEM_OPT_CONCURRENT = 22,    /* planned fused pass: k > 0 runs the direct pass on records on a second stream BESIDE the tile
+                                       pass, the tile pass limited to k CTAs per SM (0, the default: one after the
+                                       other).  Performance only. */
     TOFMLEM_OPT_SENS_SORT = 21,     /* 1: tofmlem_sensitivity orders the LORs by locality key and chord length first (32 B per
                                        LOR of scratch during the call; from 2^18 LORs on); 0 (default): as they come.
                                        Performance only (the image is the same up to the order of the float32 sums);

@@ -106,6 +106,9 @@ struct tofmlem_ctx {
         cudaEvent_t ready = nullptr;
     } rgc;
     cudaEvent_t t_ev[4] = {nullptr, nullptr, nullptr, nullptr};  // tofmlem_pass_timing: around the planned kernels
+    int concurrent = 0;            // TOFMLEM_OPT_CONCURRENT: tile CTAs per SM while the direct pass runs beside them
+    cudaStream_t side_stream = nullptr;
+    cudaEvent_t fork_ev = nullptr, join_ev = nullptr;
     int t_have = 0;                                              // bit k: part k of the last planned pass ran
     struct {
         bool valid = false;
@@ -443,26 +446,47 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         if (!ctx->t_ev[0])
             for (auto &te : ctx->t_ev) CU(cudaEventCreate(&te));
         ctx->t_have = (ctx->plan.n_items ? 1 : 0) | (ctx->plan.direct_valid ? 2 : 0) | (ctx->plan.n_tiny ? 4 : 0);
+        // TOFMLEM_OPT_CONCURRENT = k > 0: the direct pass (bound by L2 reduction requests, issue slots half idle) on a
+        // second stream beside the tile pass (issue-bound, L2 idle), the tile pass limited to k CTAs per SM so that CTAs
+        // of both fit an SM.  Both only add to the correction image and to the counters.
+        cudaStream_t ds = s;
+        const bool conc = ctx->concurrent > 0 && ctx->plan.n_items && ctx->plan.direct_valid;
+        if (conc) {
+            if (!ctx->side_stream) {
+                CU(cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking));
+                CU(cudaEventCreateWithFlags(&ctx->fork_ev, cudaEventDisableTiming));
+                CU(cudaEventCreateWithFlags(&ctx->join_ev, cudaEventDisableTiming));
+            }
+            ds = ctx->side_stream;
+            CU(cudaEventRecord(ctx->fork_ev, s));
+            CU(cudaStreamWaitEvent(ds, ctx->fork_ev, 0));
+        }
         CU(cudaEventRecord(ctx->t_ev[0], s));
         if (ctx->plan.n_items) {
             TileGeom g;
             build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, ctx->smem_per_sm, g);  // as at plan time (sigma, trunc match)
             launch_em_tile(p, g, ctx->d_geom, ctx->tile_log2, ctx->d_rec, evw, d_image, d_corr, ctx->d_stats,
                            ctx->d_items, ctx->plan.n_items, ctx->d_plan_flags, n_sm, ctx->smem_per_sm,
-                           ctx->tile_check != 0, ctx->sigma, ctx->plan.max_item_events, ctx->d_ev_scale, s);
+                           ctx->tile_check != 0, ctx->sigma, ctx->plan.max_item_events, ctx->d_ev_scale,
+                           conc ? ctx->concurrent : 0, s);
             CHECK_LAUNCH(1);
         }
         CU(cudaEventRecord(ctx->t_ev[1], s));
         if (ctx->plan.direct_valid) {
             launch_em_planned(p, ctx->d_rec, n, ctx->d_chunk_list, ctx->plan.n_pieces, evw, d_image, d_corr, vec,
-                              ctx->d_stats, ctx->d_queues, n_sm, s);
+                              ctx->d_stats, ctx->d_queues, n_sm, ds);
             CHECK_LAUNCH(1);
         }
-        CU(cudaEventRecord(ctx->t_ev[2], s));
+        if (!conc) CU(cudaEventRecord(ctx->t_ev[2], s));
         if (ctx->plan.n_tiny) {  // kRecTiny: the unplanned walk (fp64 set-up), one event per piece
             launch_em_correction_chunks(p, true, ev, n, ctx->d_tiny, ctx->plan.n_tiny, evw, d_image, d_corr, vec,
-                                        ctx->d_stats, ctx->d_queues, s);
+                                        ctx->d_stats, ctx->d_queues, ds);
             CHECK_LAUNCH(1);
+        }
+        if (conc) {
+            CU(cudaEventRecord(ctx->join_ev, ds));
+            CU(cudaStreamWaitEvent(s, ctx->join_ev, 0));
+            CU(cudaEventRecord(ctx->t_ev[2], s));  // [1] -> [2]: what the direct pass added after the tile pass ended
         }
         CU(cudaEventRecord(ctx->t_ev[3], s));
         return TOFMLEM_OK;
@@ -624,6 +648,12 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_plan_counters);
     cudaFree(ctx->d_corr_q);
     cudaFree(ctx->d_gscale);
+    if (ctx->side_stream) {
+        cudaStreamSynchronize(ctx->side_stream);
+        cudaStreamDestroy(ctx->side_stream);
+        cudaEventDestroy(ctx->fork_ev);
+        cudaEventDestroy(ctx->join_ev);
+    }
     for (auto &te : ctx->t_ev)
         if (te) cudaEventDestroy(te);
     free_records(ctx);
@@ -691,6 +721,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
         case TOFMLEM_OPT_TILE_MAX_EVENTS:
             if (value < 32 || value > 1e9 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "tile_max_events in 32..1e9");
             ctx->tile_max_events = (int)value;
+            return TOFMLEM_OK;
+        case TOFMLEM_OPT_CONCURRENT:
+            if (value < 0 || value > 4 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "concurrent in 0..4");
+            ctx->concurrent = (int)value;
             return TOFMLEM_OK;
         case TOFMLEM_OPT_SENS_SORT:
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "sens_sort is 0 or 1");

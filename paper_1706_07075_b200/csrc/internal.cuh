@@ -108,7 +108,7 @@ void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_ge
                     uint32_t n_items, unsigned *counter /* one word, zeroed by the call */, int n_sm,
                     size_t smem_per_sm, bool check, double sigma, uint32_t max_item_events /* no item holds more */,
                     float *ev_scale /* one float per event of the list: scratch between the two phases */,
-                    cudaStream_t s);
+                    int cap_ctas /* > 0: at most this many CTAs per SM */, cudaStream_t s);
 
 // ---- prepared.cu: ray records of a planned list and the passes that run on them
 // Writes one record per event (p.brick says which group count the direct records carry), one flag per 32-event piece of

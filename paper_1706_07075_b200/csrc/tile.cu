@@ -536,6 +536,7 @@ struct TileLaunch {
     int n_sm;
     FixedPoint fx;
     float *ev_scale;
+    int cap_ctas;  // > 0: at most this many CTAs per SM (the direct pass shares the SMs)
     cudaStream_t s;
 };
 
@@ -544,7 +545,7 @@ static void launch_tile(const TileLaunch &L) {
     auto k = em_tile_kernel<NT, NCTA, BRICK, CHECK>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
     cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    const uint32_t cap = (uint32_t)L.n_sm * NCTA;
+    const uint32_t cap = (uint32_t)L.n_sm * (uint32_t)(L.cap_ctas > 0 && L.cap_ctas < NCTA ? L.cap_ctas : NCTA);
     k<<<L.n_items < cap ? L.n_items : cap, NT, L.smem, L.s>>>(L.p.n[0], L.p.n[1], L.p.n[2], L.d_geom, L.tile_log2, L.rec,
                                                               L.evw, L.image, L.corr, L.stats, L.items, L.n_items,
                                                               L.counter, L.fx, L.ev_scale);
@@ -562,7 +563,7 @@ static void launch_tile_cfg(const TileLaunch &L, bool check) {
 void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_geom, int tile_log2, const RecPtrs &rec,
                     const float *evw, const float *image, float *corr, DeviceStats *stats, const TileItem *items,
                     uint32_t n_items, unsigned *counter, int n_sm, size_t smem_per_sm, bool check, double sigma,
-                    uint32_t max_item_events, float *ev_scale, cudaStream_t s) {
+                    uint32_t max_item_events, float *ev_scale, int cap_ctas, cudaStream_t s) {
     if (n_items == 0) return;
     cudaMemsetAsync(counter, 0, sizeof(unsigned), s);
     FixedPoint fx;
@@ -577,7 +578,7 @@ void launch_em_tile(const ProjParams &p, const TileGeom &g, const TileGeom *d_ge
     }
     const size_t smem = tile_smem_bytes(g);
     const TileLaunch L{p, d_geom, smem, tile_log2, rec, evw, image, corr, stats, items, n_items, counter, n_sm, fx,
-                       ev_scale, s};
+                       ev_scale, cap_ctas, s};
     // CTAs per SM by shared memory; threads so that 56 registers fit
     const int ncta = tile_ctas_per_sm(smem, smem_per_sm);
     if (ncta >= 4) launch_tile_cfg<256, 4>(L, check);
