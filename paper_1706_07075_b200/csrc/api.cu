@@ -1,9 +1,7 @@
 // api.cu -- the C ABI of libtofmlem (include/tofmlem.h): context, argument checks, stream orchestration.
 #include <math.h>
 #include <stdio.h>
-#include <stdlib.h>
 #include <string.h>
-#include <time.h>
 
 #include <algorithm>
 #include <new>
@@ -1106,9 +1104,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         int rc0 = ensure_plan_scratch(ctx, n);
         if (rc0) return rc0;
     }
-    const bool ptime = getenv("TOFMLEM_PLAN_TIMING") != nullptr;
-    auto now = [&]() { cudaStreamSynchronize(s); struct timespec ts; clock_gettime(CLOCK_MONOTONIC, &ts); return ts.tv_sec * 1e3 + ts.tv_nsec * 1e-6; };
-    double tp0 = ptime ? now() : 0.0, tp1 = 0, tp2 = 0, tp3 = 0, tp4 = 0;
     // ---- which bins become tile items?  Needs a list sorted by key (tofmlem_permute_events) and tiles that fit.
     std::vector<TileItem> items;
     std::vector<TileRange> ranges;
@@ -1127,7 +1122,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMemcpyAsync(ctx->h_hist_pinned, ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
         CU(cudaMemcpyAsync(flags, ctx->d_plan_flags, sizeof flags, cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
-        if (ptime) tp1 = now();
         sorted = flags[1] == 0;
         if (sorted) {
             // Tile items: a bin with at least tile_min_events events (pieces of at most tile_max_events, whole warps), or
@@ -1188,7 +1182,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         const size_t min_items = ctx->tile_min_items >= 0 ? (size_t)ctx->tile_min_items : auto_min;
         if (items.size() < min_items) items.clear();
     }
-    if (ptime) tp2 = now();
     ctx->plan.sorted = sorted ? 1 : 0;
     if (items.empty()) {  // no tiles (window too wide, unsorted list, sparse bins): the whole list in order
         ranges.clear();
@@ -1218,7 +1211,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMemcpyAsync(ctx->d_items, items.data(), items.size() * sizeof(TileItem), cudaMemcpyHostToDevice, s));
         CU(cudaMemcpyAsync(ctx->d_ranges, ranges.data(), ranges.size() * sizeof(TileRange), cudaMemcpyHostToDevice, s));
     }
-    if (ptime) tp3 = now();
     // ---- the records: fp64 set-up, quantisation, dry run against the tile (prepared.cu)
     launch_prepare_rays(p, ctx->sigma, items.empty() ? nullptr : ctx->d_geom, ctx->tile_log2, ev_ptrs(ev), n, ctx->d_items,
                         ctx->d_ranges, (uint32_t)ranges.size(), ctx->d_rec, ctx->d_chunk_flags, ctx->d_tiny, kTinyCap,
@@ -1235,11 +1227,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
     std::vector<unsigned char> hc(plan_counter_bytes());
     CU(cudaMemcpyAsync(hc.data(), ctx->d_plan_counters, hc.size(), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
-    if (ptime) {
-        tp4 = now();
-        fprintf(stderr, "plan timing: hist+copy %.2f ms, host items %.2f ms, alloc+upload %.2f ms, prepare %.2f ms\n", tp1 - tp0,
-                tp2 - tp1, tp3 - tp2, tp4 - tp3);
-    }
     uint64_t cnt4[5];
     read_plan_counters(hc.data(), cnt4);
     if (cnt4[4] > kTinyCap) return TOFMLEM_OK;  // a list made of slivers: not worth a plan (stays inactive)

@@ -420,3 +420,78 @@ def test_planned_forward_parity(pkg, case):
     print(f"{case}: planned forward max rel err {err.max():.2e}, tile events {plan.n_tile_events} of {n}")
     assert err.max() <= FWD_RTOL, f"max rel err {err.max():.3e} at {err.argmax()}"
     assert (fwd.cpu().numpy()[ref == 0] == 0).all()
+
+
+def test_planned_path_edge_cases(pkg):
+    """The planned path on awkward inputs: ragged sizes, a list that grows and shrinks on one context, all-invalid
+    events, odd grid sizes (no 16-byte groups, no bricks), per-event weights, iters = 0, trim between plans."""
+    cfg = synth.TINY
+    g, og = grids(pkg, cfg)
+    sig = oracle.sigma_mm(cfg.tof_fwhm_ps)
+    ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 40)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)
+    ctx.set_option(pkg.OPT_TILE_CHECK, 1)
+    img = synth.random_image((g.nvox,), 3, device="cuda")
+    img_np = img.cpu().numpy().astype(np.float64)
+    for n in (100_003, 33, 250_001, 31):  # grows, shrinks, not multiples of 32
+        ev = synth.make_events(cfg, n, start=1000, device="cuda")
+        sev, _ = binned(ctx, ev, n)
+        plan = ctx.plan_events(sev, n)
+        assert plan.active and plan.n_tile_events + plan.n_direct_events == n
+        corr = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+        ctx.set_option(pkg.OPT_CORR_BRICKS, 0)
+        ctx.plan_events(sev, n)
+        ctx.reset_stats()
+        ctx.em_correction(sev, n, img, corr)
+        st = ctx.get_stats()
+        ref, nv, vis = oracle.em_correction(og, sig, to_np(sev), img_np)
+        assert st.n_valid == nv and st.tile_oob == 0
+        if n > 1000:
+            assert st.tile_events > 0
+            check_image(corr.cpu().numpy(), ref, l2=2e-4, mx=5e-3, zero_tol=1e-6)
+        else:
+            assert float((corr.double().cpu() - torch.from_numpy(ref)).norm() / np.linalg.norm(ref)) < 1e-4
+        ctx.set_option(pkg.OPT_CORR_BRICKS, 1)
+    # all events invalid: the plan is active, nothing is walked
+    n = 5000
+    bad = {k: torch.full((n,), float("nan"), device="cuda") for k in ("x1", "y1", "z1", "x2", "y2", "z2", "dt")}
+    plan = ctx.plan_events(bad, n)
+    assert plan.active and plan.n_tile_events == 0
+    corr = torch.zeros(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.reset_stats()
+    ctx.em_correction(bad, n, img, corr)
+    assert ctx.get_stats().n_valid == 0 and float(corr.abs().max()) == 0.0
+    assert ctx.plan_events(bad, 0).active == 0  # empty list: no plan, no error
+    # trim drops plan and scratch; planning again works
+    ctx.trim()
+    ev = synth.make_events(cfg, 20_000, device="cuda")
+    sev, _ = binned(ctx, ev, 20_000)
+    assert ctx.plan_events(sev, 20_000).active
+    x = torch.ones(g.nvox, dtype=torch.float32, device="cuda")
+    sens = torch.ones(g.nvox, dtype=torch.float32, device="cuda")
+    x0 = x.clone()
+    ctx.iterate(sev, 20_000, x, sens, 0)  # no iteration: the image is untouched
+    assert torch.equal(x, x0)
+    # odd grid sizes: no brick layout, nvox not a multiple of 4 (scalar reductions), tiles all the same
+    g2 = pkg.make_grid(31, 29, 27, 4.0)
+    og2 = oracle.make_grid(31, 29, 27, 4.0)
+    ctx2 = pkg.Context(cfg.radius_mm, cfg.axial_mm, g2, cfg.tof_fwhm_ps)
+    ctx2.set_option(pkg.OPT_TILE_MIN_EVENTS, 40)
+    ctx2.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)
+    ctx2.set_option(pkg.OPT_TILE_CHECK, 1)
+    n = 80_000
+    ev = synth.make_events(cfg, n, device="cuda")
+    sev, perm = binned(ctx2, ev, n)
+    w = (0.25 + torch.rand(n, generator=torch.Generator().manual_seed(5))).cuda()
+    sw = torch.empty_like(w)
+    ctx2.gather_f32(w, perm, n, sw)
+    assert ctx2.plan_events(sev, n).n_tile_events > 0
+    img2 = synth.random_image((g2.nvox,), 9, device="cuda")
+    corr2 = torch.zeros(g2.nvox, dtype=torch.float32, device="cuda")
+    ctx2.reset_stats()
+    ctx2.em_correction_weighted(sev, n, sw, img2, corr2)
+    st = ctx2.get_stats()
+    ref, nv, _ = oracle.em_correction(og2, sig, to_np(ev), img2.cpu().numpy().astype(np.float64), weights=w.cpu().numpy())
+    assert st.n_valid == nv and st.tile_oob == 0 and st.tile_events > 0
+    check_image(corr2.cpu().numpy(), ref, l2=2e-4, mx=5e-3, zero_tol=1e-6)
