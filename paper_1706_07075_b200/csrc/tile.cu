@@ -353,40 +353,38 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
                 unsigned li = tile_addr + (rc.y >> kRecLiShift) * 4u;
                 unsigned pq = (down ? dn_addr : up_addr) + ((rc.y >> kRecPlaneShift) & 127u) * 4u;
                 int na = (int)__float_as_int(lds_f32(pq));
-                // the value loaded in one step is consumed in the next
-                float accv = 0.f, wp = 0.f, vp = 0.f;
+                // the tile value is loaded at the top of a step and consumed at its end; the nine warps of a scheduler
+                // cover the 29 cycles in between (a hand-made one-step pipeline cost three register moves per two steps)
+                float accv = 0.f;
                 while (true) {
                     float t2;
                     {
                         const float tn = min3f(ta, tf, ts);
                         if (!(tn < te)) break;
-                        const float w = chord_weight(t, tn);
-                        accv = fmaf(wp, vp, accv);
                         if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                        vp = lds_f32(li);
-                        wp = w;
+                        const float v = lds_f32(li);
+                        const float w = chord_weight(t, tn);
                         advance_plane(ta, li, na, pq, tn, da, dpq);
                         advance_addr(tf, li, tn, df, inc_f);
                         advance_addr(ts, li, tn, ds, inc_s);
+                        accv = fmaf(w, v, accv);
                         t2 = tn;
                     }
                     t = t2;
                     {
                         const float tn = min3f(ta, tf, ts);
                         if (!(tn < te)) break;
-                        const float w = chord_weight(t, tn);
-                        accv = fmaf(wp, vp, accv);
                         if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                        vp = lds_f32(li);
-                        wp = w;
+                        const float v = lds_f32(li);
+                        const float w = chord_weight(t, tn);
                         advance_plane(ta, li, na, pq, tn, da, dpq);
                         advance_addr(tf, li, tn, df, inc_f);
                         advance_addr(ts, li, tn, ds, inc_s);
+                        accv = fmaf(w, v, accv);
                         t = tn;
                     }
                 }
                 const float w = chord_weight(t, te);
-                accv = fmaf(wp, vp, accv);
                 if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
                 const float fw = fmaf(w, lds_f32(li), accv);
                 if (fw > 0.0f) {  // R9
