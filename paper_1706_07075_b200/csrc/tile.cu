@@ -368,34 +368,25 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
                 // the tile value is loaded at the top of a step and consumed at its end; the nine warps of a scheduler
                 // cover the 29 cycles in between (a hand-made one-step pipeline cost three register moves per two steps)
                 float accv = 0.f;
-                while (true) {
-                    float t2;
-                    {
-                        const float tn = min3f(ta, tf, ts);
-                        if (!(tn < te)) break;
-                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                        const float v = lds_f32(li);
-                        const float w = chord_weight(t, tn);
-                        advance_plane(ta, li, na, pq, tn, da, dpq);
-                        advance_addr(tf, li, tn, df, inc_f);
-                        advance_addr(ts, li, tn, ds, inc_s);
-                        accv = fmaf(w, v, accv);
-                        t2 = tn;
-                    }
-                    t = t2;
-                    {
-                        const float tn = min3f(ta, tf, ts);
-                        if (!(tn < te)) break;
-                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                        const float v = lds_f32(li);
-                        const float w = chord_weight(t, tn);
-                        advance_plane(ta, li, na, pq, tn, da, dpq);
-                        advance_addr(tf, li, tn, df, inc_f);
-                        advance_addr(ts, li, tn, ds, inc_s);
-                        accv = fmaf(w, v, accv);
-                        t = tn;
-                    }
+                // rc.z = voxel visits of this window, counted by the plan's dry run of this very walk: a counted loop
+                // (one test per two steps) instead of comparing every crossing with the window's end
+                auto fstep = [&]() {
+                    const float tn = min3f(ta, tf, ts);
+                    if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                    const float v = lds_f32(li);
+                    const float w = chord_weight(t, tn);
+                    advance_plane(ta, li, na, pq, tn, da, dpq);
+                    advance_addr(tf, li, tn, df, inc_f);
+                    advance_addr(ts, li, tn, ds, inc_s);
+                    accv = fmaf(w, v, accv);
+                    t = tn;
+                };
+                int left = (int)rc.z - 1;
+                for (; left >= 2; left -= 2) {
+                    fstep();
+                    fstep();
                 }
+                if (left) fstep();
                 const float w = chord_weight(t, te);
                 if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
                 const float fw = fmaf(w, lds_f32(li), accv);
@@ -471,30 +462,21 @@ em_tile_kernel(int nx, int ny, int nz, const TileGeom *__restrict__ Gp, int tile
                 unsigned li = tile_addr + (rc.y >> kRecLiShift) * 4u;
                 unsigned pq = (down ? dn_addr : up_addr) + ((rc.y >> kRecPlaneShift) & 127u) * 4u;
                 int na = (int)__float_as_int(lds_f32(pq));
-                while (true) {  // two steps per trip: t and t2 alternate, no register move
-                    float t2;
-                    {
-                        const float tn = min3f(ta, tf, ts);
-                        if (!(tn < te)) break;
-                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                        red_shared_u32(li, chord_quanta(t, tn, lg2s));
-                        advance_plane(ta, li, na, pq, tn, da, dpq);
-                        advance_addr(tf, li, tn, df, inc_f);
-                        advance_addr(ts, li, tn, ds, inc_s);
-                        t2 = tn;
-                    }
-                    t = t2;
-                    {
-                        const float tn = min3f(ta, tf, ts);
-                        if (!(tn < te)) break;
-                        if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
-                        red_shared_u32(li, chord_quanta(t, tn, lg2s));
-                        advance_plane(ta, li, na, pq, tn, da, dpq);
-                        advance_addr(tf, li, tn, df, inc_f);
-                        advance_addr(ts, li, tn, ds, inc_s);
-                        t = tn;
-                    }
+                auto sstep = [&]() {
+                    const float tn = min3f(ta, tf, ts);
+                    if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
+                    red_shared_u32(li, chord_quanta(t, tn, lg2s));
+                    advance_plane(ta, li, na, pq, tn, da, dpq);
+                    advance_addr(tf, li, tn, df, inc_f);
+                    advance_addr(ts, li, tn, ds, inc_s);
+                    t = tn;
+                };
+                int left = (int)rc.z - 1;  // counted like the forward walk
+                for (; left >= 2; left -= 2) {
+                    sstep();
+                    sstep();
                 }
+                if (left) sstep();
                 if (CHECK && li - tile_addr >= tile_bytes) { ++oob; li = tile_addr; }
                 red_shared_u32(li, chord_quanta(t, te, lg2s));
             } else {
