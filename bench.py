@@ -480,6 +480,7 @@ def main():
     ap.add_argument("--report", default="", choices=["", "sweep", "division", "next", "pipeline"],
                     help="extra single-GPU reports (one JSON line each, not the driver's bench line): cfg-5 TOF/scale "
                          "sweep, cfg-4 nine-region division vs unsplit, timings of the widened rows (NEXT-1..4)")
+    ap.add_argument("--sens-sort", type=int, default=-1, help="TOFMLEM_OPT_SENS_SORT override")
     ap.add_argument("--concurrent", type=int, default=-1, help="TOFMLEM_OPT_CONCURRENT override")
     ap.add_argument("--l2-persist", type=int, default=-1, help="TOFMLEM_OPT_L2_PERSIST override")
     ap.add_argument("--region-plan", type=int, default=-1, help="TOFMLEM_OPT_REGION_PLAN override (division report)")
@@ -522,6 +523,8 @@ def main():
         ctx.set_option(pkg.OPT_L2_PERSIST, args.l2_persist)
     if args.concurrent >= 0:
         ctx.set_option(pkg.OPT_CONCURRENT, args.concurrent)
+    if args.sens_sort >= 0:
+        ctx.set_option(pkg.OPT_SENS_SORT, args.sens_sort)
     nvox = g.nvox
 
     def timed(fn):
