@@ -349,6 +349,33 @@ const char *tofmlem_last_error(const tofmlem_ctx *ctx);
 uint64_t tofmlem_launch_count(const tofmlem_ctx *ctx);
 const char *tofmlem_version(void);
 
+/* The fused forward+back EM pass of tofmlem_em_correction (R1, R9) WITHOUT a context and without
+ * any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): d_corr[j] += sum_{e: fwd_e > 0} a_ej / fwd_e, fwd_e = sum_k a_ek d_image[k], over the n events in
+ * the order given (binned or not), on the current device.  The call itself calls no cudaMalloc, cudaFree or allocating
+ * library routine: the only scratch of the pass, the work-queue counters of its persistent kernel, is a file-scope
+ * __device__ array of TOFMLEM_STATIC_MAX_QUEUES 32-bit words (4 KB) that every GPU which loads the library holds until
+ * the process exits.
+ *   grid, tof_fwhm_ps (0 = non-TOF: ev->dt may be NULL), trunc_sigmas (3.0 = the context default): as tofmlem_create /
+ *     TOFMLEM_OPT_TRUNC_SIGMAS.  ev: device arrays, n <= 2^32 - 1 entries.
+ *   d_image: nvox floats (device), read.  d_corr: nvox floats (device) in GRID order (never bricks), accumulated into:
+ *     the caller zeroes it.  16-byte aligned d_corr with nvox % 4 == 0 takes the 16-byte reductions, else scalar ones.
+ *   queues_per_sm: work queues (list segments) per SM, 1..8, or 0 = chosen from the window length like the context
+ *     path (1, 3 or 4).  Performance only.
+ *   cuda_stream: a cudaStream_t on the current device (NULL = default stream); the call enqueues one memset of the
+ *     counters and one kernel there and returns without synchronising.
+ * Limit: (SM count of the device) x queues_per_sm <= TOFMLEM_STATIC_MAX_QUEUES, else TOFMLEM_EINVAL (a B200 has 148 SMs).
+ * ALL calls in the process share the array on a device: it is cleared on the caller's stream before every launch, and
+ * two calls that OVERLAP on the GPU (different streams with no dependency between them, or two host threads) race on
+ * the counters and give wrong sums -- the caller serialises them.  No statistics counters are kept.
+ * Returns TOFMLEM_OK or a negative status; the text of the error is in tofmlem_static_error() (per host thread).
+ * Same arithmetic as the unplanned pass of a context with TOFMLEM_OPT_CORR_BRICKS = 0 (tests/test_zz_no_alloc.py). */
+#define TOFMLEM_STATIC_MAX_QUEUES 1024
+int tofmlem_em_correction_static(const tofmlem_grid *grid, double tof_fwhm_ps, double trunc_sigmas,
+                                 const tofmlem_events *ev, uint64_t n, const float *d_image, float *d_corr,
+                                 int queues_per_sm, void *cuda_stream);
+const char *tofmlem_static_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -46,6 +46,7 @@ SYMBOLS = (
     "tofmlem_median3", "tofmlem_attenuation_weights", "tofmlem_em_correction_weighted", "tofmlem_iterate_weighted",
     "tofmlem_gather_f32", "tofmlem_scatter_reject", "tofmlem_permute_events", "tofmlem_reserve", "tofmlem_trim",
     "tofmlem_plan_events", "tofmlem_plan_info", "tofmlem_pass_timing", "tofmlem_split_regions_overlap",
+    "tofmlem_em_correction_static", "tofmlem_static_error",
 )
 
 
@@ -99,6 +100,7 @@ def lib():
         L.tofmlem_version.restype = C.c_char_p
         L.tofmlem_num_bins.restype = C.c_uint32
         L.tofmlem_launch_count.restype = C.c_uint64
+        L.tofmlem_static_error.restype = C.c_char_p
         for name in SYMBOLS:
             getattr(L, name)  # AttributeError if a declared symbol is missing
         _lib = L
@@ -364,6 +366,24 @@ def make_grid(nx: int, ny: int, nz: int, voxel_mm, origin: Optional[Sequence[flo
     if origin is None:
         origin = (-0.5 * nx * vx, -0.5 * ny * vy, -0.5 * nz * vz)
     return Grid(nx, ny, nz, vx, vy, vz, *origin)
+
+
+def em_correction_static(grid: Grid, tof_fwhm_ps: float, ev, n: int, image: torch.Tensor, corr: torch.Tensor,
+                         trunc_sigmas: float = 3.0, queues_per_sm: int = 0,
+                         stream: Optional[torch.cuda.Stream] = None):
+    """tofmlem_em_correction_static: the fused EM pass without a context and without any allocation (scratch in a static
+    __device__ array); corr in grid order, accumulated into.  Enqueued on `stream` (default: torch's current stream)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("libtofmlem needs a CUDA device (B200, sm_100a); there is no CPU fallback")
+    L = lib()
+    e = _events(ev, n)
+    s = (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+    rc = L.tofmlem_em_correction_static(C.byref(grid), C.c_double(tof_fwhm_ps), C.c_double(trunc_sigmas), C.byref(e),
+                                        C.c_uint64(n), C.c_void_p(_ptr(image, torch.float32, "cuda", grid.nvox)),
+                                        C.c_void_p(_ptr(corr, torch.float32, "cuda", grid.nvox)),
+                                        C.c_int(queues_per_sm), C.c_void_p(s))
+    if rc != 0:
+        raise TofMlemError(rc, L.tofmlem_static_error().decode())
 
 
 def version() -> str:
