@@ -117,6 +117,13 @@ enum {
     TOFMLEM_OPT_CONCURRENT = 22,    /* planned fused pass: k > 0 runs the direct pass on records on a second stream BESIDE the tile
                                        pass, the tile pass limited to k CTAs per SM (0, the default: one after the
                                        other).  Performance only. */
+    TOFMLEM_OPT_WARP_WALK = 23,     /* 1 (default): whole-chord walks -- tofmlem_sensitivity, tofmlem_attenuation_weights and every
+                                       projection / fused pass of a non-TOF context -- run with a WARP per LOR: the 32 lanes
+                                       take 32 consecutive slabs along the chord's dominant axis, on images stored with that
+                                       axis fastest (2 x nvox floats of scratch kept by the context); 0: a thread per LOR as
+                                       for TOF windows.  Same result up to float32 rounding (both within the parity
+                                       tolerances against the fp64 oracle).  With 1 the correction image of a non-TOF
+                                       context is in grid order, not in bricks (see TOFMLEM_OPT_CORR_BRICKS). */
     TOFMLEM_OPT_SENS_SORT = 21,     /* 1: tofmlem_sensitivity orders the LORs by locality key and chord length first (32 B per
                                        LOR of scratch during the call; from 2^18 LORs on); 0 (default): as they come.
                                        Performance only (the image is the same up to the order of the float32 sums);

@@ -68,6 +68,8 @@ struct tofmlem_ctx {
     const float *l2_ptr = nullptr;  // correction image the stream's access-policy window currently covers
     cudaStream_t l2_stream = nullptr;
     int region_overlap = 0;  // reading R27: an event goes to every region its window meets (TOFMLEM_OPT_REGION_OVERLAP)
+    int warp_walk = 1;            // TOFMLEM_OPT_WARP_WALK: whole-chord (non-TOF) walks with a warp per LOR (warpwalk.cu)
+    float *d_axis = nullptr;      // its scratch: image / target stored y-fastest or z-fastest (2 nvox floats)
     int sens_sort = 0;            // TOFMLEM_OPT_SENS_SORT: tofmlem_sensitivity orders the LORs by locality and chord length
     bool bin_whole_chords = false;  // tofmlem_bin_events: sub-bins by the visits of the WHOLE chord (non-TOF walks)
     int tile_min_items = -1;  // TOFMLEM_OPT_TILE_MIN_ITEMS (-1: twice the number of tile CTAs the GPU holds)
@@ -189,10 +191,29 @@ bool vec_ok(const tofmlem_ctx *c, const float *out) {
     return (c->nvox & 3) == 0 && (reinterpret_cast<uintptr_t>(out) & 15) == 0;
 }
 
+// Whole-chord walks (sensitivity, attenuation line integrals, every projection of a non-TOF context) run with a warp per
+// LOR (warpwalk.cu) unless switched off or the grid does not fit its index packing.
+bool warp_on(const tofmlem_ctx *c) { return c->warp_walk && c->projector == 0 && warp_walk_ok(make_params(c, false)); }
+// ... and so does the fused pass of a non-TOF context (default scheduling variant only); its correction image is in
+// grid order (the walk wants the ray's dominant axis fastest, not bricks).
+bool warp_em_on(const tofmlem_ctx *c) { return !c->tof && c->em_variant == 0 && warp_on(c); }
+
+int ensure_axis_scratch(tofmlem_ctx *c) {
+    if (c->d_axis) return TOFMLEM_OK;
+    if (cudaMalloc(&c->d_axis, 2 * c->nvox * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        c->d_axis = nullptr;
+        c->err = "out of device memory (axis-major scratch of the warp-per-LOR walk)";
+        return TOFMLEM_ENOMEM;
+    }
+    return TOFMLEM_OK;
+}
+
 // Is the correction image `corr` of this context's fused pass / update in the brick layout?  Depends only on the
 // context's options and the pointer, so tofmlem_em_correction and tofmlem_update agree without further state.
 bool bricks_on(const tofmlem_ctx *c, const float *corr) {
-    return c->corr_bricks && c->projector == 0 && (c->grid.nx & 1) == 0 && (c->grid.ny & 1) == 0 && vec_ok(c, corr);
+    return c->corr_bricks && c->projector == 0 && (c->grid.nx & 1) == 0 && (c->grid.ny & 1) == 0 && vec_ok(c, corr) &&
+           !warp_em_on(c);
 }
 
 // The brick-order update reads image and sens as float2: both must be 8-byte aligned there (checked by the callers
@@ -437,6 +458,10 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         int rc = ensure_lut(ctx);
         if (rc) return rc;
         launch_sampled_em(p, ctx->d_lut, ctx->samples_k, ev, n, evw, d_image, d_corr, ctx->d_stats, ctx->d_queues, s);
+    } else if (warp_em_on(ctx)) {
+        int rc = ensure_axis_scratch(ctx);
+        if (rc) return rc;
+        launch_warp_em(p, ev, n, evw, d_image, d_corr, ctx->d_axis, ctx->d_stats, s);
     } else if (plan_matches(ctx, ev.x1, n) && ctx->plan.brick == p.brick && ctx->em_variant == 0) {
         // Planned list (tofmlem_plan_events): the pass runs on the ray records -- the items on shared-memory tiles
         // (tile.cu), the other events and the stragglers of the items through the direct pass on records (prepared.cu).
@@ -633,6 +658,7 @@ int tofmlem_destroy(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_rg_sorted);
     cudaFree(ctx->d_rg_binned);
     cudaFree(ctx->d_tmp_image);
+    cudaFree(ctx->d_axis);
     cudaFree(ctx->d_lut);
     cudaFree(ctx->d_rcounts);
     cudaFree(ctx->d_hev);
@@ -724,6 +750,10 @@ int tofmlem_set_option(tofmlem_ctx *ctx, int key, double value) {
             if (value < 0 || value > 4 || value != floor(value)) return fail(ctx, TOFMLEM_EINVAL, "concurrent in 0..4");
             ctx->concurrent = (int)value;
             return TOFMLEM_OK;
+        case TOFMLEM_OPT_WARP_WALK:
+            if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "warp_walk is 0 or 1");
+            ctx->warp_walk = (int)value;
+            return TOFMLEM_OK;
         case TOFMLEM_OPT_SENS_SORT:
             if (value != 0.0 && value != 1.0) return fail(ctx, TOFMLEM_EINVAL, "sens_sort is 0 or 1");
             ctx->sens_sort = (int)value;
@@ -800,6 +830,8 @@ int tofmlem_trim(tofmlem_ctx *ctx) {
     cudaFree(ctx->d_rg_sorted);
     cudaFree(ctx->d_rg_binned);
     cudaFree(ctx->d_tmp_image);
+    cudaFree(ctx->d_axis);
+    ctx->d_axis = nullptr;
     cudaFree(ctx->d_hev);
     cudaFree(ctx->d_himg);
     cudaFree(ctx->d_hsens);
@@ -850,7 +882,13 @@ int tofmlem_sensitivity(tofmlem_ctx *ctx, const tofmlem_events *lors, uint64_t m
             cudaGetLastError();  // not enough memory for the scratch: the LORs as they come
         }
     }
-    launch_backproject(p, false, ev, m, nullptr, d_sens, vec_ok(ctx, d_sens), ctx->stream);
+    if (warp_on(ctx)) {
+        int rc = ensure_axis_scratch(ctx);
+        if (rc) return rc;
+        launch_warp_backproject(p, ev, m, nullptr, d_sens, ctx->d_axis, ctx->stream);
+    } else {
+        launch_backproject(p, false, ev, m, nullptr, d_sens, vec_ok(ctx, d_sens), ctx->stream);
+    }
     if (d_key || d_perm || d_sorted) {
         cudaStreamSynchronize(ctx->stream);
         cudaFree(d_key);
@@ -874,6 +912,10 @@ int tofmlem_forward(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, cons
                                ctx->stream);
     } else if (plan_matches(ctx, ev->x1, n)) {  // planned list: the walk of the fused pass, on the ray records
         launch_planned_forward(make_params(ctx, true), ctx->sigma, ev_ptrs(ev), ctx->d_rec, n, d_image, d_fwd, ctx->stream);
+    } else if (!ctx->tof && warp_on(ctx)) {
+        int rc = ensure_axis_scratch(ctx);
+        if (rc) return rc;
+        launch_warp_forward(make_params(ctx, false), ev_ptrs(ev), n, d_image, d_fwd, ctx->d_axis, ctx->stream);
     } else {
         launch_forward(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_image, d_fwd, ctx->stream);
     }
@@ -890,6 +932,10 @@ int tofmlem_backproject(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n, 
         if (rc) return rc;
         launch_sampled_backproject(make_params(ctx, true), ctx->d_lut, ctx->samples_k, ev_ptrs(ev), n, d_values, d_out,
                                    ctx->stream);
+    } else if (!ctx->tof && warp_on(ctx)) {
+        int rc = ensure_axis_scratch(ctx);
+        if (rc) return rc;
+        launch_warp_backproject(make_params(ctx, false), ev_ptrs(ev), n, d_values, d_out, ctx->d_axis, ctx->stream);
     } else {
         launch_backproject(make_params(ctx, ctx->tof), ctx->tof, ev_ptrs(ev), n, d_values, d_out, vec_ok(ctx, d_out),
                            ctx->stream);
@@ -965,7 +1011,13 @@ int tofmlem_attenuation_weights(tofmlem_ctx *ctx, const tofmlem_events *lors, ui
         return fail(ctx, TOFMLEM_EINVAL, "attenuation_weights: bad argument");
     EventPtrs ev = ev_ptrs(lors);
     ev.dt = nullptr;
-    launch_forward(make_params(ctx, false), false, ev, n, d_mu, d_weight, ctx->stream);  // line integral of mu
+    if (warp_on(ctx)) {  // line integral of mu
+        int rc = ensure_axis_scratch(ctx);
+        if (rc) return rc;
+        launch_warp_forward(make_params(ctx, false), ev, n, d_mu, d_weight, ctx->d_axis, ctx->stream);
+    } else {
+        launch_forward(make_params(ctx, false), false, ev, n, d_mu, d_weight, ctx->stream);
+    }
     CHECK_LAUNCH(1);
     launch_exp(d_weight, n, ctx->stream);
     CHECK_LAUNCH(1);

@@ -68,6 +68,15 @@ void launch_em_correction_chunks(const ProjParams &p, bool tof, const EventPtrs 
                                  uint32_t n_chunks, const float *evw, const float *image, float *corr, bool vec_ok,
                                  DeviceStats *stats, unsigned *queues, cudaStream_t s);
 
+// ---- warpwalk.cu: a warp per LOR for whole chords (non-TOF); scratch = 2 (forward: 1) x nvox floats
+bool warp_walk_ok(const ProjParams &p);
+void launch_warp_backproject(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *values, float *out,
+                             float *scratch, cudaStream_t s);
+void launch_warp_forward(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *image, float *fwd,
+                         float *scratch, cudaStream_t s);
+void launch_warp_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
+                    float *corr, float *scratch, DeviceStats *stats, cudaStream_t s);
+
 // ---- tile.cu: fused EM pass with the image and the correction image of one locality bin held in shared memory
 constexpr int kTileMaxPlanes = 96;
 // Footprint of a locality bin (cube of T voxels, direction class with dominant axis a): the union of the +-T sigma

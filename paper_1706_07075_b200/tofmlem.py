@@ -34,6 +34,7 @@ OPT_L2_PERSIST = 19
 OPT_TILE_MIN_ITEMS = 20
 OPT_SENS_SORT = 21
 OPT_CONCURRENT = 22
+OPT_WARP_WALK = 23
 PROJECTOR_SIDDON, PROJECTOR_SAMPLED = 0, 1
 
 # every symbol include/tofmlem.h declares (checked by tests/test_abi.py against the header text)
