@@ -195,7 +195,34 @@ __device__ __forceinline__ Slab slab_pieces(const float4 &q0, const float4 &q1, 
     return o;
 }
 
-// predicated forms (ptxas otherwise wraps every access in a branch with its convergence barrier)
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+// The pieces of 32 slabs (32 to 96 voxel visits) are put in CHORD ORDER into the warp's shared-memory buffer and handled 32
+// consecutive visits per instruction: the visits of a chord inside one (f, s) row are consecutive words, so an
+// instruction costs about one L2 request per row it meets.  Three predicated reductions per lane, piece by piece, would
+// send the second and third pieces as requests of their own: 1.3 instead of 0.7 requests per slab for a typical oblique
+// ray, and the scatter walk is bound by these requests (sensitivity of 20 M LORs: 15.8 -> 11.5 ms).
+// Returns the number of visits now in buf[0 .. total); the caller runs `for (t = lane; t < total; t += 32)` and then
+// __syncwarp() before the next call.
+__device__ __forceinline__ unsigned compact_pieces(const Slab &p, float scale, unsigned lt, uint2 *buf) {
+    const bool h0 = p.l0 > 0.0f, h1 = p.l1 > 0.0f, h2 = p.l2 > 0.0f;
+    const unsigned b0 = __ballot_sync(0xffffffffu, h0), b1 = __ballot_sync(0xffffffffu, h1);
+    const unsigned b2 = __ballot_sync(0xffffffffu, h2);
+    unsigned slot = __popc(b0 & lt) + __popc(b1 & lt) + __popc(b2 & lt);
+    if (h0) buf[slot] = make_uint2(p.i0, __float_as_uint(p.l0 * scale));
+    slot += h0;
+    if (h1) buf[slot] = make_uint2(p.i1, __float_as_uint(p.l1 * scale));
+    slot += h1;
+    if (h2) buf[slot] = make_uint2(p.i2, __float_as_uint(p.l2 * scale));
+    __syncwarp();
+    return __popc(b0) + __popc(b1) + __popc(b2);
+}
+
+// a predicated load (ptxas otherwise wraps every access in a branch with its convergence barrier)
 __device__ __forceinline__ float ldg_if_pos(float l, const float *p) {
     float v;
     asm volatile(
@@ -205,13 +232,10 @@ __device__ __forceinline__ float ldg_if_pos(float l, const float *p) {
     return v;
 }
 
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-    return v;
-}
-
-// sum over the chord of (piece length, u units) x src; every lane returns its partial sum
+// sum over the chord of (piece length, u units) x src; every lane returns its partial sum.  Three predicated loads per
+// lane, piece by piece: the chord-order compaction of the scatter walk was measured here too and is SLOWER (attenuation
+// weights of 20 M LORs 9.1 -> 19.0 ms): the round trip through shared memory puts a warp barrier between the loads of
+// consecutive iterations, which then no longer overlap, and the L1 absorbs the extra requests of the plain form anyway.
 __device__ __forceinline__ float chord_gather(const float4 &q0, const float4 &q1, const float4 &q2, const float4 &q3,
                                               unsigned lane, unsigned SF, unsigned SS,
                                               const float *__restrict__ src) {
@@ -233,11 +257,7 @@ __device__ __forceinline__ float chord_gather(const float4 &q0, const float4 &q1
     return acc;
 }
 
-// dst[j] += scale * (length of the chord in voxel j, u units).  The pieces of 32 slabs (32 to 96 voxel visits) are put
-// in chord order into the warp's shared-memory buffer and sent 32 CONSECUTIVE visits per instruction: the visits of a
-// chord inside one (f, s) row are consecutive words, so an instruction costs about one L2 request per row it meets
-// (three predicated reductions per lane, piece by piece, would send the second and third pieces as requests of their own:
-// 1.3 instead of 0.7 requests per slab for a typical oblique ray, and the pass is bound by these requests).
+// dst[j] += scale * (length of the chord in voxel j, u units)
 __device__ __forceinline__ void chord_scatter(const float4 &q0, const float4 &q1, const float4 &q2, const float4 &q3,
                                               unsigned lane, unsigned SF, unsigned SS, float *__restrict__ dst,
                                               float scale, uint2 *buf /* 96 entries of this warp */) {
@@ -248,18 +268,7 @@ __device__ __forceinline__ void chord_scatter(const float4 &q0, const float4 &q1
     unsigned j = lane;
     float jf = (float)lane;
     for (unsigned jb = 0; jb <= last; jb += 32u, j += 32u, jf += 32.0f) {
-        const Slab p = slab_pieces(q0, q1, q2, base, jf, j, dF, dS);
-        const bool h0 = p.l0 > 0.0f, h1 = p.l1 > 0.0f, h2 = p.l2 > 0.0f;
-        const unsigned b0 = __ballot_sync(0xffffffffu, h0), b1 = __ballot_sync(0xffffffffu, h1);
-        const unsigned b2 = __ballot_sync(0xffffffffu, h2);
-        unsigned slot = __popc(b0 & lt) + __popc(b1 & lt) + __popc(b2 & lt);
-        const unsigned total = __popc(b0) + __popc(b1) + __popc(b2);
-        if (h0) buf[slot] = make_uint2(p.i0, __float_as_uint(p.l0 * scale));
-        slot += h0;
-        if (h1) buf[slot] = make_uint2(p.i1, __float_as_uint(p.l1 * scale));
-        slot += h1;
-        if (h2) buf[slot] = make_uint2(p.i2, __float_as_uint(p.l2 * scale));
-        __syncwarp();
+        const unsigned total = compact_pieces(slab_pieces(q0, q1, q2, base, jf, j, dF, dS), scale, lt, buf);
         for (unsigned t = lane; t < total; t += 32u) {
             const uint2 v = buf[t];
             asm volatile("red.global.add.f32 [%0], %1;" ::"l"(dst + v.x), "f"(__uint_as_float(v.y)) : "memory");
