@@ -234,8 +234,8 @@ __device__ __forceinline__ float ldg_if_pos(float l, const float *p) {
 
 // sum over the chord of (piece length, u units) x src; every lane returns its partial sum.  Three predicated loads per
 // lane, piece by piece: the chord-order compaction of the scatter walk was measured here too and is SLOWER (attenuation
-// weights of 20 M LORs 9.1 -> 19.0 ms): the round trip through shared memory puts a warp barrier between the loads of
-// consecutive iterations, which then no longer overlap, and the L1 absorbs the extra requests of the plain form anyway.
+// weights of 20 M LORs 9.1 -> 19.0 ms; 13.7 ms with the loads of one iteration consumed in the next): the round trip
+// through shared memory and its two warp barriers cost more issue slots and latency than the merged requests save.
 __device__ __forceinline__ float chord_gather(const float4 &q0, const float4 &q1, const float4 &q2, const float4 &q3,
                                               unsigned lane, unsigned SF, unsigned SS,
                                               const float *__restrict__ src) {
