@@ -176,7 +176,8 @@ double tofmlem_sigma_mm(const tofmlem_ctx *ctx);
 /* Scratch memory.  The context allocates device scratch at first use and keeps it until tofmlem_destroy: the
  * correction image of tofmlem_iterate (4 B per voxel), the histogram of tofmlem_bin_events (8 B per locality bin and
  * sub-bin, 1 B per event), the records of tofmlem_permute_events (32 B per event), the event copies of
- * tofmlem_reconstruct_regions (64 B per event), the staging buffers of tofmlem_iterate_host.  cudaMalloc inside a
+ * tofmlem_reconstruct_regions (64 B per event), the staging buffers of tofmlem_iterate_host, the axis-fastest image copies of
+ * the whole-chord walks (TOFMLEM_OPT_WARP_WALK: 8 B per voxel, also allocated by tofmlem_reserve).  cudaMalloc inside a
  * call synchronises the device, so a caller who times calls or runs several contexts concurrently reserves first:
  * tofmlem_reserve allocates what iterate / bin_events / permute_events need for up to n_events events under the
  * context's CURRENT options (call it after tofmlem_set_option).  tofmlem_trim SYNCHRONISES and releases every

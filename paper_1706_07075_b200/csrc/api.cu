@@ -806,6 +806,10 @@ int tofmlem_reserve(tofmlem_ctx *ctx, uint64_t n_events) {
     if (!ctx || n_events > 0xFFFFFFFFull) return TOFMLEM_EINVAL;
     int rc = ensure_corr(ctx);
     if (rc) return rc;
+    if (warp_on(ctx)) {  // axis-fastest scratch of the whole-chord walks (sensitivity, attenuation weights, non-TOF passes)
+        rc = ensure_axis_scratch(ctx);
+        if (rc) return rc;
+    }
     if (n_events) {
         const uint32_t S = effective_subbins(ctx);
         rc = ensure_bin_scratch(ctx, (size_t)num_bins(ctx) * S + 1, S > 1 ? n_events : 0);
