@@ -142,10 +142,12 @@ enum {
                                        the ONE region that holds its TOF centre (bit-exact split), extended images summed;
                                        1 = reading R27, an event in every region its window reaches (1 or 2),
                                        wider margins, cores only */
-    TOFMLEM_OPT_REGION_PLAN = 17,   /* 1: tofmlem_reconstruct_regions calls tofmlem_plan_events on every region's binned
-                                       list (ray records + tiles; 48 B per event more scratch); 0 (default): unplanned
-                                       passes -- nine plans synchronise nine times, which costs more than five planned
-                                       iterations save (measured: 184 vs 142 ms at cfg-4) */
+    TOFMLEM_OPT_REGION_PLAN = 17,   /* 1: tofmlem_reconstruct_regions plans every region's binned list (ray records + tiles;
+                                       48 B per event more scratch), the phases of the nine plans interleaved so that
+                                       the host waits twice in all; 0 (default): unplanned passes.  Measured at cfg-4,
+                                       5 iterations: 140.5 ms with plans against 142.4 ms without (184 ms when every plan
+                                       synchronised on its own) -- nine concurrent regions are not bound by their
+                                       iteration kernels, so the default stays 0. */
     TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
                                        generated an identically reconstructed image").  1: the iterations of
                                        tofmlem_iterate[_weighted] on a PLANNED list (tofmlem_plan_events; else

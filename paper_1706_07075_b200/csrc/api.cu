@@ -123,6 +123,18 @@ struct tofmlem_ctx {
         uint64_t tile_events = 0, direct_events = 0, valid_events = 0, visits = 0;
         int sorted = 0;
     } plan;
+    // state of a plan between the phases of tofmlem_plan_events (plan_begin / plan_build / plan_finish)
+    struct PlanJob {
+        tofmlem_events ev{};
+        uint64_t n = 0;
+        ProjParams p{};
+        TileGeom g{};
+        std::vector<TileItem> items;
+        std::vector<TileRange> ranges;
+        unsigned flags[2] = {0, 0};
+        uint32_t n_pieces = 0;
+        std::vector<unsigned char> hc;
+    } job;
     std::string err;
 };
 
@@ -1139,33 +1151,42 @@ int tofmlem_iterate_host(tofmlem_ctx *ctx, const tofmlem_events *h_ev, uint64_t 
     return TOFMLEM_OK;
 }
 
-int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) {
-    if (!ctx) return TOFMLEM_EINVAL;
+// tofmlem_plan_events in three phases, so that a caller with several contexts on several streams
+// (tofmlem_reconstruct_regions) can enqueue phase 1 everywhere, then phase 2 everywhere, then phase 3: each phase ends with
+// asynchronous copies to the host, and the NEXT phase starts after a synchronisation of the context's stream -- two rounds
+// of waiting in all instead of two per context with the other streams idle meanwhile.
+//   plan_begin  : validation, scratch, key histogram of the list -> host (asynchronous).  1 = nothing to plan, 0 = started.
+//   plan_build  : (stream synchronised) tile items from the bin counts; ray records, dry run, piece list -> counters to host
+//   plan_finish : (stream synchronised) the plan becomes valid
+namespace {
+
+int plan_begin(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) {
     ctx->plan.valid = false;
     ctx->plan.n_items = ctx->plan.n_strag = 0;
     ctx->plan.direct_valid = 0;
     ctx->plan.tile_events = ctx->plan.direct_events = ctx->plan.valid_events = ctx->plan.visits = 0;
     ctx->plan.sorted = 0;
-    if (n == 0) return TOFMLEM_OK;
+    if (n == 0) return 1;
     if (!ev_ok(ev, ctx->tof) || n > 0xFFFFFFFFull) return fail(ctx, TOFMLEM_EINVAL, "plan_events: bad argument");
-    if (!ctx->tof || ctx->projector != 0) return TOFMLEM_OK;  // records exist for the TOF Siddon pass only
-    ProjParams p = make_params(ctx, true);
+    if (!ctx->tof || ctx->projector != 0) return 1;  // records exist for the TOF Siddon pass only
+    auto &J = ctx->job;
+    J.ev = *ev;
+    J.n = n;
+    J.p = make_params(ctx, true);
     // the layout the context's own correction image will have (ensure_corr aligns it): decides which group count the
     // direct records carry; a pass into another layout ignores the plan
-    p.brick = ctx->corr_bricks && (ctx->grid.nx & 1) == 0 && (ctx->grid.ny & 1) == 0 && (ctx->nvox & 3) == 0 ? 1 : 0;
-    TileGeom g;
-    build_tile_geom(p, ctx->tile_log2, ctx->smem_optin, ctx->smem_per_sm, g);
+    J.p.brick = ctx->corr_bricks && (ctx->grid.nx & 1) == 0 && (ctx->grid.ny & 1) == 0 && (ctx->nvox & 3) == 0 ? 1 : 0;
+    build_tile_geom(J.p, ctx->tile_log2, ctx->smem_optin, ctx->smem_per_sm, J.g);
     cudaStream_t s = ctx->stream;
     {
         int rc0 = ensure_plan_scratch(ctx, n);
         if (rc0) return rc0;
     }
+    J.items.clear();
+    J.ranges.clear();
+    J.flags[0] = J.flags[1] = 0;
     // ---- which bins become tile items?  Needs a list sorted by key (tofmlem_permute_events) and tiles that fit.
-    std::vector<TileItem> items;
-    std::vector<TileRange> ranges;
-    uint64_t in_items = 0;
-    bool sorted = false;
-    if (g.ok) {
+    if (J.g.ok) {
         const uint32_t nb = num_bins(ctx);
         int rc = ensure_bin_scratch(ctx, (size_t)nb + 1, 0);
         if (rc) return rc;
@@ -1173,12 +1194,26 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         CU(cudaMemsetAsync(ctx->d_plan_flags, 0, 2 * sizeof(unsigned), s));
         launch_plan_hist(grid_f32(ctx), ctx->tile_log2, ev_ptrs(ev), n, ctx->d_hist, nb, ctx->d_plan_flags + 1, s);
         CHECK_LAUNCH(1);
-        const uint32_t *cnt = ctx->h_hist_pinned;
-        unsigned flags[2] = {0, 0};
         CU(cudaMemcpyAsync(ctx->h_hist_pinned, ctx->d_hist, (size_t)nb * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-        CU(cudaMemcpyAsync(flags, ctx->d_plan_flags, sizeof flags, cudaMemcpyDeviceToHost, s));
-        CU(cudaStreamSynchronize(s));
-        sorted = flags[1] == 0;
+        CU(cudaMemcpyAsync(J.flags, ctx->d_plan_flags, sizeof J.flags, cudaMemcpyDeviceToHost, s));
+    }
+    return 0;
+}
+
+int plan_build(tofmlem_ctx *ctx) {
+    auto &J = ctx->job;
+    const TileGeom &g = J.g;
+    const ProjParams &p = J.p;
+    const tofmlem_events *ev = &J.ev;
+    const uint64_t n = J.n;
+    cudaStream_t s = ctx->stream;
+    std::vector<TileItem> &items = J.items;
+    std::vector<TileRange> &ranges = J.ranges;
+    bool sorted = false;
+    if (g.ok) {
+        const uint32_t nb = num_bins(ctx);
+        const uint32_t *cnt = ctx->h_hist_pinned;
+        sorted = J.flags[1] == 0;
         if (sorted) {
             // Tile items: a bin with at least tile_min_events events (pieces of at most tile_max_events, whole warps), or
             // a PAIR of bins that are neighbours along the class's dominant axis and hold tile_min_events .. tile_max_events
@@ -1211,7 +1246,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
                     state[b] = 1;
                     state[b2] = 2;
                     items.push_back(TileItem{(uint32_t)start[b], c, (uint32_t)start[b2], c2, b, 1u, 0u, 0u});
-                    in_items += c + c2;
                 } else if (c >= thr) {
                     state[b] = 1;
                     const uint32_t pieces = (c + mx - 1) / mx;
@@ -1219,7 +1253,6 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
                     per = (per + 31u) & ~31u;
                     for (uint32_t k = 0; k < c; k += per)
                         items.push_back(TileItem{(uint32_t)(start[b] + k), c - k < per ? c - k : per, 0u, 0u, b, 0u, 0u, 0u});
-                    in_items += c;
                 }
             }
             // the items' event ranges in list order: the record set-up finds the item of an event by bisection
@@ -1239,10 +1272,7 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
         if (items.size() < min_items) items.clear();
     }
     ctx->plan.sorted = sorted ? 1 : 0;
-    if (items.empty()) {  // no tiles (window too wide, unsorted list, sparse bins): the whole list in order
-        ranges.clear();
-        in_items = 0;
-    }
+    if (items.empty()) ranges.clear();  // no tiles (window too wide, unsorted list, sparse bins): the whole list in order
     // ---- scratch (grows only)
     if (ctx->items_cap < items.size()) {
         cudaFree(ctx->d_items);
@@ -1274,38 +1304,55 @@ int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) 
     CHECK_LAUNCH(1);
     // the pieces of the direct pass: the flagged 32-event pieces, compacted in list order on the device
     const uint32_t nc = (uint32_t)((n + 31) / 32);
-    uint32_t n_pieces = 0;
+    J.n_pieces = 0;
     CU(cudaMemsetAsync(ctx->d_chunk_flags + nc, 0, sizeof(uint32_t), s));
     ctx->launches += launch_exclusive_scan_u32(ctx->d_chunk_flags, ctx->d_chunk_pos, ctx->d_chunk_tmp, nc + 1, s);
     launch_compact_flags(ctx->d_chunk_flags, ctx->d_chunk_pos, nc, ctx->d_chunk_list, s);
     CHECK_LAUNCH(1);
-    CU(cudaMemcpyAsync(&n_pieces, ctx->d_chunk_pos + nc, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
-    std::vector<unsigned char> hc(plan_counter_bytes());
-    CU(cudaMemcpyAsync(hc.data(), ctx->d_plan_counters, hc.size(), cudaMemcpyDeviceToHost, s));
-    CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
+    CU(cudaMemcpyAsync(&J.n_pieces, ctx->d_chunk_pos + nc, sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    J.hc.resize(plan_counter_bytes());
+    CU(cudaMemcpyAsync(J.hc.data(), ctx->d_plan_counters, J.hc.size(), cudaMemcpyDeviceToHost, s));
+    return TOFMLEM_OK;  // the host vectors of the job stay alive until plan_finish
+}
+
+int plan_finish(tofmlem_ctx *ctx) {
+    auto &J = ctx->job;
     uint64_t cnt4[5];
-    read_plan_counters(hc.data(), cnt4);
+    read_plan_counters(J.hc.data(), cnt4);
     if (cnt4[4] > kTinyCap) return TOFMLEM_OK;  // a list made of slivers: not worth a plan (stays inactive)
     ctx->plan.n_tiny = (uint32_t)cnt4[4];
     ctx->plan.valid = true;
-    ctx->plan.x1 = ev->x1;
-    ctx->plan.n = n;
+    ctx->plan.x1 = J.ev.x1;
+    ctx->plan.n = J.n;
     ctx->plan.tile_log2 = ctx->tile_log2;
     ctx->plan.sigma = ctx->sigma;
     ctx->plan.trunc = ctx->trunc_sigmas;
-    ctx->plan.brick = p.brick;
-    ctx->plan.n_items = (uint32_t)items.size();
+    ctx->plan.brick = J.p.brick;
+    ctx->plan.n_items = (uint32_t)J.items.size();
     ctx->plan.max_item_events = 0;
-    for (const TileItem &it : items)
+    for (const TileItem &it : J.items)
         if (it.count + it.count2 > ctx->plan.max_item_events) ctx->plan.max_item_events = it.count + it.count2;
     ctx->plan.n_strag = (uint32_t)cnt4[2];
     ctx->plan.valid_events = cnt4[0];
     ctx->plan.tile_events = cnt4[1];
-    ctx->plan.direct_events = n - cnt4[1];
+    ctx->plan.direct_events = J.n - cnt4[1];
     ctx->plan.visits = cnt4[3];
     ctx->plan.direct_valid = cnt4[0] - cnt4[1] - cnt4[4];
-    ctx->plan.n_pieces = n_pieces;
+    ctx->plan.n_pieces = J.n_pieces;
     return TOFMLEM_OK;
+}
+
+}  // namespace
+
+int tofmlem_plan_events(tofmlem_ctx *ctx, const tofmlem_events *ev, uint64_t n) {
+    if (!ctx) return TOFMLEM_EINVAL;
+    int rc = plan_begin(ctx, ev, n);
+    if (rc) return rc < 0 ? rc : TOFMLEM_OK;
+    CU(cudaStreamSynchronize(ctx->stream));
+    rc = plan_build(ctx);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(ctx->stream));
+    return plan_finish(ctx);
 }
 
 int tofmlem_plan_info(const tofmlem_ctx *ctx, tofmlem_plan *h_out) {
@@ -1634,6 +1681,9 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
         (void)cmax;
     }
     uint64_t off = 0;
+    std::vector<tofmlem_events> run_evs(n_regions);
+    std::vector<int> planning(n_regions, 0);
+    const bool want_plan = ctx->region_plan && ctx->tof && ctx->projector == 0 && ctx->em_variant == 0 && iters > 1;
     for (int r = 0; r < n_regions; ++r) {
         tofmlem_ctx *sc = C.subs[r];
         cudaStream_t rs = C.streams[r];
@@ -1666,21 +1716,41 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
                 return rc;
             }
         }
-        tofmlem_events run_ev{bin_ev.x1, bin_ev.y1, bin_ev.z1, bin_ev.x2, bin_ev.y2, bin_ev.z2, bin_ev.dt};
-        // ray records + tiles for the region's own binned list (synchronises the region's stream only; the regions
-        // launched before keep the GPU busy meanwhile)
-        if (counts[r] && ctx->region_plan && ctx->tof && ctx->projector == 0 && ctx->em_variant == 0 && iters > 1) {
-            rc = tofmlem_plan_events(sc, &run_ev, counts[r]);
+        run_evs[r] = tofmlem_events{bin_ev.x1, bin_ev.y1, bin_ev.z1, bin_ev.x2, bin_ev.y2, bin_ev.z2, bin_ev.dt};
+        // ray records + tiles for the region's own binned list, phase 1 (key histogram -> host, asynchronous)
+        planning[r] = 0;
+        sc->plan.valid = false;
+        if (counts[r] && want_plan) {
+            rc = plan_begin(sc, &run_evs[r], counts[r]);
+            if (rc < 0) {
+                ctx->err = sc->err;
+                cudaDeviceSynchronize();
+                free_region_cache(ctx);
+                return rc;
+            }
+            planning[r] = rc == 0;
+        }
+        off += counts[r];
+    }
+    // phases 2 and 3 of the plans, region by region: while the host waits for one region's stream the others work
+    for (int phase = 2; phase <= 3 && want_plan; ++phase)
+        for (int r = 0; r < n_regions; ++r) {
+            if (!planning[r]) continue;
+            tofmlem_ctx *sc = C.subs[r];
+            rc = cudaStreamSynchronize(C.streams[r]) == cudaSuccess ? TOFMLEM_OK : TOFMLEM_ECUDA;
+            if (rc == TOFMLEM_OK) rc = phase == 2 ? plan_build(sc) : plan_finish(sc);
             if (rc != TOFMLEM_OK) {
                 ctx->err = sc->err;
                 cudaDeviceSynchronize();
                 free_region_cache(ctx);
                 return rc;
             }
-        } else {
-            sc->plan.valid = false;
         }
-        rc = iterate_device(sc, counts[r] ? ev_ptrs(&run_ev) : EventPtrs{}, counts[r], nullptr, C.images[r], sens_r, iters, false);
+    for (int r = 0; r < n_regions; ++r) {
+        tofmlem_ctx *sc = C.subs[r];
+        cudaStream_t rs = C.streams[r];
+        const float *sens_r = d_sens + (size_t)C.z0[r] * slice;
+        rc = iterate_device(sc, counts[r] ? ev_ptrs(&run_evs[r]) : EventPtrs{}, counts[r], nullptr, C.images[r], sens_r, iters, false);
         if (rc != TOFMLEM_OK) {
             ctx->err = sc->err;
             cudaDeviceSynchronize();
@@ -1688,7 +1758,6 @@ int tofmlem_reconstruct_regions(tofmlem_ctx *ctx, const tofmlem_events *ev, uint
             return rc;
         }
         RCU(cudaEventRecord(C.done[r], rs));
-        off += counts[r];
     }
     // R13: sum of the extended region images, overlapping margins add up.  R27: every region has seen all
     // the events that reach its core, so the cores alone tile the volume (margins discarded).
