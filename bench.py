@@ -241,6 +241,7 @@ def run_report(args):
         # own stream, the extended images summed; compared with the unsplit reconstruction (same x0 = mask).
         cfg = full
         n = args.events or cfg.n_events
+        it = args.division_iters or cfg.iters
         ev = synth.make_events_chunked(cfg, n, device=dev)
         sev, _, bin_ms = binned(base, ev, n)
         mx = sens.max()
@@ -249,17 +250,17 @@ def run_report(args):
         plan_ms = timed(lambda: base.plan_events(sev, n)) if args.tile else 0.0
         base.iterate(sev, n, whole, sens, 1)  # warm-up
         whole = x0.clone()
-        whole_ms = timed(lambda: base.iterate(sev, n, whole, sens, cfg.iters))
+        whole_ms = timed(lambda: base.iterate(sev, n, whole, sens, it))
         del sev
         base.trim()  # drop the unsplit plan's records
         split = torch.empty(nvox, dtype=torch.float32, device=dev)
         if args.region_plan >= 0:
             base.set_option(pkg.OPT_REGION_PLAN, args.region_plan)
-        base.reconstruct_regions(ev, n, 9, None, split, sens, 2)  # warm-up: builds the sub-contexts and scratch
+        base.reconstruct_regions(ev, n, 9, None, split, sens, it)  # warm-up: builds the sub-contexts and scratch
         split_runs = []
         for _ in range(5):
             t0 = time.perf_counter()
-            base.reconstruct_regions(ev, n, 9, None, split, sens, cfg.iters)  # synchronises
+            base.reconstruct_regions(ev, n, 9, None, split, sens, it)  # synchronises
             split_runs.append((time.perf_counter() - t0) * 1e3)
         split_ms = statistics.median(split_runs)
         region = torch.empty(n, dtype=torch.int32, device=dev)
@@ -283,11 +284,11 @@ def run_report(args):
             # the other reading of PAPER.md:101 (R27): an event in every region its window reaches, wide margins, cores only
             base.set_option(pkg.OPT_REGION_OVERLAP, 1)
             o = torch.empty(nvox, dtype=torch.float32, device=dev)
-            base.reconstruct_regions(ev, n, 9, None, o, sens, 2)  # warm-up (new sub-contexts: other margins)
+            base.reconstruct_regions(ev, n, 9, None, o, sens, it)  # warm-up (new sub-contexts: other margins)
             runs = []
             for _ in range(3):
                 t0 = time.perf_counter()
-                base.reconstruct_regions(ev, n, 9, None, o, sens, cfg.iters)
+                base.reconstruct_regions(ev, n, 9, None, o, sens, it)
                 runs.append((time.perf_counter() - t0) * 1e3)
             span = torch.empty(n, dtype=torch.int32, device=dev)
             oc = base.split_regions_overlap(ev, n, 9, None, span, None)
@@ -299,7 +300,7 @@ def run_report(args):
                     "rel_l2_region_interiors": float(dd[~near_v].norm() / w2[~near_v].norm()),
                     "rel_l2_within_margin_of_borders": float(dd[near_v].norm() / w2[near_v].norm())}
 
-        out["config"] = {"workload": f"cfg-4 division: {n} events of cfg-3, 9 regions, {cfg.iters} iterations each"}
+        out["config"] = {"workload": f"cfg-4 division: {n} events of cfg-3, 9 regions, {it} iterations each"}
         out.update({
             "unsplit_ms": whole_ms, "unsplit_bin_ms": bin_ms, "unsplit_plan_ms": plan_ms, "split_total_ms": split_ms,
             "split_runs_ms": split_runs,
@@ -484,6 +485,7 @@ def main():
     ap.add_argument("--concurrent", type=int, default=-1, help="TOFMLEM_OPT_CONCURRENT override")
     ap.add_argument("--l2-persist", type=int, default=-1, help="TOFMLEM_OPT_L2_PERSIST override")
     ap.add_argument("--region-plan", type=int, default=-1, help="TOFMLEM_OPT_REGION_PLAN override (division report)")
+    ap.add_argument("--division-iters", type=int, default=0, help="iterations of the division report (0 = the config's 5)")
     ap.add_argument("--sweep-events", default="10000000,146000000,500000000")
     ap.add_argument("--sweep-fwhm", default="100,300,600,0")
     args = ap.parse_args()

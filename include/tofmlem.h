@@ -142,12 +142,12 @@ enum {
                                        the ONE region that holds its TOF centre (bit-exact split), extended images summed;
                                        1 = reading R27, an event in every region its window reaches (1 or 2),
                                        wider margins, cores only */
-    TOFMLEM_OPT_REGION_PLAN = 17,   /* 1: tofmlem_reconstruct_regions plans every region's binned list (ray records + tiles;
+    TOFMLEM_OPT_REGION_PLAN = 17,   /* tofmlem_reconstruct_regions plans every region's binned list (ray records + tiles;
                                        48 B per event more scratch), the phases of the nine plans interleaved so that
-                                       the host waits twice in all; 0 (default): unplanned passes.  Measured at cfg-4,
-                                       5 iterations: 140.5 ms with plans against 142.4 ms without (184 ms when every plan
-                                       synchronised on its own) -- nine concurrent regions are not bound by their
-                                       iteration kernels, so the default stays 0. */
+                                       the host waits twice in all: 0 never, 1 always (when iters > 1), 2 (default) from
+                                       6 iterations on.  Measured at cfg-4: an iteration of the nine concurrent regions
+                                       takes 21.4 ms with plans against 25.1 ms without, the plans 14 ms: 5 iterations
+                                       141.5 against 142.3 ms, 9 iterations 226.9 against 242.6 ms. */
     TOFMLEM_OPT_DETERMINISTIC = 13, /* run-to-run bit-identical accumulation (the paper's LUT kernel "always
                                        generated an identically reconstructed image").  1: the iterations of
                                        tofmlem_iterate[_weighted] on a PLANNED list (tofmlem_plan_events; else

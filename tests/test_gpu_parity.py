@@ -442,6 +442,16 @@ def test_reconstruct_regions_parity(pkg):
             x = oracle.update(x, corr, sens_np[z0 * sl:z1 * sl], mask[z0 * sl:z1 * sl])
         total[z0 * sl:z1 * sl] += x
     check_image(out.cpu().numpy(), total)
+    # the same through per-region plans (ray records + tiles, TOFMLEM_OPT_REGION_PLAN = 1; tile thresholds lowered so that
+    # these small regions really run on tiles): the same image within the tolerance of the oracle comparison
+    ctx.set_option(pkg.OPT_REGION_PLAN, 1)
+    ctx.set_option(pkg.OPT_TILE_MIN_EVENTS, 64)
+    ctx.set_option(pkg.OPT_TILE_MIN_ITEMS, 1)
+    out2 = torch.empty(g.nvox, dtype=torch.float32, device="cuda")
+    ctx.reconstruct_regions(ev, n, R, None, out2, sens, iters)
+    check_image(out2.cpu().numpy(), total)
+    assert float((out2 - out).double().norm() / out.double().norm()) <= 1e-4
+    ctx.set_option(pkg.OPT_REGION_PLAN, 0)
     # unpinned (visual only): report how far the split result is from the unsplit one
     x = torch.from_numpy(mask.astype(np.float32)).cuda()
     ctx.iterate(ev, n, x, sens, iters)
