@@ -509,7 +509,7 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         CU(cudaEventRecord(ctx->t_ev[1], s));
         if (ctx->plan.direct_valid) {
             launch_em_planned(p, ctx->d_rec, n, ctx->d_chunk_list, ctx->plan.n_pieces, evw, d_image, d_corr, vec,
-                              ctx->d_stats, ctx->d_queues, n_sm, ds);
+                              ctx->d_stats, ctx->d_queues, n_sm, ctx->plan.n_items > 0, ds);
             CHECK_LAUNCH(1);
         }
         if (!conc) CU(cudaEventRecord(ctx->t_ev[2], s));

@@ -135,9 +135,10 @@ void read_plan_counters(const void *h_counters, uint64_t out[5]);  // ... and th
 void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &ev, const RecPtrs &rec, uint64_t n,
                             const float *image, float *fwd, cudaStream_t s);
 // pieces: n_pieces indices of the 32-event pieces of the list that hold work for this pass, ascending
+// sparse: the pieces are what a tile pass leaves over (the sparse bins), not a whole list
 void launch_em_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, const uint32_t *pieces, uint32_t n_pieces,
                        const float *evw, const float *image, float *corr, bool vec_ok, DeviceStats *stats,
-                       unsigned *queues, int n_sm, cudaStream_t s);
+                       unsigned *queues, int n_sm, bool sparse, cudaStream_t s);
 
 // reproducible accumulation (TOFMLEM_OPT_DETERMINISTIC): every event of the planned list, 64-bit integer correction image
 void launch_em_det(const ProjParams &p, const RecPtrs &rec, uint64_t n, const float *evw, const float *image,

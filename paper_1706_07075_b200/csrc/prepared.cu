@@ -614,13 +614,16 @@ void launch_planned_forward(const ProjParams &p, double sigma, const EventPtrs &
 template <bool VEC, bool BRICK>
 static void launch_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, const uint32_t *pieces, uint32_t n_pieces,
                            const float *evw, const float *image, float *corr, DeviceStats *stats, unsigned *queues,
-                           int n_sm, cudaStream_t s) {
+                           int n_sm, bool sparse, cudaStream_t s) {
     int per_sm = 0;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, em_planned_kernel<VEC, BRICK>, kBlock, 0);
     if (per_sm < 1) per_sm = 1;
     if (n_sm < 1) n_sm = 1;
     const double reach = 2.0 * p.half_window * sqrt(p.iv[0] * p.iv[0] + p.iv[1] * p.iv[1] + p.iv[2] * p.iv[2]);
-    const unsigned segs = reach > 80.0 ? 1u : (reach > 30.0 ? 3u : 4u);  // launch_em (projector.cu) has the measurements
+    // list segments per SM: as launch_em (projector.cu) measured them for whole lists; when the dense bins run on tiles
+    // the pieces left over are the sparse bins, whose warps gain nothing from several segments (measured at cfg-3 with
+    // 1 / 2 / 3 / 4 / 6 / 8 segments: 5.05 / 5.12 / 5.28 / 5.26 / 5.80 / 5.86 ms)
+    const unsigned segs = sparse ? 1u : (reach > 80.0 ? 1u : (reach > 30.0 ? 3u : 4u));
     unsigned nseg = (unsigned)n_sm * segs;
     if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / segs * segs;
     if (nseg % 61u == 0) nseg -= segs;
@@ -632,14 +635,14 @@ static void launch_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, 
 
 void launch_em_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, const uint32_t *pieces, uint32_t n_pieces,
                        const float *evw, const float *image, float *corr, bool vec_ok, DeviceStats *stats,
-                       unsigned *queues, int n_sm, cudaStream_t s) {
+                       unsigned *queues, int n_sm, bool sparse, cudaStream_t s) {
     if (n == 0 || n_pieces == 0) return;
     if (p.brick && vec_ok)
-        launch_planned<true, true>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<true, true>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, sparse, s);
     else if (vec_ok)
-        launch_planned<true, false>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<true, false>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, sparse, s);
     else
-        launch_planned<false, false>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, s);
+        launch_planned<false, false>(p, rec, n, pieces, n_pieces, evw, image, corr, stats, queues, n_sm, sparse, s);
 }
 
 }  // namespace tofmlem
