@@ -471,6 +471,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-bin", action="store_true", help="skip locality binning (for comparison)")
     ap.add_argument("--subbins", type=int, default=0, help="TOFMLEM_OPT_SUBBINS override (0 = library default)")
+    ap.add_argument("--tile-log2", type=int, default=0, help="TOFMLEM_OPT_TILE_LOG2 override (0 = library default, 3)")
     ap.add_argument("--em-variant", type=int, default=-1, help="TOFMLEM_OPT_EM_VARIANT override (-1 = library default)")
     ap.add_argument("--cache-share", type=int, default=-1, help="TOFMLEM_OPT_CACHE_SHARE override")
     ap.add_argument("--tile", type=int, default=1,
@@ -517,6 +518,8 @@ def main():
     ctx = pkg.Context(cfg.radius_mm, cfg.axial_mm, g, cfg.tof_fwhm_ps)
     if args.subbins:
         ctx.set_option(pkg.OPT_SUBBINS, args.subbins)
+    if args.tile_log2:
+        ctx.set_option(pkg.OPT_TILE_LOG2, args.tile_log2)
     if args.em_variant >= 0:
         ctx.set_option(pkg.OPT_EM_VARIANT, args.em_variant)
     if args.cache_share >= 0:
