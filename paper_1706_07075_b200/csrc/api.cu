@@ -515,7 +515,7 @@ int em_pass(tofmlem_ctx *ctx, const ProjParams &p_in, const EventPtrs &ev, uint6
         if (!conc) CU(cudaEventRecord(ctx->t_ev[2], s));
         if (ctx->plan.n_tiny) {  // kRecTiny: the unplanned walk (fp64 set-up), one event per piece
             launch_em_correction_chunks(p, true, ev, n, ctx->d_tiny, ctx->plan.n_tiny, evw, d_image, d_corr, vec,
-                                        ctx->d_stats, ctx->d_queues, ds);
+                                        ctx->d_stats, ctx->d_queues, ds, true);
             CHECK_LAUNCH(1);
         }
         if (conc) {

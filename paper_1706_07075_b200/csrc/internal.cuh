@@ -66,7 +66,8 @@ void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, ui
 // tile-mode pass leaves over); then n_chunks pieces are processed and `n` only bounds the event indices.
 void launch_em_correction_chunks(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const uint2 *chunks,
                                  uint32_t n_chunks, const float *evw, const float *image, float *corr, bool vec_ok,
-                                 DeviceStats *stats, unsigned *queues, cudaStream_t s);
+                                 DeviceStats *stats, unsigned *queues, cudaStream_t s,
+                                 bool gather /* the pieces are single events: a warp takes 32 of them, a lane each */);
 
 // ---- warpwalk.cu: a warp per LOR for whole chords (non-TOF); scratch = 2 (forward: 1) x nvox floats
 bool warp_walk_ok(const ProjParams &p);

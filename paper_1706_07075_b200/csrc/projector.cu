@@ -127,7 +127,8 @@ __global__ void __launch_bounds__(kBlock, 5) em_persistent_kernel(ProjParams P, 
                                                                float *__restrict__ corr, DeviceStats *stats,
                                                                unsigned *queues, unsigned nseg, unsigned per_seg,
                                                                unsigned segs_per_sm,
-                                                               const uint2 *__restrict__ chunks, unsigned n_chunks) {
+                                                               const uint2 *__restrict__ chunks, unsigned n_chunks,
+                                                               unsigned gather) {
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
     const unsigned lane = threadIdx.x & 31u;
@@ -147,7 +148,10 @@ __global__ void __launch_bounds__(kBlock, 5) em_persistent_kernel(ProjParams P, 
         bool valid;
         const uint64_t wc = (uint64_t)seg * per_seg + c;  // index of the warp's 32-event piece
         uint64_t e = wc * 32u + lane;
-        if (chunks) {  // the pieces come from a list (the events the tile-mode pass leaves over)
+        if (chunks && gather) {  // a list of single events: 32 of them per warp, a lane each
+            const uint64_t k = wc * 32u + lane;
+            e = k < n_chunks ? (uint64_t)__ldg(chunks + k).x : n;
+        } else if (chunks) {  // the pieces come from a list (the events the tile-mode pass leaves over)
             e = n;
             if (wc < n_chunks) {
                 const uint2 ch = __ldg(chunks + wc);
@@ -319,7 +323,7 @@ void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint
 template <bool TOF, bool VEC, bool BRICK>
 static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, const float *evw, const float *image,
                       float *corr, DeviceStats *stats, unsigned *queues, cudaStream_t s, const uint2 *chunks = nullptr,
-                      uint32_t n_chunks = 0) {
+                      uint32_t n_chunks = 0, bool gather = false) {
     if ((p.variant != 1 || chunks) && queues) {
         // SM count of the context's device (queried in tofmlem_create) and resident CTAs per SM of THIS instantiation on
         // the current device (a host-side table look-up in the runtime: asked on every launch, no cached state)
@@ -338,7 +342,7 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         unsigned segs = kSegsPerSm;
         unsigned nseg = (unsigned)n_sm * segs;
         unsigned grid = (unsigned)n_sm * (unsigned)(per_sm > 0 ? per_sm : 1);
-        const uint64_t wchunks = chunks ? (uint64_t)n_chunks : (n + 31) / 32;
+        const uint64_t wchunks = chunks ? (gather ? ((uint64_t)n_chunks + 31) / 32 : (uint64_t)n_chunks) : (n + 31) / 32;
         if (wchunks < 8ull * nseg) {
             // a short list (the sliver windows of a planned list: a few thousand one-event pieces): a few queues and CTAs
             // only -- a full-size launch spends 0.26 ms polling 444 empty queues
@@ -354,7 +358,7 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
         cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
         em_persistent_kernel<TOF, VEC, BRICK><<<grid, kBlock, 0, s>>>(
-            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, segs, chunks, n_chunks);
+            p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, segs, chunks, n_chunks, gather ? 1u : 0u);
     } else {
         em_correction_kernel<TOF, VEC, BRICK><<<grid_for(n, p.stride), kBlock, 0, s>>>(p, ev, n, evw, image, corr, stats);
     }
@@ -363,12 +367,12 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
 void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *evw,
                           const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,
                           cudaStream_t s) {
-    launch_em_correction_chunks(p, tof, ev, n, nullptr, 0, evw, image, corr, vec_ok, stats, queues, s);
+    launch_em_correction_chunks(p, tof, ev, n, nullptr, 0, evw, image, corr, vec_ok, stats, queues, s, false);
 }
 
 void launch_em_correction_chunks(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const uint2 *chunks,
                                  uint32_t n_chunks, const float *evw, const float *image, float *corr, bool vec_ok,
-                                 DeviceStats *stats, unsigned *queues, cudaStream_t s) {
+                                 DeviceStats *stats, unsigned *queues, cudaStream_t s, bool gather) {
     if (n == 0 || (chunks && n_chunks == 0)) return;
     if (p.variant == 2 && queues && vec_ok && !chunks) {
         if (tof) {
@@ -386,21 +390,21 @@ void launch_em_correction_chunks(const ProjParams &p, bool tof, const EventPtrs 
     }
     if (p.brick && vec_ok) {  // the brick layout exists only together with the 16-byte reductions
         if (tof)
-            launch_em<true, true, true>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
+            launch_em<true, true, true>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks, gather);
         else
-            launch_em<false, true, true>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
+            launch_em<false, true, true>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks, gather);
         return;
     }
     if (tof) {
         if (vec_ok)
-            launch_em<true, true, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
+            launch_em<true, true, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks, gather);
         else
-            launch_em<true, false, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
+            launch_em<true, false, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks, gather);
     } else {
         if (vec_ok)
-            launch_em<false, true, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
+            launch_em<false, true, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks, gather);
         else
-            launch_em<false, false, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks);
+            launch_em<false, false, false>(p, ev, n, evw, image, corr, stats, queues, s, chunks, n_chunks, gather);
     }
 }
 
