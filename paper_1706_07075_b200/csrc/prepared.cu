@@ -269,42 +269,36 @@ __device__ __forceinline__ RecRay rec_ray(const float4 &a, const float4 &b) {
     return RecRay{a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
 }
 
-// sum_j w_j image[j] (t units); the gather issued in one step is consumed in the next
+// sum_j w_j image[j] (t units); three steps per trip, each with its own (weight, value) slot: the gather issued in one step
+// is consumed three steps later
+#define TOFMLEM_GATHER_STEP(WS, VS)                        \
+    {                                                      \
+        const float tn = min3f(r.tx, r.ty, r.tz);          \
+        if (!(tn < r.te)) break;                           \
+        const float w = chord_weight(t, tn);               \
+        acc = fmaf(WS, VS, acc);                           \
+        VS = __ldg(image + idx);                           \
+        WS = w;                                            \
+        advance_axis(r.tx, idx, tn, r.dx, ix);             \
+        advance_axis(r.ty, idx, tn, r.dy, iy);             \
+        advance_axis(r.tz, idx, tn, r.dz, iz);             \
+        t = tn;                                            \
+    }
 __device__ __forceinline__ float rec_gather(RecRay r, int idx, int ix, int iy, int iz, const float *__restrict__ image) {
-    float acc = 0.f, wp = 0.f, vp = 0.f;
+    float acc = 0.f, w0 = 0.f, v0 = 0.f, w1 = 0.f, v1 = 0.f, w2 = 0.f, v2 = 0.f;
     float t = r.t;
     while (true) {
-        float t2;
-        {
-            const float tn = min3f(r.tx, r.ty, r.tz);
-            if (!(tn < r.te)) break;
-            const float w = chord_weight(t, tn);
-            acc = fmaf(wp, vp, acc);
-            vp = __ldg(image + idx);
-            wp = w;
-            advance_axis(r.tx, idx, tn, r.dx, ix);
-            advance_axis(r.ty, idx, tn, r.dy, iy);
-            advance_axis(r.tz, idx, tn, r.dz, iz);
-            t2 = tn;
-        }
-        t = t2;
-        {
-            const float tn = min3f(r.tx, r.ty, r.tz);
-            if (!(tn < r.te)) break;
-            const float w = chord_weight(t, tn);
-            acc = fmaf(wp, vp, acc);
-            vp = __ldg(image + idx);
-            wp = w;
-            advance_axis(r.tx, idx, tn, r.dx, ix);
-            advance_axis(r.ty, idx, tn, r.dy, iy);
-            advance_axis(r.tz, idx, tn, r.dz, iz);
-            t = tn;
-        }
+        TOFMLEM_GATHER_STEP(w0, v0)
+        TOFMLEM_GATHER_STEP(w1, v1)
+        TOFMLEM_GATHER_STEP(w2, v2)
     }
     const float w = chord_weight(t, r.te);
-    acc = fmaf(wp, vp, acc);
+    acc = fmaf(w0, v0, acc);
+    acc = fmaf(w1, v1, acc);
+    acc = fmaf(w2, v2, acc);
     return fmaf(w, __ldg(image + idx), acc);
 }
+#undef TOFMLEM_GATHER_STEP
 
 // if (tx <= tn) { tx += dx; idx += inc; inc = sum - inc; }   (brick layout: the index increment of a step alternates)
 __device__ __forceinline__ void advance_axis_alt(float &tx, int &idx, int &inc, float tn, float dx, int sum) {
