@@ -626,7 +626,7 @@ int tofmlem_create(const tofmlem_scanner *scanner, const tofmlem_grid *grid, flo
     }
     cudaError_t e = cudaMalloc(&ctx->d_max, sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, sizeof(DeviceStats));
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_queues, kMaxQueues * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_queues, (size_t)kMaxQueues * kQueueStride * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_rcounts, 2 * (kMaxRegions + 1) * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_flags, 2 * sizeof(unsigned));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_plan_counters, plan_counter_bytes());

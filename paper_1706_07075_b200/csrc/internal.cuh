@@ -57,6 +57,10 @@ void launch_backproject(const ProjParams &p, bool tof, const EventPtrs &ev, uint
                         float *out, bool vec_ok, cudaStream_t s);
 // queues: kMaxQueues work counters owned by the context (persistent variant), may be NULL
 constexpr int kMaxQueues = 2048;
+// the counters of kernels that space them kQueueStride words apart (one 128-byte line each: 148 counters side by side sit in
+// five lines, i.e. on a few L2 slices, which then carry every warp's polling and atomics); the array holds
+// kMaxQueues * kQueueStride words
+constexpr int kQueueStride = 32;
 // evw: optional per-event weights (NEXT-3), NULL => 1
 void launch_em_correction(const ProjParams &p, bool tof, const EventPtrs &ev, uint64_t n, const float *evw,
                           const float *image, float *corr, bool vec_ok, DeviceStats *stats, unsigned *queues,

@@ -421,7 +421,8 @@ em_planned_kernel(RecPtrs rec, uint64_t n, int nx, int ny, const uint32_t *__res
     unsigned seg = smid % base + base * ((threadIdx.x >> 5) % segs_per_sm), tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
-        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        if (lane == 0 && *(volatile unsigned *)(queues + seg * kQueueStride) < per_seg)
+            c = atomicAdd(queues + seg * kQueueStride, 1u);
         c = __shfl_sync(0xffffffffu, c, 0);
         if (c >= per_seg) {
             if (++tries >= nseg) break;
@@ -492,7 +493,8 @@ em_det_kernel(RecPtrs rec, uint64_t n, int nx, int ny, const float *__restrict__
     unsigned seg = smid % nseg, tries = 0, nv = 0, vis = 0;
     while (true) {
         unsigned c = per_seg;
-        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        if (lane == 0 && *(volatile unsigned *)(queues + seg * kQueueStride) < per_seg)
+            c = atomicAdd(queues + seg * kQueueStride, 1u);
         c = __shfl_sync(0xffffffffu, c, 0);
         if (c >= per_seg) {
             if (++tries >= nseg) break;
@@ -554,7 +556,7 @@ void launch_em_det(const ProjParams &p, const RecPtrs &rec, uint64_t n, const fl
     if (nseg % 61u == 0) nseg -= 1;
     const uint64_t n_pieces = (n + 31) / 32;
     const unsigned per_seg = (unsigned)((n_pieces + nseg - 1) / nseg);
-    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    cudaMemsetAsync(queues, 0, (size_t)nseg * kQueueStride * sizeof(unsigned), s);
     em_det_kernel<<<n_sm * per_sm, kBlock, 0, s>>>(rec, n, p.n[0], p.n[1], evw, image, corr_q, gscale, stats, queues, nseg,
                                                    per_seg);
 }
@@ -622,7 +624,7 @@ static void launch_planned(const ProjParams &p, const RecPtrs &rec, uint64_t n, 
     if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / segs * segs;
     if (nseg % 61u == 0) nseg -= segs;
     const unsigned per_seg = (n_pieces + nseg - 1) / nseg;
-    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    cudaMemsetAsync(queues, 0, (size_t)nseg * kQueueStride * sizeof(unsigned), s);
     em_planned_kernel<VEC, BRICK><<<n_sm * per_sm, kBlock, 0, s>>>(rec, n, p.n[0], p.n[1], pieces, n_pieces, evw, image,
                                                                   corr, stats, queues, nseg, per_seg, segs);
 }

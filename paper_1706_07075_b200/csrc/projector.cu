@@ -137,7 +137,8 @@ __global__ void __launch_bounds__(kBlock, 5) em_persistent_kernel(ProjParams P, 
     unsigned seg = smid % base + base * ((threadIdx.x >> 5) % segs_per_sm), tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
-        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        if (lane == 0 && *(volatile unsigned *)(queues + seg * kQueueStride) < per_seg)
+            c = atomicAdd(queues + seg * kQueueStride, 1u);
         c = __shfl_sync(0xffffffffu, c, 0);
         if (c >= per_seg) {
             if (++tries >= nseg) break;
@@ -220,7 +221,8 @@ __global__ void __launch_bounds__(kCachedBlock, 1) em_cached_kernel(ProjParams P
     unsigned seg = blockIdx.x % nseg, tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
-        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        if (lane == 0 && *(volatile unsigned *)(queues + seg * kQueueStride) < per_seg)
+            c = atomicAdd(queues + seg * kQueueStride, 1u);
         c = __shfl_sync(0xffffffffu, c, 0);
         if (c >= per_seg) {
             if (++tries >= nseg) break;
@@ -283,7 +285,7 @@ static void launch_em_cached(const ProjParams &p, const EventPtrs &ev, uint64_t 
     if (nseg % 61u == 0) nseg -= 1;
     const uint64_t wchunks = (n + 31) / 32;
     const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
-    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    cudaMemsetAsync(queues, 0, (size_t)nseg * kQueueStride * sizeof(unsigned), s);
     em_cached_kernel<TOF, BRICK><<<n_sm, kCachedBlock, smem, s>>>(p, ev, n, evw, image, corr, stats, queues, nseg,
                                                                  per_seg);
 }
@@ -356,7 +358,7 @@ static void launch_em(const ProjParams &p, const EventPtrs &ev, uint64_t n, cons
         if (nseg > (unsigned)kMaxQueues) nseg = (unsigned)kMaxQueues / segs * segs;
         if (nseg > segs && nseg % 61u == 0) nseg -= segs;  // the stealing stride 61 must not divide the number of segments
         const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
-        cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+        cudaMemsetAsync(queues, 0, (size_t)nseg * kQueueStride * sizeof(unsigned), s);
         em_persistent_kernel<TOF, VEC, BRICK><<<grid, kBlock, 0, s>>>(
             p, ev, n, evw, image, corr, stats, queues, nseg, per_seg, segs, chunks, n_chunks, gather ? 1u : 0u);
     } else {

@@ -235,7 +235,8 @@ __global__ void __launch_bounds__(kBlock) sampled_em_kernel(ProjParams P, const 
     unsigned seg = smid % base + base * ((threadIdx.x >> 5) % segs_per_sm), tries = 0, nv = 0, vis = 0, nr = 0;
     while (true) {
         unsigned c = per_seg;
-        if (lane == 0 && *(volatile unsigned *)(queues + seg) < per_seg) c = atomicAdd(queues + seg, 1u);
+        if (lane == 0 && *(volatile unsigned *)(queues + seg * kQueueStride) < per_seg)
+            c = atomicAdd(queues + seg * kQueueStride, 1u);
         c = __shfl_sync(0xffffffffu, c, 0);
         if (c >= per_seg) {
             if (++tries >= nseg) break;
@@ -291,7 +292,7 @@ void launch_sampled_em(const ProjParams &p, const SampleLutEntry *lut, int K, co
     if (nseg % 61u == 0) nseg -= kSegsPerSm;
     const uint64_t wchunks = (n + 31) / 32;
     const unsigned per_seg = (unsigned)((wchunks + nseg - 1) / nseg);
-    cudaMemsetAsync(queues, 0, nseg * sizeof(unsigned), s);
+    cudaMemsetAsync(queues, 0, (size_t)nseg * kQueueStride * sizeof(unsigned), s);
     sampled_em_kernel<<<n_sm * (per_sm > 0 ? per_sm : 1), kBlock, 0, s>>>(p, lut, K, ev, n, evw, image, corr, stats,
                                                                         queues, nseg, per_seg, kSegsPerSm);
 }
