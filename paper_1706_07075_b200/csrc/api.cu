@@ -131,6 +131,8 @@ struct tofmlem_ctx {
         TileGeom g{};
         std::vector<TileItem> items;
         std::vector<TileRange> ranges;
+        std::vector<uint64_t> start;
+        std::vector<uint8_t> state;
         unsigned flags[2] = {0, 0};
         uint32_t n_pieces = 0;
         std::vector<unsigned char> hc;
@@ -1225,34 +1227,51 @@ int plan_build(tofmlem_ctx *ctx) {
             const uint32_t Tx = (uint32_t)((ctx->grid.nx + t - 1) >> ctx->tile_log2),
                            Ty = (uint32_t)((ctx->grid.ny + t - 1) >> ctx->tile_log2),
                            Tz = (uint32_t)((ctx->grid.nz + t - 1) >> ctx->tile_log2), T3 = Tx * Ty * Tz;
-            std::vector<uint64_t> start(nb + 1);
-            uint64_t off = 0;
-            for (uint32_t b = 0; b < nb; ++b) {
-                start[b] = off;
-                off += cnt[b];
-            }
-            start[nb] = off;
-            std::vector<uint8_t> state(nb, 0);  // 0: direct, 1: item (first cube or single), 2: second cube of a pair
-            for (uint32_t b = 0; b < nb; ++b) {
-                const uint32_t c = cnt[b];
-                if (c == 0 || state[b]) continue;
-                const uint32_t D = b / T3, tl = b - D * T3, a = D >> 2;
-                const uint32_t step = a == 0 ? 1u : (a == 1 ? Tx : Tx * Ty);
-                const uint32_t ca = a == 0 ? tl % Tx : (a == 1 ? (tl / Tx) % Ty : tl / (Tx * Ty));
-                const uint32_t na = a == 0 ? Tx : (a == 1 ? Ty : Tz);
-                const uint32_t b2 = b + step;
-                const uint32_t c2 = (g.pairs && ca + 1 < na && !state[b2]) ? cnt[b2] : 0u;
-                if (c2 > 0 && c + c2 >= thr && c + c2 <= mx) {
-                    state[b] = 1;
-                    state[b2] = 2;
-                    items.push_back(TileItem{(uint32_t)start[b], c, (uint32_t)start[b2], c2, b, 1u, 0u, 0u});
-                } else if (c >= thr) {
-                    state[b] = 1;
-                    const uint32_t pieces = (c + mx - 1) / mx;
-                    uint32_t per = (c + pieces - 1) / pieces;
-                    per = (per + 31u) & ~31u;
-                    for (uint32_t k = 0; k < c; k += per)
-                        items.push_back(TileItem{(uint32_t)(start[b] + k), c - k < per ? c - k : per, 0u, 0u, b, 0u, 0u, 0u});
+            const auto add_pieces = [&](uint64_t first, uint32_t c, uint32_t b) {
+                const uint32_t pieces = (c + mx - 1) / mx;
+                uint32_t per = (c + pieces - 1) / pieces;
+                per = (per + 31u) & ~31u;
+                for (uint32_t k = 0; k < c; k += per)
+                    items.push_back(TileItem{(uint32_t)(first + k), c - k < per ? c - k : per, 0u, 0u, b, 0u, 0u, 0u});
+            };
+            if (!g.pairs) {
+                // no pair items (they do not fit at this window length): one pass over the bin counts with a running offset
+                // (the general form below costs 4 ms of host time at 384 k bins: an array of bin starts, and four integer
+                // divisions per bin to find its neighbour along the dominant axis)
+                uint64_t off = 0;
+                for (uint32_t b = 0; b < nb; ++b) {
+                    const uint32_t c = cnt[b];
+                    if (c >= thr) add_pieces(off, c, b);
+                    off += c;
+                }
+            } else {
+                std::vector<uint64_t> &start = J.start;  // kept by the job: no fresh pages per plan
+                start.resize((size_t)nb + 1);
+                uint64_t off = 0;
+                for (uint32_t b = 0; b < nb; ++b) {
+                    start[b] = off;
+                    off += cnt[b];
+                }
+                start[nb] = off;
+                std::vector<uint8_t> &state = J.state;  // 0: direct, 1: item (first cube or single), 2: second cube of a pair
+                state.assign(nb, 0);
+                for (uint32_t b = 0; b < nb; ++b) {
+                    const uint32_t c = cnt[b];
+                    if (c == 0 || state[b]) continue;
+                    const uint32_t D = b / T3, tl = b - D * T3, a = D >> 2;
+                    const uint32_t step = a == 0 ? 1u : (a == 1 ? Tx : Tx * Ty);
+                    const uint32_t ca = a == 0 ? tl % Tx : (a == 1 ? (tl / Tx) % Ty : tl / (Tx * Ty));
+                    const uint32_t na = a == 0 ? Tx : (a == 1 ? Ty : Tz);
+                    const uint32_t b2 = b + step;
+                    const uint32_t c2 = (ca + 1 < na && !state[b2]) ? cnt[b2] : 0u;
+                    if (c2 > 0 && c + c2 >= thr && c + c2 <= mx) {
+                        state[b] = 1;
+                        state[b2] = 2;
+                        items.push_back(TileItem{(uint32_t)start[b], c, (uint32_t)start[b2], c2, b, 1u, 0u, 0u});
+                    } else if (c >= thr) {
+                        state[b] = 1;
+                        add_pieces(start[b], c, b);
+                    }
                 }
             }
             // the items' event ranges in list order: the record set-up finds the item of an event by bisection
@@ -1260,7 +1279,9 @@ int plan_build(tofmlem_ctx *ctx) {
                 ranges.push_back(TileRange{items[i].start, items[i].count, (uint32_t)i, 0u});
                 if (items[i].count2) ranges.push_back(TileRange{items[i].start2, items[i].count2, (uint32_t)i, 0u});
             }
-            std::sort(ranges.begin(), ranges.end(), [](const TileRange &x, const TileRange &y) { return x.start < y.start; });
+            // single-cube items come out in list order already; only the second cubes of pair items break it
+            if (!std::is_sorted(ranges.begin(), ranges.end(), [](const TileRange &x, const TileRange &y) { return x.start < y.start; }))
+                std::sort(ranges.begin(), ranges.end(), [](const TileRange &x, const TileRange &y) { return x.start < y.start; });
         }
     }
     // too few items to fill the GPU twice over: the tile pass would run on a fraction of the SMs before the direct pass
