@@ -110,6 +110,7 @@ struct PlanCounters {
 };
 
 __device__ __forceinline__ int sel3i(int a, int v0, int v1, int v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
+__device__ __forceinline__ float sel3f(int a, float v0, float v1, float v2) { return a == 0 ? v0 : (a == 1 ? v1 : v2); }
 
 __global__ void __launch_bounds__(kBlock)
 prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2, EventPtrs ev, uint64_t n,
@@ -172,29 +173,35 @@ prepare_rays_kernel(ProjParams P, const TileGeom *__restrict__ Gp, int tile_log2
                 };
                 bool fit = inside();
                 const int p0 = p, lf0 = fit ? nf - lof[p] : 0, ls0 = fit ? ns - los[p] : 0;
-                float ta = r.t0[a], tf = r.t0[f], tsl = r.t0[s];
+                // (selects, not r.t0[a]: a run-time index would put the arrays into local memory)
+                const float t0a = sel3f(a, r.t0[0], r.t0[1], r.t0[2]), t0f = sel3f(f, r.t0[0], r.t0[1], r.t0[2]),
+                            t0s = sel3f(s, r.t0[0], r.t0[1], r.t0[2]);
+                const float tda = sel3f(a, r.td[0], r.td[1], r.td[2]), tdf = sel3f(f, r.td[0], r.td[1], r.td[2]),
+                            tds = sel3f(s, r.td[0], r.td[1], r.td[2]);
+                float ta = t0a, tf = t0f, tsl = t0s;
                 unsigned nvis = 1;
                 while (fit) {
                     const float tn = min3f(ta, tf, tsl);
                     if (!(tn < r.te)) break;
-                    if (ta <= tn) { ta += r.td[a]; p += da; }
-                    if (tf <= tn) { tf += r.td[f]; nf += df; }
-                    if (tsl <= tn) { tsl += r.td[s]; ns += ds; }
+                    if (ta <= tn) { ta += tda; p += da; }
+                    if (tf <= tn) { tf += tdf; nf += df; }
+                    if (tsl <= tn) { tsl += tds; ns += ds; }
                     ++nvis;
                     fit = inside();
                 }
                 if (fit) {
                     tile = true;
                     visits = nvis;
-                    ra = make_float4(r.ts, r.te, r.t0[a], r.t0[f]);
-                    rb = make_float4(r.t0[s], r.td[a], r.td[f], r.td[s]);
+                    ra = make_float4(r.ts, r.te, t0a, t0f);
+                    rb = make_float4(t0s, tda, tdf, tds);
                     const unsigned li0 = (unsigned)(p0 * PS + ls0 * Wf + lf0);
                     rc.x = (unsigned)idx0;
                     rc.y = kRecValid | kRecTile | ((unsigned)a << kRecAxisShift) | (da < 0 ? kRecNeg0 : 0u) |
                            (df < 0 ? kRecNeg1 : 0u) | (ds < 0 ? kRecNeg2 : 0u) | ((unsigned)p0 << kRecPlaneShift) |
                            (li0 << kRecLiShift);
                     rc.z = nvis;
-                    rc.w = (g.neg[a] ? 1u : 0u) | (g.neg[f] ? 2u : 0u) | (g.neg[s] ? 4u : 0u);  // grid directions
+                    rc.w = (sel3i(a, g.neg[0], g.neg[1], g.neg[2]) ? 1u : 0u) | (sel3i(f, g.neg[0], g.neg[1], g.neg[2]) ? 2u : 0u) |
+                           (sel3i(s, g.neg[0], g.neg[1], g.neg[2]) ? 4u : 0u);  // grid directions
                 } else {
                     straggler = true;
                 }
